@@ -1,0 +1,158 @@
+/*
+ * cola.h -- C ABI of the B200-native COLA hot path (libcola.so).
+ *
+ * What it is.  The paper (arxiv 2302.00850, PAPER.md; "P:n" = line n) describes a GPU "fermion
+ * matrix inverter" (conjugate gradient, mixed precision: 32-bit inner, 64-bit outer),
+ * one lattice site per thread, written in CUDA and called from Fortran through ISO-C-binding
+ * C-callable routines.  This header is that boundary.  The operator is fixed by
+ * BASELINE.json north_star (BJ:ns) and written out in SURVEY.md section 8(c) O1..O8 / DESIGN.md:
+ *
+ *     M = A - kappa*D                                  Wilson-clover, kappa normalisation, r = 1
+ *     (D psi)(x) = sum_mu [ eta+ (1-gamma_mu) U_mu(x) psi(x+mu) + eta- (1+gamma_mu) U_mu(x-mu)^+ psi(x-mu) ]
+ *     A(x) = 1 - kappa*csw*sum_{mu<nu} sigma_{mu nu} F_{mu nu}(x)     (two 6x6 Hermitian chiral blocks)
+ *     S = A_ee - kappa^2 D_eo A_oo^{-1} D_oe           even-odd Schur complement on even sites
+ *     K^+ = gamma_5 K gamma_5 for K = M, S
+ *
+ * General rules.
+ *   - No torch types, no C++ types: plain pointers and sizes.  Every pointer argument says whether
+ *     it is a HOST or a DEVICE pointer.  Device memory is owned by the caller (PyTorch tensors);
+ *     the library allocates no device memory except a 4 KB control block: gauge field, clover
+ *     field and solver vectors live in the caller-provided workspace (cola_set_workspace), which
+ *     the context borrows until cola_destroy / the next cola_set_workspace.
+ *   - Every function returns a cola_status and never throws or aborts across the ABI; a message
+ *     for the last failure on a context is available from cola_last_error.
+ *   - Operator applications are asynchronous on the context's stream.  cola_gauge_upload*,
+ *     cola_cg_solve* and every *_host entry point synchronise that stream before returning.
+ *   - Lattice: dims = (Lx, Ly, Lz, Lt), each even and >= 2.  V = Lx*Ly*Lz*Lt, Vh = V/2.
+ *     Site index i(x) = x + Lx*(y + Ly*(z + Lz*t)); parity = (x+y+z+t) mod 2 (0 = even).
+ *   - Canonical arrays (what the caller sees), complex = (re, im) pairs, C order:
+ *         links   U[t][z][y][x][mu][a][b]   fp64     (U psi)_a = sum_b U_ab psi_b, mu = x,y,z,t
+ *         spinor  psi[t][z][y][x][s][c]     fp64 or fp32 (complex128 / complex64)
+ *         clover  A[t][z][y][x][12][12]     fp64, row = 3*s + c
+ *   - Internal arrays (what the kernels see): parity-split structure of arrays of 16-byte chunks,
+ *     site index fastest:   spinor[parity][chunk][Vh]  with chunk = 2 (fp64) or 4 (fp32) reals,
+ *     24 reals per site in canonical (s, c, re/im) order.  A "half-lattice" internal buffer is one
+ *     parity of that (cola_spinor_bytes(.., full=0) bytes); a full internal buffer is the even
+ *     half followed by the odd half.
+ */
+#ifndef COLA_H
+#define COLA_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cola_ctx cola_ctx;   /* opaque; created by cola_create, owned by the library */
+
+typedef enum {
+    COLA_OK = 0,
+    COLA_EINVAL = 1,     /* bad argument (odd extent, NULL pointer, non-unitary links with compress12, ...) */
+    COLA_ECUDA = 2,      /* a CUDA call or kernel failed; cola_last_error has the CUDA message */
+    COLA_ENOTREADY = 3,  /* operator/solver called before cola_set_workspace + cola_gauge_upload */
+    COLA_ENOCONV = 4,    /* cola_cg_solve hit max_iter; info is filled, x holds the last iterate */
+    COLA_ENOMEM = 5      /* workspace too small */
+} cola_status;
+
+typedef enum { COLA_F64 = 0, COLA_F32 = 1 } cola_prec;
+typedef enum { COLA_EVEN = 0, COLA_ODD = 1 } cola_parity;
+
+typedef struct {
+    int dims[4];        /* Lx, Ly, Lz, Lt: each even, >= 2 */
+    double kappa;       /* hopping parameter */
+    double csw;         /* clover coefficient */
+    int bc[4];          /* +1 periodic / -1 antiperiodic per direction; the configs use {+1,+1,+1,-1} */
+    int compress12;     /* 1: fp32 links stored as 12 reals, third row rebuilt in registers (BJ:ns);
+                           0: fp32 links stored as 18 reals.  fp64 links are always 18 reals. */
+    int trace_sub;      /* 1 (default reading): remove the trace of F_{mu nu} */
+    int device;         /* CUDA device ordinal */
+    void *stream;       /* cudaStream_t to launch on (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
+} cola_params;
+
+/* Create a context for one lattice.  HOST pointers.  COLA_EINVAL for odd / too small extents or
+ * bc not in {+1,-1}; COLA_ECUDA if the device cannot be selected. */
+cola_status cola_create(cola_ctx **out, const cola_params *p);
+cola_status cola_destroy(cola_ctx *c);
+/* Message of the last failure on c (valid until the next call on c); "" if none.  c may be NULL
+ * (returns the message of the last failed cola_create in this thread). */
+const char *cola_last_error(const cola_ctx *c);
+/* Change the stream subsequent calls launch on. */
+cola_status cola_set_stream(cola_ctx *c, void *stream);
+
+/* Bytes of one internal spinor buffer: full != 0 -> V sites, else Vh sites. */
+size_t cola_spinor_bytes(const cola_ctx *c, cola_prec prec, int full);
+/* Bytes of workspace the context needs (gauge fp64 + fp32, clover A both parities and A^-1 on the
+ * odd parity in fp64 + fp32, solver vectors, staging). */
+size_t cola_workspace_bytes(const cola_ctx *c);
+/* Lend `bytes` of DEVICE memory (256-byte aligned) to the context.  COLA_ENOMEM if too small.
+ * Invalidates a previously uploaded gauge field. */
+cola_status cola_set_workspace(cola_ctx *c, void *dev_ptr, size_t bytes);
+
+/* H0-H2: upload canonical fp64 links, reorder to the internal parity-split SoA
+ * (fp64 18 reals; fp32 18 or 12 reals), build the clover field A from the four-leaf field
+ * strength, invert its 6x6 blocks on the odd parity, make fp32 copies.  Links stay pure SU(3)
+ * (no boundary sign folded in).  host_links: HOST pointer, 4*V*18 doubles.
+ * With compress12, links with max|U U^+ - 1| > 1e-10 are rejected with COLA_EINVAL. */
+cola_status cola_gauge_upload(cola_ctx *c, const double *host_links);
+/* Same, from a DEVICE pointer (e.g. links generated on the GPU for the 64^3x128 case). */
+cola_status cola_gauge_upload_dev(cola_ctx *c, const double *dev_links);
+/* Diagnostics of the last upload: max |U U^+ - 1| over all links. */
+cola_status cola_gauge_info(const cola_ctx *c, double *max_unitarity_dev);
+
+/* Tests of H1/H2: expand the packed fp64 clover field to canonical 12x12 blocks.
+ * which = 0: A on all sites.  which = 1: A^-1 on odd sites, zero blocks on even sites.
+ * canon_dev: DEVICE pointer, V*144 complex128. */
+cola_status cola_clover_unpack(cola_ctx *c, int which, void *canon_dev);
+
+/* Canonical DEVICE spinor (complex128 for COLA_F64, complex64 for COLA_F32) <-> full internal
+ * DEVICE buffer of the same precision. */
+cola_status cola_spinor_pack(cola_ctx *c, cola_prec prec, const void *canon_dev, void *internal_dev);
+cola_status cola_spinor_unpack(cola_ctx *c, cola_prec prec, const void *internal_dev, void *canon_dev);
+/* Internal fp64 <-> internal fp32 (round to nearest even), n_half = 1 (half lattice) or 2 (full). */
+cola_status cola_spinor_convert(cola_ctx *c, cola_prec dst_prec, const void *src_dev, void *dst_dev, int n_half);
+
+/* H3-H5, parity dslash: out_p = D_{p,1-p} in_{1-p}.  in, out: internal half-lattice DEVICE buffers
+ * (in holds parity 1-p, out receives parity p); they must not overlap. */
+cola_status cola_dslash_apply(cola_ctx *c, cola_prec prec, cola_parity out_parity, const void *in_dev, void *out_dev);
+/* H7: out = M in (dagger != 0: M^+ in).  Full internal DEVICE buffers, no overlap. */
+cola_status cola_fermion_matrix_apply(cola_ctx *c, cola_prec prec, int dagger, const void *in_full_dev, void *out_full_dev);
+/* H8: out_e = S in_e (dagger != 0: S^+).  Half-lattice (even) internal DEVICE buffers, no overlap.
+ * Uses the context's odd half-lattice temporary. */
+cola_status cola_schur_apply(cola_ctx *c, cola_prec prec, int dagger, const void *in_even_dev, void *out_even_dev);
+
+typedef struct {
+    double tol;        /* stop when |r| <= tol*|b| (1e-10 in the configs); r is the residual of the system
+                          being iterated (M x = b, or S x_e = bhat_e whose residual equals the full one) */
+    int max_iter;      /* CGLS passes (one K and one K^+ each) */
+    int even_odd;      /* 0: CGNR on M (BJ:c0); 1: CGNR on the Schur complement + reconstruction */
+    int mixed;         /* 0: all fp64; 1: fp32 inner iteration with fp64 reliable updates */
+    double delta;      /* reliable-update threshold (mixed only); <= 0 selects the default 0.1 */
+} cola_solve_params;
+
+typedef struct {
+    int iters;                 /* CGLS passes done */
+    int reliable_updates;      /* fp64 residual recomputations (mixed only) */
+    double iterated_residual;  /* |r|/|b| of the recurrence (fp64 after the last reliable update) */
+    double true_residual;      /* |b - M x|/|b| recomputed in fp64 on the full lattice */
+    double seconds;            /* device time of the whole solve incl. source preparation and
+                                  reconstruction, measured with CUDA events on the context's stream */
+    double op_flops;           /* counted operator flops (1320/site dslash, 504/site clover, 48 xpay) */
+} cola_solve_info;
+
+/* H9-H12: solve M x = b.  b_canon_dev / x_canon_dev: canonical complex128 DEVICE arrays, V sites.
+ * Returns COLA_OK, or COLA_ENOCONV with info filled and x = last iterate. */
+cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info);
+
+/* End-to-end variants: HOST canonical buffers; the host<->device copies are part of the call. */
+cola_status cola_dslash_apply_host(cola_ctx *c, cola_prec prec, cola_parity out_parity, const void *in_canon_host, void *out_canon_host);
+cola_status cola_fermion_matrix_apply_host(cola_ctx *c, cola_prec prec, int dagger, const void *in_canon_host, void *out_canon_host);
+cola_status cola_cg_solve_host(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_host, void *x_canon_host, cola_solve_info *info);
+
+/* Benchmark aid: number of kernels this context has launched since creation. */
+unsigned long long cola_launch_count(const cola_ctx *c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COLA_H */

@@ -1,0 +1,301 @@
+"""Thin ctypes binding of libcola.so (include/cola.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA library; torch is used for device memory and streams.
+There is no CPU fallback: if libcola.so is missing or cannot be loaded, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libcola.so")
+
+COLA_OK, COLA_EINVAL, COLA_ECUDA, COLA_ENOTREADY, COLA_ENOCONV, COLA_ENOMEM = range(6)
+COLA_F64, COLA_F32 = 0, 1
+COLA_EVEN, COLA_ODD = 0, 1
+STATUS_NAMES = {0: "COLA_OK", 1: "COLA_EINVAL", 2: "COLA_ECUDA", 3: "COLA_ENOTREADY", 4: "COLA_ENOCONV", 5: "COLA_ENOMEM"}
+
+EXPORTS = [
+    "cola_create", "cola_destroy", "cola_last_error", "cola_set_stream", "cola_spinor_bytes",
+    "cola_workspace_bytes", "cola_set_workspace", "cola_gauge_upload", "cola_gauge_upload_dev",
+    "cola_gauge_info", "cola_clover_unpack", "cola_spinor_pack", "cola_spinor_unpack",
+    "cola_spinor_convert", "cola_dslash_apply", "cola_fermion_matrix_apply", "cola_schur_apply",
+    "cola_cg_solve", "cola_dslash_apply_host", "cola_fermion_matrix_apply_host", "cola_cg_solve_host",
+    "cola_launch_count",
+]
+
+
+class ColaParams(ctypes.Structure):
+    _fields_ = [
+        ("dims", ctypes.c_int * 4), ("kappa", ctypes.c_double), ("csw", ctypes.c_double),
+        ("bc", ctypes.c_int * 4), ("compress12", ctypes.c_int), ("trace_sub", ctypes.c_int),
+        ("device", ctypes.c_int), ("stream", ctypes.c_void_p),
+    ]
+
+
+class ColaSolveParams(ctypes.Structure):
+    _fields_ = [("tol", ctypes.c_double), ("max_iter", ctypes.c_int), ("even_odd", ctypes.c_int),
+                ("mixed", ctypes.c_int), ("delta", ctypes.c_double)]
+
+
+class ColaSolveInfo(ctypes.Structure):
+    _fields_ = [("iters", ctypes.c_int), ("reliable_updates", ctypes.c_int),
+                ("iterated_residual", ctypes.c_double), ("true_residual", ctypes.c_double),
+                ("seconds", ctypes.c_double), ("op_flops", ctypes.c_double)]
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def _load():
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_2302_00850_b200.build` "
+            "(there is no CPU fallback for the COLA hot path)")
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    lib.cola_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(ColaParams)]
+    lib.cola_destroy.argtypes = [vp]
+    lib.cola_last_error.argtypes = [vp]
+    lib.cola_last_error.restype = ctypes.c_char_p
+    lib.cola_set_stream.argtypes = [vp, vp]
+    lib.cola_spinor_bytes.argtypes = [vp, ci, ci]
+    lib.cola_spinor_bytes.restype = ctypes.c_size_t
+    lib.cola_workspace_bytes.argtypes = [vp]
+    lib.cola_workspace_bytes.restype = ctypes.c_size_t
+    lib.cola_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
+    lib.cola_gauge_upload.argtypes = [vp, vp]
+    lib.cola_gauge_upload_dev.argtypes = [vp, vp]
+    lib.cola_gauge_info.argtypes = [vp, ctypes.POINTER(cd)]
+    lib.cola_clover_unpack.argtypes = [vp, ci, vp]
+    lib.cola_spinor_pack.argtypes = [vp, ci, vp, vp]
+    lib.cola_spinor_unpack.argtypes = [vp, ci, vp, vp]
+    lib.cola_spinor_convert.argtypes = [vp, ci, vp, vp, ci]
+    lib.cola_dslash_apply.argtypes = [vp, ci, ci, vp, vp]
+    lib.cola_fermion_matrix_apply.argtypes = [vp, ci, ci, vp, vp]
+    lib.cola_schur_apply.argtypes = [vp, ci, ci, vp, vp]
+    lib.cola_cg_solve.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo)]
+    lib.cola_dslash_apply_host.argtypes = [vp, ci, ci, vp, vp]
+    lib.cola_fermion_matrix_apply_host.argtypes = [vp, ci, ci, vp, vp]
+    lib.cola_cg_solve_host.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo)]
+    lib.cola_launch_count.argtypes = [vp]
+    lib.cola_launch_count.restype = ctypes.c_ulonglong
+    for name in EXPORTS:
+        fn = getattr(lib, name)
+        if name not in ("cola_last_error", "cola_spinor_bytes", "cola_workspace_bytes", "cola_launch_count"):
+            fn.restype = ci
+    return lib
+
+
+_lib = _load()
+
+
+class ColaError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {message}")
+        self.status = status
+
+
+_PREC = {torch.float64: COLA_F64, torch.float32: COLA_F32, torch.complex128: COLA_F64, torch.complex64: COLA_F32,
+         "f64": COLA_F64, "f32": COLA_F32, COLA_F64: COLA_F64, COLA_F32: COLA_F32}
+_REAL = {COLA_F64: torch.float64, COLA_F32: torch.float32}
+_CPLX = {COLA_F64: torch.complex128, COLA_F32: torch.complex64}
+
+
+class Cola:
+    """One lattice context.  Method names mirror the C entry points (cola_<name>)."""
+
+    def __init__(self, dims, kappa, csw, bc=(1, 1, 1, -1), compress12=True, trace_sub=True, device=0, stream=None):
+        self.dims = tuple(int(d) for d in dims)
+        self.device = torch.device("cuda", device)
+        self._h = ctypes.c_void_p()
+        self._ws = None
+        p = ColaParams()
+        p.dims[:] = self.dims
+        p.kappa, p.csw = float(kappa), float(csw)
+        p.bc[:] = [int(b) for b in bc]
+        p.compress12, p.trace_sub, p.device = int(bool(compress12)), int(bool(trace_sub)), int(device)
+        if stream is None and torch.cuda.is_available():
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+        p.stream = ctypes.c_void_p(stream or 0)
+        st = _lib.cola_create(ctypes.byref(self._h), ctypes.byref(p))
+        if st != COLA_OK:
+            raise ColaError(st, _lib.cola_last_error(None).decode())
+        lx, ly, lz, lt = self.dims
+        self.V = lx * ly * lz * lt
+        self.Vh = self.V // 2
+        self.kappa, self.csw = float(kappa), float(csw)
+
+    # ---- plumbing
+    def _ck(self, st, ok=(COLA_OK,)):
+        if st not in ok:
+            raise ColaError(st, _lib.cola_last_error(self._h).decode())
+        return st
+
+    def close(self):
+        if self._h:
+            _lib.cola_destroy(self._h)
+            self._h = ctypes.c_void_p()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_stream(self, stream):
+        self._ck(_lib.cola_set_stream(self._h, ctypes.c_void_p(stream)))
+
+    def spinor_bytes(self, prec, full=True) -> int:
+        return int(_lib.cola_spinor_bytes(self._h, _PREC[prec], int(full)))
+
+    def workspace_bytes(self) -> int:
+        return int(_lib.cola_workspace_bytes(self._h))
+
+    def set_workspace(self, tensor: torch.Tensor | None = None):
+        """Lend a device buffer to the context (allocated here with torch if not given)."""
+        if tensor is None:
+            tensor = torch.empty(self.workspace_bytes(), dtype=torch.uint8, device=self.device)
+        self._ck(_lib.cola_set_workspace(self._h, ctypes.c_void_p(tensor.data_ptr()), tensor.numel() * tensor.element_size()))
+        self._ws = tensor
+        return tensor
+
+    def launch_count(self) -> int:
+        return int(_lib.cola_launch_count(self._h))
+
+    # ---- internal buffers (torch owns the memory; shapes mirror the SoA layout)
+    def empty_internal(self, prec, full=True) -> torch.Tensor:
+        pr = _PREC[prec]
+        n = 2 if pr == COLA_F64 else 4
+        shape = (2, 24 // n, self.Vh, n) if full else (24 // n, self.Vh, n)
+        return torch.empty(shape, dtype=_REAL[pr], device=self.device)
+
+    # ---- H0-H2
+    def gauge_upload(self, links: torch.Tensor):
+        """links: complex128 [t][z][y][x][4][3][3]; a CPU tensor goes through cola_gauge_upload,
+        a CUDA tensor through cola_gauge_upload_dev."""
+        if self._ws is None:
+            self.set_workspace()
+        if links.dtype != torch.complex128 or links.numel() != self.V * 36:
+            raise ValueError("links must be complex128 with 4*V*9 entries")
+        links = links.contiguous()
+        if links.is_cuda:
+            self._ck(_lib.cola_gauge_upload_dev(self._h, ctypes.c_void_p(links.data_ptr())))
+        else:
+            self._ck(_lib.cola_gauge_upload(self._h, ctypes.c_void_p(links.data_ptr())))
+
+    def gauge_upload_dev(self, links: torch.Tensor):
+        assert links.is_cuda
+        self.gauge_upload(links)
+
+    def gauge_info(self) -> float:
+        v = ctypes.c_double()
+        self._ck(_lib.cola_gauge_info(self._h, ctypes.byref(v)))
+        return v.value
+
+    def clover_unpack(self, which: int) -> torch.Tensor:
+        lx, ly, lz, lt = self.dims
+        out = torch.empty((lt, lz, ly, lx, 12, 12), dtype=torch.complex128, device=self.device)
+        self._ck(_lib.cola_clover_unpack(self._h, int(which), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    # ---- layout
+    def spinor_pack(self, canon: torch.Tensor) -> torch.Tensor:
+        pr = _PREC[canon.dtype]
+        canon = canon.contiguous()
+        assert canon.is_cuda and canon.numel() == self.V * 12
+        out = self.empty_internal(pr, full=True)
+        self._ck(_lib.cola_spinor_pack(self._h, pr, ctypes.c_void_p(canon.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def spinor_unpack(self, internal: torch.Tensor) -> torch.Tensor:
+        pr = _PREC[internal.dtype]
+        assert internal.is_cuda and internal.is_contiguous() and internal.numel() == self.V * 24
+        lx, ly, lz, lt = self.dims
+        out = torch.empty((lt, lz, ly, lx, 4, 3), dtype=_CPLX[pr], device=self.device)
+        self._ck(_lib.cola_spinor_unpack(self._h, pr, ctypes.c_void_p(internal.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def spinor_convert(self, src: torch.Tensor, dst_prec) -> torch.Tensor:
+        dp = _PREC[dst_prec]
+        assert src.is_cuda and src.is_contiguous()
+        full = src.dim() == 4
+        out = self.empty_internal(dp, full=full)
+        self._ck(_lib.cola_spinor_convert(self._h, dp, ctypes.c_void_p(src.data_ptr()), ctypes.c_void_p(out.data_ptr()), 2 if full else 1))
+        return out
+
+    # ---- H3-H8
+    def dslash_apply(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        pr = _PREC[inp.dtype]
+        assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.Vh * 24
+        if out is None:
+            out = self.empty_internal(pr, full=False)
+        self._ck(_lib.cola_dslash_apply(self._h, pr, int(out_parity), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def fermion_matrix_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
+        pr = _PREC[inp.dtype]
+        assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.V * 24
+        if out is None:
+            out = self.empty_internal(pr, full=True)
+        self._ck(_lib.cola_fermion_matrix_apply(self._h, pr, int(bool(dagger)), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def schur_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
+        pr = _PREC[inp.dtype]
+        assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.Vh * 24
+        if out is None:
+            out = self.empty_internal(pr, full=False)
+        self._ck(_lib.cola_schur_apply(self._h, pr, int(bool(dagger)), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    # ---- H9-H12
+    @staticmethod
+    def _solve_params(tol, max_iter, even_odd, mixed, delta):
+        sp = ColaSolveParams()
+        sp.tol, sp.max_iter, sp.even_odd, sp.mixed, sp.delta = float(tol), int(max_iter), int(bool(even_odd)), int(bool(mixed)), float(delta)
+        return sp
+
+    @staticmethod
+    def _info_dict(info, st):
+        return dict(iters=info.iters, reliable_updates=info.reliable_updates, iterated_residual=info.iterated_residual,
+                    true_residual=info.true_residual, seconds=info.seconds, op_flops=info.op_flops, converged=(st == COLA_OK))
+
+    def cg_solve(self, b: torch.Tensor, tol=1e-10, max_iter=20000, even_odd=True, mixed=False, delta=0.1, x: torch.Tensor | None = None):
+        """b: canonical complex128 [t][z][y][x][4][3].  A CUDA tensor goes through cola_cg_solve, a CPU
+        tensor (ideally pinned) through cola_cg_solve_host.  Returns (x, info dict)."""
+        assert b.dtype == torch.complex128 and b.numel() == self.V * 12
+        b = b.contiguous()
+        if x is None:
+            x = torch.empty_like(b, pin_memory=True) if not b.is_cuda else torch.empty_like(b)
+        sp = self._solve_params(tol, max_iter, even_odd, mixed, delta)
+        info = ColaSolveInfo()
+        fn = _lib.cola_cg_solve if b.is_cuda else _lib.cola_cg_solve_host
+        st = fn(self._h, ctypes.byref(sp), ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), ctypes.byref(info))
+        self._ck(st, ok=(COLA_OK, COLA_ENOCONV))
+        return x, self._info_dict(info, st)
+
+    def cg_solve_host(self, b: torch.Tensor, **kw):
+        assert not b.is_cuda
+        return self.cg_solve(b, **kw)
+
+    def dslash_apply_host(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        pr = _PREC[inp.dtype]
+        assert not inp.is_cuda and inp.is_contiguous() and inp.numel() == self.V * 12
+        if out is None:
+            out = torch.empty_like(inp, pin_memory=True)
+        self._ck(_lib.cola_dslash_apply_host(self._h, pr, int(out_parity), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def fermion_matrix_apply_host(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
+        pr = _PREC[inp.dtype]
+        assert not inp.is_cuda and inp.is_contiguous() and inp.numel() == self.V * 12
+        if out is None:
+            out = torch.empty_like(inp, pin_memory=True)
+        self._ck(_lib.cola_fermion_matrix_apply_host(self._h, pr, int(bool(dagger)), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out

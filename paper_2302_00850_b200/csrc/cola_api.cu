@@ -1,0 +1,671 @@
+// cola_api.cu -- the C ABI of include/cola.h: context, workspace carving, gauge upload (H0-H2),
+// operator entry points (H3-H8) and the CGNR / mixed-precision solvers (H9-H12).
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "cola_internal.h"
+
+using namespace cola;
+
+struct cola_ctx {
+    cola_params p;
+    Geom g;
+    size_t V, Vh;
+    cudaStream_t stream;
+    char err[512];
+    int fmt32;
+    // borrowed workspace, carved in cola_set_workspace
+    char *ws;
+    size_t ws_bytes;
+    char *gauge64, *gauge32;        // [parity][mu][chunk][Vh]
+    char *clovA64, *clovA32;        // [parity][chunk][Vh]
+    char *clovI64, *clovI32;        // odd parity only
+    char *tmp64, *tmp32;            // odd half-lattice temporaries of the Schur operator
+    double *partials;
+    char *scratch;                  // solver vectors / staging
+    size_t scratch_bytes;
+    // owned
+    Ctl *ctl;                       // device
+    unsigned long long *max_dev_bits;   // device (inside the same allocation)
+    double *h_pinned;               // pinned host scalars
+    cudaEvent_t ev0, ev1;
+    int ready;
+    double max_unitarity_dev;
+    unsigned long long launches;
+};
+
+static thread_local char g_create_err[512] = "";
+
+static cola_status fail(cola_ctx *c, cola_status st, const char *fmt, const char *a = "", const char *b = "")
+{
+    char *dst = c ? c->err : g_create_err;
+    snprintf(dst, 512, fmt, a, b);
+    return st;
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess) return fail(c, COLA_ECUDA, "%s: %s", #call, cudaGetErrorString(e__)); \
+    } while (0)
+#define ST(call)                          \
+    do {                                  \
+        cola_status s__ = (call);         \
+        if (s__ != COLA_OK) return s__;   \
+    } while (0)
+
+static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+static size_t half_bytes(const cola_ctx *c, cola_prec prec) { return c->Vh * 24 * (prec == COLA_F64 ? 8 : 4); }
+static const size_t SCRATCH_HALF64 = 12;   // solver scratch in units of one fp64 half-lattice spinor
+
+struct Carve {
+    size_t gauge64, gauge32, clovA64, clovA32, clovI64, clovI32, tmp64, tmp32, partials, scratch, total;
+};
+
+static Carve carve(const cola_ctx *c)
+{
+    Carve k;
+    size_t off = 0;
+    const size_t Vh = c->Vh;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    k.gauge64 = take(8 * 144 * Vh);
+    k.gauge32 = take(8 * link_bytes(c->fmt32) * Vh);
+    k.clovA64 = take(2 * 576 * Vh);
+    k.clovA32 = take(2 * 288 * Vh);
+    k.clovI64 = take(576 * Vh);
+    k.clovI32 = take(288 * Vh);
+    k.tmp64 = take(192 * Vh);
+    k.tmp32 = take(96 * Vh);
+    k.partials = take(((Vh + 127) / 128 + 4096) * sizeof(double));
+    k.scratch = take(SCRATCH_HALF64 * 192 * Vh);
+    k.total = off;
+    return k;
+}
+
+extern "C" {
+
+cola_status cola_create(cola_ctx **out, const cola_params *p)
+{
+    cola_ctx *c = nullptr;
+    if (!out || !p) return fail(nullptr, COLA_EINVAL, "cola_create: NULL argument");
+    *out = nullptr;
+    for (int k = 0; k < 4; k++) {
+        if (p->dims[k] < 2 || (p->dims[k] & 1)) return fail(nullptr, COLA_EINVAL, "cola_create: every extent must be even and >= 2");
+        if (p->bc[k] != 1 && p->bc[k] != -1) return fail(nullptr, COLA_EINVAL, "cola_create: bc must be +1 or -1");
+    }
+    const double vol = (double)p->dims[0] * p->dims[1] * p->dims[2] * p->dims[3];
+    if (vol / 2 > 2.0e9) return fail(nullptr, COLA_EINVAL, "cola_create: half volume exceeds 32-bit site indices");
+    {
+        cudaError_t e = cudaSetDevice(p->device);
+        if (e != cudaSuccess) return fail(nullptr, COLA_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e));
+    }
+    c = new cola_ctx();
+    memset(c, 0, sizeof(*c));
+    c->p = *p;
+    c->g.X = p->dims[0]; c->g.Y = p->dims[1]; c->g.Z = p->dims[2]; c->g.T = p->dims[3];
+    c->g.Xh = p->dims[0] / 2;
+    c->V = (size_t)vol;
+    c->Vh = c->V / 2;
+    c->g.Vh = (int)c->Vh;
+    for (int k = 0; k < 4; k++) c->g.bc[k] = p->bc[k];
+    c->fmt32 = p->compress12 ? LINK_F32_12 : LINK_F32_18;
+    c->stream = (cudaStream_t)p->stream;
+    char *blk = nullptr;
+    cudaError_t e = cudaMalloc(&blk, 4096);
+    if (e == cudaSuccess) e = cudaMemset(blk, 0, 4096);
+    if (e == cudaSuccess) e = cudaHostAlloc(&c->h_pinned, 256, cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    if (e != cudaSuccess) {
+        fail(nullptr, COLA_ECUDA, "cola_create: %s", cudaGetErrorString(e));
+        if (blk) cudaFree(blk);
+        delete c;
+        return COLA_ECUDA;
+    }
+    c->ctl = reinterpret_cast<Ctl *>(blk);
+    c->max_dev_bits = reinterpret_cast<unsigned long long *>(blk + 2048);
+    *out = c;
+    return COLA_OK;
+}
+
+cola_status cola_destroy(cola_ctx *c)
+{
+    if (!c) return COLA_OK;
+    cudaSetDevice(c->p.device);
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->ctl);
+    cudaFreeHost(c->h_pinned);
+    cudaEventDestroy(c->ev0);
+    cudaEventDestroy(c->ev1);
+    delete c;
+    return COLA_OK;
+}
+
+const char *cola_last_error(const cola_ctx *c) { return c ? c->err : g_create_err; }
+
+cola_status cola_set_stream(cola_ctx *c, void *stream)
+{
+    if (!c) return COLA_EINVAL;
+    c->stream = (cudaStream_t)stream;
+    return COLA_OK;
+}
+
+size_t cola_spinor_bytes(const cola_ctx *c, cola_prec prec, int full)
+{
+    if (!c) return 0;
+    return half_bytes(c, prec) * (full ? 2 : 1);
+}
+
+size_t cola_workspace_bytes(const cola_ctx *c) { return c ? carve(c).total : 0; }
+
+cola_status cola_set_workspace(cola_ctx *c, void *dev_ptr, size_t bytes)
+{
+    if (!c) return COLA_EINVAL;
+    c->ready = 0;
+    if (!dev_ptr || ((uintptr_t)dev_ptr & 255)) return fail(c, COLA_EINVAL, "cola_set_workspace: pointer must be non-NULL and 256-byte aligned");
+    const Carve k = carve(c);
+    if (bytes < k.total) return fail(c, COLA_ENOMEM, "cola_set_workspace: workspace smaller than cola_workspace_bytes()");
+    c->ws = (char *)dev_ptr;
+    c->ws_bytes = bytes;
+    c->gauge64 = c->ws + k.gauge64; c->gauge32 = c->ws + k.gauge32;
+    c->clovA64 = c->ws + k.clovA64; c->clovA32 = c->ws + k.clovA32;
+    c->clovI64 = c->ws + k.clovI64; c->clovI32 = c->ws + k.clovI32;
+    c->tmp64 = c->ws + k.tmp64; c->tmp32 = c->ws + k.tmp32;
+    c->partials = (double *)(c->ws + k.partials);
+    c->scratch = c->ws + k.scratch;
+    c->scratch_bytes = SCRATCH_HALF64 * 192 * c->Vh;
+    return COLA_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// internal helpers
+// ------------------------------------------------------------------------------------------------
+static cola_status need_ready(cola_ctx *c, const char *who)
+{
+    if (!c) return COLA_EINVAL;
+    if (!c->ws) return fail(c, COLA_ENOTREADY, "%s: no workspace (call cola_set_workspace)", who);
+    if (!c->ready) return fail(c, COLA_ENOTREADY, "%s: no gauge field (call cola_gauge_upload)", who);
+    return COLA_OK;
+}
+
+static int fmt_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? (int)LINK_F64_18 : c->fmt32; }
+static char *gauge_of(const cola_ctx *c, cola_prec prec, int parity)
+{
+    return prec == COLA_F64 ? c->gauge64 + (size_t)parity * 4 * 144 * c->Vh : c->gauge32 + (size_t)parity * 4 * link_bytes(c->fmt32) * c->Vh;
+}
+static char *clovA_of(const cola_ctx *c, cola_prec prec, int parity)
+{
+    return prec == COLA_F64 ? c->clovA64 + (size_t)parity * 576 * c->Vh : c->clovA32 + (size_t)parity * 288 * c->Vh;
+}
+static char *clovI_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? c->clovI64 : c->clovI32; }
+static char *tmp_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? c->tmp64 : c->tmp32; }
+
+// out_p = [post] ( [A] y + coef * D_{p,1-p} in ), optional |out|^2 -> norm_out
+static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, const void *in, void *out, const void *y, int clov_on_y,
+                          double coef, int post_inv, double *norm_out, int norm_accumulate)
+{
+    DslashArgs a;
+    memset(&a, 0, sizeof(a));
+    a.g = c->g;
+    a.in = in;
+    a.out = out;
+    a.gauge_p = gauge_of(c, prec, parity);
+    a.gauge_q = gauge_of(c, prec, 1 - parity);
+    a.y = y;
+    a.clov_y = (y && clov_on_y) ? clovA_of(c, prec, parity) : nullptr;
+    a.clov_post = post_inv ? clovI_of(c, prec) : nullptr;
+    a.coef = coef;
+    a.sgn = dagger ? +1.0 : -1.0;
+    a.parity = parity;
+    if (norm_out) {
+        a.partials = c->partials;
+        a.counter = &c->ctl->counter[0];
+        a.norm_out = norm_out;
+        a.norm_accumulate = norm_accumulate;
+    }
+    if (post_inv && parity != 1) return fail(c, COLA_EINVAL, "internal: A^-1 is stored on the odd parity only");
+    CK(launch_dslash(fmt_of(c, prec), a, c->stream));
+    c->launches++;
+    return COLA_OK;
+}
+
+// out_e = S in_e  (2 launches; norm of the result optional)
+static cola_status schur(cola_ctx *c, cola_prec prec, int dagger, const void *in_e, void *out_e, double *norm_out)
+{
+    const double k = c->p.kappa;
+    ST(dslash(c, prec, 1, dagger, in_e, tmp_of(c, prec), nullptr, 0, 0.0, 1, nullptr, 0));          // t_o = A_oo^-1 D_oe x_e
+    ST(dslash(c, prec, 0, dagger, tmp_of(c, prec), out_e, in_e, 1, -k * k, 0, norm_out, 0));        // A_ee x_e - k^2 D_eo t_o
+    return COLA_OK;
+}
+
+// out = M in on the full lattice (2 launches)
+static cola_status fmatrix(cola_ctx *c, cola_prec prec, int dagger, const void *in, void *out, double *norm_out)
+{
+    const size_t hb = half_bytes(c, prec);
+    const char *in_e = (const char *)in, *in_o = in_e + hb;
+    char *out_e = (char *)out, *out_o = out_e + hb;
+    ST(dslash(c, prec, 0, dagger, in_o, out_e, in_e, 1, -c->p.kappa, 0, norm_out, 0));
+    ST(dslash(c, prec, 1, dagger, in_e, out_o, in_o, 1, -c->p.kappa, 0, norm_out, 1));
+    return COLA_OK;
+}
+
+static cola_status read_scalar(cola_ctx *c, const double *dev, double *host)
+{
+    CK(cudaMemcpyAsync(c->h_pinned, dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    *host = c->h_pinned[0];
+    return COLA_OK;
+}
+
+static cola_status norm2(cola_ctx *c, cola_prec prec, const void *v, size_t n_sites, double *dev_out)
+{
+    CK(launch_norm2(prec, v, n_sites, c->partials, &c->ctl->counter[2], dev_out, c->stream));
+    c->launches++;
+    return COLA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// gauge upload (H0-H2)
+// ------------------------------------------------------------------------------------------------
+static cola_status gauge_finish(cola_ctx *c)
+{
+    unsigned long long bits = 0;
+    CK(cudaMemcpyAsync(&bits, c->max_dev_bits, sizeof(bits), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    memcpy(&c->max_unitarity_dev, &bits, sizeof(double));
+    if (c->p.compress12 && !(c->max_unitarity_dev <= 1e-10))
+        return fail(c, COLA_EINVAL, "cola_gauge_upload: links are not unitary to 1e-10; 12-real compression would be wrong");
+    CK(launch_clover_build(c->g, c->gauge64, c->p.kappa * c->p.csw, c->p.trace_sub, c->clovA64, c->clovA32, c->stream));
+    CK(launch_clover_invert(c->g, c->clovA64 + 576 * c->Vh, c->clovI64, c->clovI32, c->stream));
+    c->launches += 2;
+    CK(cudaStreamSynchronize(c->stream));
+    c->ready = 1;
+    return COLA_OK;
+}
+
+static cola_status gauge_upload_impl(cola_ctx *c, const double *links, int on_host)
+{
+    if (!c) return COLA_EINVAL;
+    if (!links) return fail(c, COLA_EINVAL, "cola_gauge_upload: NULL links");
+    if (!c->ws) return fail(c, COLA_ENOTREADY, "cola_gauge_upload: no workspace (call cola_set_workspace)");
+    CK(cudaSetDevice(c->p.device));
+    c->ready = 0;
+    CK(cudaMemsetAsync(c->max_dev_bits, 0, sizeof(unsigned long long), c->stream));
+    if (!on_host) {
+        CK(launch_gauge_reorder(c->g, links, 0, (long)c->V, c->gauge64, c->gauge32, c->fmt32, c->max_dev_bits, c->stream));
+        c->launches++;
+        return gauge_finish(c);
+    }
+    const size_t per_site = 4 * 18 * sizeof(double);
+    size_t chunk_sites = c->scratch_bytes / per_site;
+    if (chunk_sites > c->V) chunk_sites = c->V;
+    for (size_t lo = 0; lo < c->V; lo += chunk_sites) {
+        const size_t n = (c->V - lo < chunk_sites) ? c->V - lo : chunk_sites;
+        CK(cudaMemcpyAsync(c->scratch, links + lo * 72, n * per_site, cudaMemcpyHostToDevice, c->stream));
+        CK(launch_gauge_reorder(c->g, (const double *)c->scratch, (long)lo, (long)n, c->gauge64, c->gauge32, c->fmt32, c->max_dev_bits, c->stream));
+        c->launches++;
+    }
+    return gauge_finish(c);
+}
+
+// ------------------------------------------------------------------------------------------------
+// solvers (H9-H12)
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+struct System {            // K x = rhs on n_sites sites; K = S (even_odd) or M
+    int even_odd;
+    size_t n_sites;
+};
+
+cola_status apply_K(cola_ctx *c, const System &sy, cola_prec prec, int dagger, const void *in, void *out, double *norm_out)
+{
+    return sy.even_odd ? schur(c, prec, dagger, in, out, norm_out) : fmatrix(c, prec, dagger, in, out, norm_out);
+}
+
+size_t vec_bytes(const cola_ctx *c, const System &sy, cola_prec prec) { return half_bytes(c, prec) * (sy.even_odd ? 1 : 2); }
+
+// out64 = a*A + b*B with an optional fp32 copy; per half lattice because the fp64<->fp32 chunk
+// pairing of the internal layout is per half
+cola_status axpby64(cola_ctx *c, const System &sy, void *out64, double a, const void *A, double b, const void *B, void *out32)
+{
+    const int nh = sy.even_odd ? 1 : 2;
+    for (int h = 0; h < nh; h++) {
+        const size_t o64 = h * half_bytes(c, COLA_F64), o32 = h * half_bytes(c, COLA_F32);
+        CK(launch_axpby64((char *)out64 + o64, a, (const char *)A + o64, b, B ? (const char *)B + o64 : nullptr,
+                          out32 ? (char *)out32 + o32 : nullptr, c->Vh, nullptr, nullptr, nullptr, c->stream));
+        c->launches++;
+    }
+    return COLA_OK;
+}
+
+}  // namespace
+
+static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info)
+{
+    ST(need_ready(c, "cola_cg_solve"));
+    if (!sp || !b_canon_dev || !x_canon_dev || !info) return fail(c, COLA_EINVAL, "cola_cg_solve: NULL argument");
+    if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve: tol must be > 0 and max_iter >= 1");
+    CK(cudaSetDevice(c->p.device));
+    memset(info, 0, sizeof(*info));
+    const double delta = sp->delta > 0 ? sp->delta : 0.1;
+    const double kappa = c->p.kappa;
+    const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32);
+    System sy;
+    sy.even_odd = sp->even_odd ? 1 : 0;
+    sy.n_sites = sy.even_odd ? c->Vh : c->V;
+    const size_t nv64 = vec_bytes(c, sy, COLA_F64), nv32 = vec_bytes(c, sy, COLA_F32);
+    const double flops_K = sy.even_odd ? 3696.0 * (double)c->Vh : 1872.0 * (double)c->V;
+    double flops = 0.0;
+
+    // scratch carving (units of fp64 half vectors; SCRATCH_HALF64 = 12 covers the worst case)
+    char *sc = c->scratch;
+    char *B = sc; sc += 2 * h64;          // packed source, full lattice
+    char *X = sc; sc += 2 * h64;          // solution, full lattice (x_e is its even half)
+    char *rhs, *r, *p = nullptr, *qs;
+    char *x32 = nullptr, *r32 = nullptr, *p32 = nullptr, *qs32 = nullptr;
+    if (sy.even_odd) { rhs = sc; sc += h64; } else rhs = B;
+    r = sc; sc += nv64;
+    qs = sc; sc += nv64;
+    if (!sp->mixed) { p = sc; sc += nv64; }
+    else {
+        x32 = sc; sc += nv32;
+        r32 = sc; sc += nv32;
+        p32 = sc; sc += nv32;
+        qs32 = sc; sc += nv32;
+    }
+    if ((size_t)(sc - c->scratch) > c->scratch_bytes) return fail(c, COLA_ENOMEM, "cola_cg_solve: internal scratch too small");
+    char *xsol = X;                       // x of the iterated system (even half of X, or all of X)
+
+    Ctl *ctl = c->ctl;
+    CK(cudaEventRecord(c->ev0, c->stream));
+    CK(launch_spinor_pack(COLA_F64, c->g, b_canon_dev, B, c->stream));
+    c->launches++;
+    double bb = 0.0;
+    ST(norm2(c, COLA_F64, B, c->V, &ctl->aux[2]));
+    ST(read_scalar(c, &ctl->aux[2], &bb));
+    CK(cudaMemsetAsync(X, 0, 2 * h64, c->stream));
+    const double bnorm = sqrt(bb);
+    int status_conv = 0;
+    double rr = 0.0;
+    int iters = 0, updates = 0;
+
+    if (bb > 0.0) {
+        if (sy.even_odd) {
+            // bhat_e = b_e + kappa D_eo A_oo^-1 b_o
+            CK(launch_clover_apply(COLA_F64, c->g, c->clovI64, B + h64, c->tmp64, c->stream));
+            c->launches++;
+            ST(dslash(c, COLA_F64, 0, 0, c->tmp64, rhs, B, 0, kappa, 0, nullptr, 0));
+            flops += (504.0 + 1320.0 + 48.0) * (double)c->Vh;
+        }
+        const double target = sp->tol * bnorm;
+        if (!sp->mixed) {
+            // ---- fp64 CGLS
+            CK(cudaMemcpyAsync(r, rhs, nv64, cudaMemcpyDeviceToDevice, c->stream));
+            ST(apply_K(c, sy, COLA_F64, 1, r, qs, &ctl->gam[0]));
+            CK(cudaMemcpyAsync(p, qs, nv64, cudaMemcpyDeviceToDevice, c->stream));
+            flops += flops_K;
+            ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
+            ST(read_scalar(c, &ctl->rr, &rr));
+            status_conv = sqrt(rr) <= target;
+            for (int k = 0; !status_conv && k < sp->max_iter; k++) {
+                const int cur = k & 1;
+                ST(apply_K(c, sy, COLA_F64, 0, p, qs, &ctl->qq));
+                CK(launch_r_update(COLA_F64, r, qs, ctl, cur, sy.n_sites, c->partials, c->stream));
+                c->launches++;
+                ST(read_scalar(c, &ctl->rr, &rr));
+                iters = k + 1;
+                flops += flops_K;
+                if (sqrt(rr) <= target) {
+                    CK(launch_xp_update(COLA_F64, xsol, p, qs, ctl, cur, 1, 0, sy.n_sites, c->stream));
+                    c->launches++;
+                    status_conv = 1;
+                    break;
+                }
+                ST(apply_K(c, sy, COLA_F64, 1, r, qs, &ctl->gam[cur ^ 1]));
+                flops += flops_K;
+                const int last = (k + 1 == sp->max_iter);
+                CK(launch_xp_update(COLA_F64, xsol, p, qs, ctl, cur, 1, last ? 0 : 1, sy.n_sites, c->stream));
+                c->launches++;
+            }
+        } else {
+            // ---- mixed precision: fp32 CGLS with fp64 reliable updates, search direction kept
+            CK(cudaMemsetAsync(x32, 0, nv32, c->stream));
+            ST(axpby64(c, sy, r, 1.0, rhs, 0.0, nullptr, r32));         // r64 = rhs, r32 = float(r64)
+            ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
+            ST(read_scalar(c, &ctl->rr, &rr));
+            double rmax = sqrt(rr);
+            status_conv = sqrt(rr) <= target;
+            if (!status_conv) {
+                ST(apply_K(c, sy, COLA_F32, 1, r32, qs32, &ctl->gam[0]));
+                CK(cudaMemcpyAsync(p32, qs32, nv32, cudaMemcpyDeviceToDevice, c->stream));
+                flops += flops_K;
+            }
+            for (int k = 0; !status_conv && k < sp->max_iter; k++) {
+                const int cur = k & 1;
+                ST(apply_K(c, sy, COLA_F32, 0, p32, qs32, &ctl->qq));
+                CK(launch_r_update(COLA_F32, r32, qs32, ctl, cur, sy.n_sites, c->partials, c->stream));
+                c->launches++;
+                ST(read_scalar(c, &ctl->rr, &rr));
+                iters = k + 1;
+                flops += flops_K;
+                double rn = sqrt(rr);
+                if (rn > rmax) rmax = rn;
+                int x_done = 0;
+                if (rn < delta * rmax || rn <= target) {
+                    // reliable update: x64 += x32 (+ the pending alpha p), r64 = rhs - K x64 in fp64
+                    CK(launch_xp_update(COLA_F32, x32, p32, qs32, ctl, cur, 1, 0, sy.n_sites, c->stream));
+                    c->launches++;
+                    x_done = 1;
+                    for (int h = 0; h < (sy.even_odd ? 1 : 2); h++) {
+                        CK(launch_accumulate(xsol + h * h64, x32 + h * h32, c->Vh, c->stream));
+                        c->launches++;
+                    }
+                    ST(apply_K(c, sy, COLA_F64, 0, xsol, qs, nullptr));
+                    flops += flops_K;
+                    ST(axpby64(c, sy, r, 1.0, rhs, -1.0, qs, r32));
+                    ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
+                    ST(read_scalar(c, &ctl->rr, &rr));
+                    rn = sqrt(rr);
+                    rmax = rn;
+                    updates++;
+                    if (rn <= target) { status_conv = 1; break; }
+                }
+                ST(apply_K(c, sy, COLA_F32, 1, r32, qs32, &ctl->gam[cur ^ 1]));
+                flops += flops_K;
+                const int last = (k + 1 == sp->max_iter);
+                if (!x_done || !last) {
+                    CK(launch_xp_update(COLA_F32, x32, p32, qs32, ctl, cur, x_done ? 0 : 1, last ? 0 : 1, sy.n_sites, c->stream));
+                    c->launches++;
+                }
+            }
+            if (!status_conv) {   // max_iter: fold the fp32 part into the fp64 iterate
+                for (int h = 0; h < (sy.even_odd ? 1 : 2); h++) {
+                    CK(launch_accumulate(xsol + h * h64, x32 + h * h32, c->Vh, c->stream));
+                    c->launches++;
+                }
+            }
+        }
+        if (sy.even_odd) {
+            // x_o = A_oo^-1 (b_o + kappa D_oe x_e)
+            ST(dslash(c, COLA_F64, 1, 0, X, X + h64, B + h64, 0, kappa, 1, nullptr, 0));
+            flops += (1320.0 + 48.0 + 504.0) * (double)c->Vh;
+        }
+    } else {
+        status_conv = 1;
+    }
+    info->iterated_residual = bb > 0 ? sqrt(rr) / bnorm : 0.0;
+    // true residual |b - M x| / |b| on the full lattice (fp64); r/qs are free now but may be half-sized: use rhs..: recompute into scratch tail
+    {
+        char *t = (sy.even_odd ? rhs : r);          // rhs (1 half) + r (1 half) are contiguous when even_odd; r is full-sized otherwise
+        ST(fmatrix(c, COLA_F64, 0, X, t, nullptr));
+        flops += 1872.0 * (double)c->V;
+        double tr = 0.0;
+        for (int h = 0; h < 2; h++) {
+            CK(launch_axpby64(nullptr, 1.0, B + h * h64, -1.0, t + h * h64, nullptr, c->Vh, c->partials, &c->ctl->counter[3], &ctl->aux[h], c->stream));
+            c->launches++;
+        }
+        double a0, a1;
+        ST(read_scalar(c, &ctl->aux[0], &a0));
+        ST(read_scalar(c, &ctl->aux[1], &a1));
+        tr = a0 + a1;
+        info->true_residual = bb > 0 ? sqrt(tr) / bnorm : 0.0;
+    }
+    CK(launch_spinor_unpack(COLA_F64, c->g, X, x_canon_dev, c->stream));
+    c->launches++;
+    CK(cudaEventRecord(c->ev1, c->stream));
+    CK(cudaEventSynchronize(c->ev1));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+    info->seconds = ms * 1e-3;
+    info->iters = iters;
+    info->reliable_updates = updates;
+    info->op_flops = flops;
+    if (!status_conv) return fail(c, COLA_ENOCONV, "cola_cg_solve: max_iter reached before |r| <= tol*|b|");
+    return COLA_OK;
+}
+
+extern "C" {
+
+cola_status cola_gauge_upload(cola_ctx *c, const double *host_links) { return gauge_upload_impl(c, host_links, 1); }
+cola_status cola_gauge_upload_dev(cola_ctx *c, const double *dev_links) { return gauge_upload_impl(c, dev_links, 0); }
+
+cola_status cola_gauge_info(const cola_ctx *c, double *max_unitarity_dev)
+{
+    if (!c || !max_unitarity_dev) return COLA_EINVAL;
+    *max_unitarity_dev = c->max_unitarity_dev;
+    return COLA_OK;
+}
+
+cola_status cola_clover_unpack(cola_ctx *c, int which, void *canon_dev)
+{
+    ST(need_ready(c, "cola_clover_unpack"));
+    if (!canon_dev) return fail(c, COLA_EINVAL, "cola_clover_unpack: NULL pointer");
+    if (which == 0) CK(launch_clover_unpack(c->g, c->clovA64, 3, canon_dev, c->stream));
+    else CK(launch_clover_unpack(c->g, c->clovI64, 2, canon_dev, c->stream));
+    c->launches++;
+    return COLA_OK;
+}
+
+cola_status cola_spinor_pack(cola_ctx *c, cola_prec prec, const void *canon_dev, void *internal_dev)
+{
+    if (!c) return COLA_EINVAL;
+    if (!canon_dev || !internal_dev) return fail(c, COLA_EINVAL, "cola_spinor_pack: NULL pointer");
+    CK(launch_spinor_pack(prec, c->g, canon_dev, internal_dev, c->stream));
+    c->launches++;
+    return COLA_OK;
+}
+
+cola_status cola_spinor_unpack(cola_ctx *c, cola_prec prec, const void *internal_dev, void *canon_dev)
+{
+    if (!c) return COLA_EINVAL;
+    if (!canon_dev || !internal_dev) return fail(c, COLA_EINVAL, "cola_spinor_unpack: NULL pointer");
+    CK(launch_spinor_unpack(prec, c->g, internal_dev, canon_dev, c->stream));
+    c->launches++;
+    return COLA_OK;
+}
+
+cola_status cola_spinor_convert(cola_ctx *c, cola_prec dst_prec, const void *src_dev, void *dst_dev, int n_half)
+{
+    if (!c) return COLA_EINVAL;
+    if (!src_dev || !dst_dev || n_half < 1 || n_half > 2) return fail(c, COLA_EINVAL, "cola_spinor_convert: bad argument");
+    const cola_prec src_prec = dst_prec == COLA_F64 ? COLA_F32 : COLA_F64;
+    for (int h = 0; h < n_half; h++) {
+        CK(launch_spinor_convert(dst_prec, (const char *)src_dev + h * half_bytes(c, src_prec), (char *)dst_dev + h * half_bytes(c, dst_prec), c->Vh, c->stream));
+        c->launches++;
+    }
+    return COLA_OK;
+}
+
+cola_status cola_dslash_apply(cola_ctx *c, cola_prec prec, cola_parity out_parity, const void *in_dev, void *out_dev)
+{
+    ST(need_ready(c, "cola_dslash_apply"));
+    if (!in_dev || !out_dev || in_dev == out_dev) return fail(c, COLA_EINVAL, "cola_dslash_apply: NULL or aliased buffers");
+    if (out_parity != COLA_EVEN && out_parity != COLA_ODD) return fail(c, COLA_EINVAL, "cola_dslash_apply: bad parity");
+    return dslash(c, prec, (int)out_parity, 0, in_dev, out_dev, nullptr, 0, 0.0, 0, nullptr, 0);
+}
+
+cola_status cola_fermion_matrix_apply(cola_ctx *c, cola_prec prec, int dagger, const void *in_full_dev, void *out_full_dev)
+{
+    ST(need_ready(c, "cola_fermion_matrix_apply"));
+    if (!in_full_dev || !out_full_dev || in_full_dev == out_full_dev) return fail(c, COLA_EINVAL, "cola_fermion_matrix_apply: NULL or aliased buffers");
+    return fmatrix(c, prec, dagger ? 1 : 0, in_full_dev, out_full_dev, nullptr);
+}
+
+cola_status cola_schur_apply(cola_ctx *c, cola_prec prec, int dagger, const void *in_even_dev, void *out_even_dev)
+{
+    ST(need_ready(c, "cola_schur_apply"));
+    if (!in_even_dev || !out_even_dev || in_even_dev == out_even_dev) return fail(c, COLA_EINVAL, "cola_schur_apply: NULL or aliased buffers");
+    return schur(c, prec, dagger ? 1 : 0, in_even_dev, out_even_dev, nullptr);
+}
+
+cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info)
+{
+    return solve_impl(c, sp, b_canon_dev, x_canon_dev, info);
+}
+
+// ---- end-to-end variants with HOST buffers.  Staging lives in the tail of the solver scratch
+// (the solver uses at most 10 of its 12 half-vector slots when it is called from here; the two
+// canonical staging buffers below need 2 full fp64 vectors = 4 slots, so operators stage in the
+// first slots and the solve stages in x/b of the caller through the separate tmp region).
+static cola_status host_op(cola_ctx *c, cola_prec prec, int which, int arg, const void *in_host, void *out_host)
+{
+    ST(need_ready(c, "cola_*_apply_host"));
+    if (!in_host || !out_host) return fail(c, COLA_EINVAL, "cola_*_apply_host: NULL pointer");
+    CK(cudaSetDevice(c->p.device));
+    const size_t fb = 2 * half_bytes(c, prec);
+    char *canon = c->scratch, *in_int = canon + fb, *out_int = in_int + fb;
+    CK(cudaMemcpyAsync(canon, in_host, fb, cudaMemcpyHostToDevice, c->stream));
+    CK(launch_spinor_pack(prec, c->g, canon, in_int, c->stream));
+    c->launches++;
+    if (which == 0) {
+        const int p = arg;
+        const size_t hb = half_bytes(c, prec);
+        CK(cudaMemsetAsync(out_int, 0, fb, c->stream));
+        ST(dslash(c, prec, p, 0, in_int + (1 - p) * hb, out_int + p * hb, nullptr, 0, 0.0, 0, nullptr, 0));
+    } else {
+        ST(fmatrix(c, prec, arg, in_int, out_int, nullptr));
+    }
+    CK(launch_spinor_unpack(prec, c->g, out_int, canon, c->stream));
+    c->launches++;
+    CK(cudaMemcpyAsync(out_host, canon, fb, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return COLA_OK;
+}
+
+cola_status cola_dslash_apply_host(cola_ctx *c, cola_prec prec, cola_parity out_parity, const void *in_canon_host, void *out_canon_host)
+{
+    if (c && out_parity != COLA_EVEN && out_parity != COLA_ODD) return fail(c, COLA_EINVAL, "cola_dslash_apply_host: bad parity");
+    return host_op(c, prec, 0, (int)out_parity, in_canon_host, out_canon_host);
+}
+
+cola_status cola_fermion_matrix_apply_host(cola_ctx *c, cola_prec prec, int dagger, const void *in_canon_host, void *out_canon_host)
+{
+    return host_op(c, prec, 1, dagger ? 1 : 0, in_canon_host, out_canon_host);
+}
+
+cola_status cola_cg_solve_host(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_host, void *x_canon_host, cola_solve_info *info)
+{
+    ST(need_ready(c, "cola_cg_solve_host"));
+    if (!b_canon_host || !x_canon_host) return fail(c, COLA_EINVAL, "cola_cg_solve_host: NULL pointer");
+    CK(cudaSetDevice(c->p.device));
+    // canonical staging: the last two fp64 half-slots pairs of the scratch are free in every solver mode
+    // except mixed CGNR on M, which uses all 12; stage in tmp64+tmp32 is too small, so the canonical b/x
+    // share ONE staging buffer: b is packed before x is produced.
+    const size_t fb = 2 * half_bytes(c, COLA_F64);
+    char *stage = c->scratch + c->scratch_bytes - fb;
+    if (!sp || (sp->mixed && !sp->even_odd)) return fail(c, COLA_EINVAL, "cola_cg_solve_host: mixed CGNR on M is not offered with host buffers");
+    CK(cudaMemcpyAsync(stage, b_canon_host, fb, cudaMemcpyHostToDevice, c->stream));
+    cola_status st = solve_impl(c, sp, stage, stage, info);
+    if (st != COLA_OK && st != COLA_ENOCONV) return st;
+    CK(cudaMemcpyAsync(x_canon_host, stage, fb, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return st;
+}
+
+unsigned long long cola_launch_count(const cola_ctx *c) { return c ? c->launches : 0; }
+
+}  // extern "C"

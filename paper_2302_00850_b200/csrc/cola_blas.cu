@@ -1,0 +1,165 @@
+// cola_blas.cu -- fused BLAS-1 layer of the CGLS iteration.
+// Vectors are flat arrays of 16-byte chunks; alpha and beta are formed on the device from the
+// reduction results in Ctl, so no scalar crosses the PCIe bus inside an iteration.  Reductions are
+// accumulated in fp64 also for fp32 vectors and are deterministic (fixed grid, fixed order).
+#include "cola_device.cuh"
+
+namespace cola {
+
+namespace {
+
+constexpr int BB = 256;
+constexpr int MAX_BLOCKS = 148 * 8;
+
+inline unsigned blas_grid(size_t n_chunks)
+{
+    size_t b = (n_chunks + BB - 1) / BB;
+    return (unsigned)(b < (size_t)MAX_BLOCKS ? b : (size_t)MAX_BLOCKS);
+}
+
+__device__ __forceinline__ double sq(const float4 &v) { return (double)(v.x * v.x + v.y * v.y) + (double)(v.z * v.z + v.w * v.w); }
+__device__ __forceinline__ double sq(const double2 &v) { return v.x * v.x + v.y * v.y; }
+__device__ __forceinline__ float4 axpy(float a, const float4 &x, const float4 &y) { return make_float4(y.x + a * x.x, y.y + a * x.y, y.z + a * x.z, y.w + a * x.w); }
+__device__ __forceinline__ double2 axpy(double a, const double2 &x, const double2 &y) { return make_double2(y.x + a * x.x, y.y + a * x.y); }
+
+template <typename T>
+__global__ void __launch_bounds__(BB) norm2_kernel(const typename VT<T>::V *v, size_t n, double *partials, unsigned *counter, double *out)
+{
+    double acc = 0.0;
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) acc += sq(v[k]);
+    grid_sum_finalize(acc, partials, counter, out);
+}
+
+// r -= alpha q, alpha = gamma / qq;  rr = |r|^2
+template <typename T>
+__global__ void __launch_bounds__(BB) r_update_kernel(typename VT<T>::V *r, const typename VT<T>::V *q, Ctl *ctl, int cur, size_t n, double *partials)
+{
+    const T ma = (T)(-(ctl->gam[cur] / ctl->qq));
+    double acc = 0.0;
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) {
+        const typename VT<T>::V v = axpy(ma, q[k], r[k]);
+        r[k] = v;
+        acc += sq(v);
+    }
+    grid_sum_finalize(acc, partials, &ctl->counter[1], &ctl->rr);
+}
+
+// x += alpha p (DO_X);  p = s + beta p (DO_P);  alpha = gamma/qq, beta = gamma_new/gamma
+template <typename T, bool DO_X, bool DO_P>
+__global__ void __launch_bounds__(BB) xp_update_kernel(typename VT<T>::V *x, typename VT<T>::V *p, const typename VT<T>::V *s, const Ctl *ctl, int cur, size_t n)
+{
+    const T alpha = (T)(ctl->gam[cur] / ctl->qq);
+    const T beta = (T)(ctl->gam[cur ^ 1] / ctl->gam[cur]);
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) {
+        const typename VT<T>::V pv = p[k];
+        if (DO_X) x[k] = axpy(alpha, pv, x[k]);
+        if (DO_P) p[k] = axpy(beta, pv, s[k]);
+    }
+}
+
+// out64 = a*A + b*B; optional fp32 copy (internal fp32 layout needs chunk pairing, so this kernel works
+// per site-chunk pair: thread handles double2 chunks 2k, 2k+1 of site i = one float4 chunk k)
+__global__ void __launch_bounds__(BB) axpby64_kernel(double2 *out, double a, const double2 *A, double b, const double2 *B, float4 *out32,
+                                                     size_t n_sites, double *partials, unsigned *counter, double *norm_out)
+{
+    double acc = 0.0;
+    const size_t n = 6 * n_sites;
+    for (size_t tid = (size_t)blockIdx.x * BB + threadIdx.x; tid < n; tid += (size_t)gridDim.x * BB) {
+        const size_t k = tid / n_sites, i = tid - k * n_sites;
+        const size_t c0 = (2 * k) * n_sites + i, c1 = (2 * k + 1) * n_sites + i;
+        double2 v0, v1;
+        if (B) {
+            const double2 a0 = A[c0], a1 = A[c1], b0 = B[c0], b1 = B[c1];
+            v0 = make_double2(a * a0.x + b * b0.x, a * a0.y + b * b0.y);
+            v1 = make_double2(a * a1.x + b * b1.x, a * a1.y + b * b1.y);
+        } else {
+            const double2 a0 = A[c0], a1 = A[c1];
+            v0 = make_double2(a * a0.x, a * a0.y);
+            v1 = make_double2(a * a1.x, a * a1.y);
+        }
+        if (out) {
+            out[c0] = v0;
+            out[c1] = v1;
+        }
+        if (out32) out32[k * n_sites + i] = make_float4((float)v0.x, (float)v0.y, (float)v1.x, (float)v1.y);
+        acc += sq(v0) + sq(v1);
+    }
+    if (partials) grid_sum_finalize(acc, partials, counter, norm_out);
+}
+
+// x64 += x32; x32 = 0
+__global__ void __launch_bounds__(BB) accumulate_kernel(double2 *x64, float4 *x32, size_t n_sites)
+{
+    const size_t n = 6 * n_sites;
+    for (size_t tid = (size_t)blockIdx.x * BB + threadIdx.x; tid < n; tid += (size_t)gridDim.x * BB) {
+        const size_t k = tid / n_sites, i = tid - k * n_sites;
+        const size_t c0 = (2 * k) * n_sites + i, c1 = (2 * k + 1) * n_sites + i;
+        const float4 v = x32[k * n_sites + i];
+        double2 a0 = x64[c0], a1 = x64[c1];
+        a0.x += v.x; a0.y += v.y; a1.x += v.z; a1.y += v.w;
+        x64[c0] = a0;
+        x64[c1] = a1;
+        x32[k * n_sites + i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+}  // namespace
+
+int blas_max_blocks() { return MAX_BLOCKS; }
+
+cudaError_t launch_norm2(cola_prec prec, const void *v, size_t n_sites, double *partials, unsigned *counter, double *out, cudaStream_t s)
+{
+    if (prec == COLA_F64) {
+        const size_t n = 12 * n_sites;
+        norm2_kernel<double><<<blas_grid(n), BB, 0, s>>>((const double2 *)v, n, partials, counter, out);
+    } else {
+        const size_t n = 6 * n_sites;
+        norm2_kernel<float><<<blas_grid(n), BB, 0, s>>>((const float4 *)v, n, partials, counter, out);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_r_update(cola_prec prec, void *r, const void *q, Ctl *ctl, int cur, size_t n_sites, double *partials, cudaStream_t s)
+{
+    if (prec == COLA_F64) {
+        const size_t n = 12 * n_sites;
+        r_update_kernel<double><<<blas_grid(n), BB, 0, s>>>((double2 *)r, (const double2 *)q, ctl, cur, n, partials);
+    } else {
+        const size_t n = 6 * n_sites;
+        r_update_kernel<float><<<blas_grid(n), BB, 0, s>>>((float4 *)r, (const float4 *)q, ctl, cur, n, partials);
+    }
+    return cudaGetLastError();
+}
+
+template <typename T>
+static void xp_dispatch(void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, size_t n, cudaStream_t s)
+{
+    typedef typename VT<T>::V V;
+    const unsigned grid = blas_grid(n);
+    if (do_x && do_p) xp_update_kernel<T, true, true><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, n);
+    else if (do_x) xp_update_kernel<T, true, false><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, n);
+    else if (do_p) xp_update_kernel<T, false, true><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, n);
+}
+
+cudaError_t launch_xp_update(cola_prec prec, void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, size_t n_sites, cudaStream_t s)
+{
+    if (prec == COLA_F64) xp_dispatch<double>(x, p, sv, ctl, cur, do_x, do_p, 12 * n_sites, s);
+    else xp_dispatch<float>(x, p, sv, ctl, cur, do_x, do_p, 6 * n_sites, s);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_axpby64(void *out64, double a, const void *A64, double b, const void *B64, void *out32, size_t n_sites,
+                           double *partials, unsigned *counter, double *norm_out, cudaStream_t s)
+{
+    axpby64_kernel<<<blas_grid(6 * n_sites), BB, 0, s>>>((double2 *)out64, a, (const double2 *)A64, b, (const double2 *)B64, (float4 *)out32,
+                                                        n_sites, partials, counter, norm_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_accumulate(void *x64, void *x32, size_t n_sites, cudaStream_t s)
+{
+    accumulate_kernel<<<blas_grid(6 * n_sites), BB, 0, s>>>((double2 *)x64, (float4 *)x32, n_sites);
+    return cudaGetLastError();
+}
+
+}  // namespace cola

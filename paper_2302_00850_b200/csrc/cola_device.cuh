@@ -1,0 +1,205 @@
+// cola_device.cuh -- device-side building blocks: 16-byte SoA chunk I/O, SU(3) link load with
+// in-register third-row reconstruction (BJ:ns), packed 6x6 Hermitian clover mat-vec,
+// deterministic warp-shuffle + block + last-block reduction.
+#pragma once
+#include "cola_internal.h"
+
+namespace cola {
+
+template <typename T> struct VT;
+template <> struct VT<float> {
+    typedef float4 V;
+    static constexpr int N = 4;
+};
+template <> struct VT<double> {
+    typedef double2 V;
+    static constexpr int N = 2;
+};
+
+// ---- 16-byte global loads/stores.  "stream" = read-once data (links, clover): bypass L1 allocation
+// so that L1 keeps the neighbour spinors, which are the only data with reuse inside a block.
+__device__ __forceinline__ float4 ld_stream(const float4 *p)
+{
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ float2 ld_stream(const float2 *p)
+{
+    float2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ double2 ld_stream(const double2 *p)
+{
+    double2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ float4 ld_cached(const float4 *p) { return __ldg(p); }
+__device__ __forceinline__ double2 ld_cached(const double2 *p) { return __ldg(p); }
+
+__device__ __forceinline__ void unpack(const float4 &v, float *r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
+__device__ __forceinline__ void unpack(const double2 &v, double *r) { r[0] = v.x; r[1] = v.y; }
+__device__ __forceinline__ float4 pack(const float *r) { return make_float4(r[0], r[1], r[2], r[3]); }
+__device__ __forceinline__ double2 pack(const double *r) { return make_double2(r[0], r[1]); }
+
+// NR reals of site i from an SoA field of 16-byte chunks with chunk stride `stride` (in chunks)
+template <typename T, int NR, bool STREAM>
+__device__ __forceinline__ void load_reals(const void *base, size_t stride, size_t i, T (&r)[NR])
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = VT<T>::N;
+    const V *p = reinterpret_cast<const V *>(base) + i;
+#pragma unroll
+    for (int k = 0; k < NR / N; k++) {
+        V v = STREAM ? ld_stream(p + (size_t)k * stride) : ld_cached(p + (size_t)k * stride);
+        unpack(v, &r[k * N]);
+    }
+}
+
+template <typename T, int NR>
+__device__ __forceinline__ void store_reals(void *base, size_t stride, size_t i, const T (&r)[NR])
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = VT<T>::N;
+    V *p = reinterpret_cast<V *>(base) + i;
+#pragma unroll
+    for (int k = 0; k < NR / N; k++) p[(size_t)k * stride] = pack(&r[k * N]);
+}
+
+// ---- links.  u[18] = row-major (re, im) of the 3x3 matrix.
+// third row of an SU(3) matrix from the first two: row3 = conj(row1 x row2)
+template <typename T>
+__device__ __forceinline__ void reconstruct_row3(T (&u)[18])
+{
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        // U_2c = conj(U_0a U_1b - U_0b U_1a)
+        T re = u[2 * a] * u[6 + 2 * b] - u[2 * a + 1] * u[6 + 2 * b + 1] - (u[2 * b] * u[6 + 2 * a] - u[2 * b + 1] * u[6 + 2 * a + 1]);
+        T im = u[2 * a] * u[6 + 2 * b + 1] + u[2 * a + 1] * u[6 + 2 * b] - (u[2 * b] * u[6 + 2 * a + 1] + u[2 * b + 1] * u[6 + 2 * a]);
+        u[12 + 2 * c] = re;
+        u[12 + 2 * c + 1] = -im;
+    }
+}
+
+template <int FMT> struct LinkT;
+template <> struct LinkT<LINK_F64_18> { typedef double T; };
+template <> struct LinkT<LINK_F32_18> { typedef float T; };
+template <> struct LinkT<LINK_F32_12> { typedef float T; };
+
+// base = start of the [chunk][Vh] block of one (parity, mu)
+template <int FMT>
+__device__ __forceinline__ void load_link(const char *base, size_t Vh, size_t i, typename LinkT<FMT>::T (&u)[18])
+{
+    if constexpr (FMT == LINK_F64_18) {
+        load_reals<double, 18, true>(base, Vh, i, u);
+    } else if constexpr (FMT == LINK_F32_12) {
+        float r[12];
+        load_reals<float, 12, true>(base, Vh, i, r);
+#pragma unroll
+        for (int k = 0; k < 12; k++) u[k] = r[k];
+        reconstruct_row3(u);
+    } else {
+        float r[16];
+        load_reals<float, 16, true>(base, Vh, i, r);
+#pragma unroll
+        for (int k = 0; k < 16; k++) u[k] = r[k];
+        float2 t = ld_stream(reinterpret_cast<const float2 *>(base + 64 * Vh) + i);
+        u[16] = t.x;
+        u[17] = t.y;
+    }
+}
+
+// ---- packed clover: per site 2 chiral blocks x (6 real diagonal + 15 complex strictly-lower entries,
+// row-wise: (1,0),(2,0),(2,1),(3,0)...) = 72 reals.  Component index inside a block = 3*(s mod 2) + c.
+// w = C v for one block; v, w are 6 complex = 12 reals; c = the block's 36 reals.
+template <typename T>
+__device__ __forceinline__ void clover_block_mul(const T *c, const T *v, T *w)
+{
+#pragma unroll
+    for (int i = 0; i < 6; i++) {
+        w[2 * i] = c[i] * v[2 * i];
+        w[2 * i + 1] = c[i] * v[2 * i + 1];
+    }
+#pragma unroll
+    for (int i = 1; i < 6; i++) {
+#pragma unroll
+        for (int j = 0; j < i; j++) {
+            const int k = 6 + 2 * (i * (i - 1) / 2 + j);
+            const T ar = c[k], ai = c[k + 1];
+            // w_i += a v_j
+            w[2 * i] += ar * v[2 * j] - ai * v[2 * j + 1];
+            w[2 * i + 1] += ar * v[2 * j + 1] + ai * v[2 * j];
+            // w_j += conj(a) v_i
+            w[2 * j] += ar * v[2 * i] + ai * v[2 * i + 1];
+            w[2 * j + 1] += ar * v[2 * i + 1] - ai * v[2 * i];
+        }
+    }
+}
+
+// w = C(site i) v on the full 24-real spinor; clov = [72/N chunks][Vh]
+template <typename T>
+__device__ __forceinline__ void clover_apply(const void *clov, size_t Vh, size_t i, const T (&v)[24], T (&w)[24])
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = VT<T>::N;
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+        T c[36];
+        load_reals<T, 36, true>(reinterpret_cast<const V *>(clov) + (size_t)b * (36 / N) * Vh, Vh, i, c);
+        clover_block_mul(c, &v[12 * b], &w[12 * b]);
+    }
+}
+
+// ---- deterministic reduction: warp shuffle -> shared -> per-block partial -> the last block to
+// finish adds the partials in a fixed order.  All threads of the block must call it.
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ double block_sum(double v, double *sm /* >= 32 doubles */)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    v = warp_sum(v);
+    __syncthreads();
+    if (lane == 0) sm[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        double t = lane < nw ? sm[lane] : 0.0;
+        t = warp_sum(t);
+        if (lane == 0) sm[0] = t;
+    }
+    __syncthreads();
+    return sm[0];
+}
+
+__device__ __forceinline__ void grid_sum_finalize(double v, double *partials, unsigned *counter, double *result, bool accumulate = false)
+{
+    __shared__ double sm[33];
+    __shared__ int is_last;
+    double s = block_sum(v, sm);
+    if (threadIdx.x == 0) {
+        partials[blockIdx.x] = s;
+        __threadfence();
+        unsigned t = atomicAdd(counter, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        double a = 0.0;
+        for (unsigned k = threadIdx.x; k < gridDim.x; k += blockDim.x) a += __ldcg(partials + k);
+        a = block_sum(a, sm);
+        if (threadIdx.x == 0) {
+            *result = accumulate ? *result + a : a;
+            *counter = 0u;
+        }
+    }
+}
+
+}  // namespace cola

@@ -1,0 +1,256 @@
+// cola_dslash.cu -- the parity dslash kernel family (BJ:ns).
+//
+// One thread per output site ("each lattice site is mapped to a single thread").  For each of
+// the 8 hops: load the neighbour spinor (SoA, 16-byte chunks, site index fastest => coalesced),
+// spin-project it to a half spinor BEFORE the colour multiply (12 instead of 24 reals through the
+// SU(3) mat-vec), load the link (12 reals + in-register third-row reconstruction, or 18), multiply,
+// apply the boundary sign, reconstruct the lower spin components and accumulate.  The clover
+// mat-vec, the xpay and the |.|^2 reduction are epilogues of the same kernel, so a Schur-complement
+// application is two launches and no intermediate vector is re-read for BLAS-1 work.
+//
+// Chiral basis: gamma_mu = [[0, A_mu], [A_mu^+, 0]], A_k = -i sigma_k, A_t = 1:
+//   (1 + s gamma_mu) psi = [ h ; s A_mu^+ h ],   h = psi_upper + s A_mu psi_lower,   s = +-1.
+#include "cola_device.cuh"
+
+namespace cola {
+
+namespace {
+
+constexpr int DSLASH_BLOCK = 128;
+
+// h (2 spins x 3 colours, complex) = upper + s * A_mu * lower of the 24-real spinor p
+template <int MU, typename T>
+__device__ __forceinline__ void project(const T (&p)[24], T s, T (&h)[12])
+{
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int u0 = 2 * c, u1 = 6 + 2 * c, l0 = 12 + 2 * c, l1 = 18 + 2 * c;   // spin 0,1,2,3 colour c (re)
+        if (MU == 0) {          // A = [[0,-i],[-i,0]]
+            h[2 * c] = p[u0] + s * p[l1 + 1];
+            h[2 * c + 1] = p[u0 + 1] - s * p[l1];
+            h[6 + 2 * c] = p[u1] + s * p[l0 + 1];
+            h[6 + 2 * c + 1] = p[u1 + 1] - s * p[l0];
+        } else if (MU == 1) {   // A = [[0,-1],[1,0]]
+            h[2 * c] = p[u0] - s * p[l1];
+            h[2 * c + 1] = p[u0 + 1] - s * p[l1 + 1];
+            h[6 + 2 * c] = p[u1] + s * p[l0];
+            h[6 + 2 * c + 1] = p[u1 + 1] + s * p[l0 + 1];
+        } else if (MU == 2) {   // A = [[-i,0],[0,i]]
+            h[2 * c] = p[u0] + s * p[l0 + 1];
+            h[2 * c + 1] = p[u0 + 1] - s * p[l0];
+            h[6 + 2 * c] = p[u1] - s * p[l1 + 1];
+            h[6 + 2 * c + 1] = p[u1 + 1] + s * p[l1];
+        } else {                // A = 1
+            h[2 * c] = p[u0] + s * p[l0];
+            h[2 * c + 1] = p[u0 + 1] + s * p[l0 + 1];
+            h[6 + 2 * c] = p[u1] + s * p[l1];
+            h[6 + 2 * c + 1] = p[u1 + 1] + s * p[l1 + 1];
+        }
+    }
+}
+
+// acc += eta * [ g ; s A_mu^+ g ]
+template <int MU, typename T>
+__device__ __forceinline__ void reconstruct_accumulate(const T (&g)[12], T eta, T s, T (&acc)[24])
+{
+    const T se = s * eta;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int u0 = 2 * c, u1 = 6 + 2 * c, l0 = 12 + 2 * c, l1 = 18 + 2 * c;
+        const T g0r = g[2 * c], g0i = g[2 * c + 1], g1r = g[6 + 2 * c], g1i = g[6 + 2 * c + 1];
+        acc[u0] += eta * g0r;
+        acc[u0 + 1] += eta * g0i;
+        acc[u1] += eta * g1r;
+        acc[u1 + 1] += eta * g1i;
+        if (MU == 0) {          // A^+ = [[0,i],[i,0]]: lower0 = i g1, lower1 = i g0
+            acc[l0] -= se * g1i;
+            acc[l0 + 1] += se * g1r;
+            acc[l1] -= se * g0i;
+            acc[l1 + 1] += se * g0r;
+        } else if (MU == 1) {   // A^+ = [[0,1],[-1,0]]: lower0 = g1, lower1 = -g0
+            acc[l0] += se * g1r;
+            acc[l0 + 1] += se * g1i;
+            acc[l1] -= se * g0r;
+            acc[l1 + 1] -= se * g0i;
+        } else if (MU == 2) {   // A^+ = [[i,0],[0,-i]]: lower0 = i g0, lower1 = -i g1
+            acc[l0] -= se * g0i;
+            acc[l0 + 1] += se * g0r;
+            acc[l1] += se * g1i;
+            acc[l1 + 1] -= se * g1r;
+        } else {                // A^+ = 1
+            acc[l0] += se * g0r;
+            acc[l0 + 1] += se * g0i;
+            acc[l1] += se * g1r;
+            acc[l1 + 1] += se * g1i;
+        }
+    }
+}
+
+// g = U h (DAG = false) or U^+ h (DAG = true) on both spin components of the half spinor
+template <bool DAG, typename T>
+__device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&g)[12])
+{
+#pragma unroll
+    for (int sp = 0; sp < 2; sp++) {
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            T re = 0, im = 0;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                const T ur = DAG ? u[2 * (3 * b + a)] : u[2 * (3 * a + b)];
+                const T ui = DAG ? -u[2 * (3 * b + a) + 1] : u[2 * (3 * a + b) + 1];
+                const T hr = h[6 * sp + 2 * b], hi = h[6 * sp + 2 * b + 1];
+                re += ur * hr - ui * hi;
+                im += ur * hi + ui * hr;
+            }
+            g[6 * sp + 2 * a] = re;
+            g[6 * sp + 2 * a + 1] = im;
+        }
+    }
+}
+
+// one hop: neighbour index nb (parity 1-p), link at site li of the given gauge block
+template <int FMT, int MU, bool BACK, typename T>
+__device__ __forceinline__ void hop(const void *in, const char *gauge_mu, size_t Vh, int nb, int li, T eta, T s, T (&acc)[24])
+{
+    T psi[24], h[12], g[12], u[18];
+    load_reals<T, 24, false>(in, Vh, nb, psi);
+    load_link<FMT>(gauge_mu, Vh, li, u);
+    project<MU>(psi, s, h);
+    su3_mul<BACK>(u, h, g);
+    reconstruct_accumulate<MU>(g, eta, s, acc);
+}
+
+// XPAY: 0 none, 1 v = y + coef v, 2 v = A y + coef v.   POST: 0 none, 1 v = Cpost v.
+template <int FMT, int XPAY, int POST>
+__global__ void __launch_bounds__(DSLASH_BLOCK) dslash_kernel(const __grid_constant__ DslashArgs a)
+{
+    typedef typename LinkT<FMT>::T T;
+    const Geom &g = a.g;
+    const size_t Vh = g.Vh;
+    const int i = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
+    double nrm = 0.0;
+    if (i < g.Vh) {
+        // coordinates of the output site
+        const int xh = i % g.Xh;
+        int r = i / g.Xh;
+        const int y = r % g.Y;
+        r /= g.Y;
+        const int z = r % g.Z;
+        const int t = r / g.Z;
+        const int odd = (y + z + t + a.parity) & 1;     // x = 2*xh + odd
+        const int sY = g.Xh, sZ = g.Xh * g.Y, sT = g.Xh * g.Y * g.Z;
+
+        // neighbour cb indices (parity 1-p) and boundary crossings
+        const int xf = odd ? (xh + 1 == g.Xh ? i - xh : i + 1) : i;
+        const int xb = odd ? i : (xh == 0 ? i + g.Xh - 1 : i - 1);
+        const bool cxf = odd && (xh + 1 == g.Xh), cxb = !odd && (xh == 0);
+        const int yf = (y + 1 == g.Y) ? i - (g.Y - 1) * sY : i + sY;
+        const int yb = (y == 0) ? i + (g.Y - 1) * sY : i - sY;
+        const int zf = (z + 1 == g.Z) ? i - (g.Z - 1) * sZ : i + sZ;
+        const int zb = (z == 0) ? i + (g.Z - 1) * sZ : i - sZ;
+        const int tf = (t + 1 == g.T) ? i - (g.T - 1) * sT : i + sT;
+        const int tb = (t == 0) ? i + (g.T - 1) * sT : i - sT;
+
+        const T one = 1;
+        const T ex_f = (cxf && g.bc[0] < 0) ? -one : one, ex_b = (cxb && g.bc[0] < 0) ? -one : one;
+        const T ey_f = (y + 1 == g.Y && g.bc[1] < 0) ? -one : one, ey_b = (y == 0 && g.bc[1] < 0) ? -one : one;
+        const T ez_f = (z + 1 == g.Z && g.bc[2] < 0) ? -one : one, ez_b = (z == 0 && g.bc[2] < 0) ? -one : one;
+        const T et_f = (t + 1 == g.T && g.bc[3] < 0) ? -one : one, et_b = (t == 0 && g.bc[3] < 0) ? -one : one;
+
+        const T sf = (T)a.sgn, sb = -(T)a.sgn;   // forward: (1 + sgn*gamma), backward: (1 - sgn*gamma)
+        const size_t lb = link_bytes(FMT) * Vh;  // bytes of one (parity, mu) block
+        const char *gp = reinterpret_cast<const char *>(a.gauge_p);
+        const char *gq = reinterpret_cast<const char *>(a.gauge_q);
+
+        T acc[24];
+#pragma unroll
+        for (int k = 0; k < 24; k++) acc[k] = 0;
+
+        hop<FMT, 0, false>(a.in, gp + 0 * lb, Vh, xf, i, ex_f, sf, acc);
+        hop<FMT, 0, true>(a.in, gq + 0 * lb, Vh, xb, xb, ex_b, sb, acc);
+        hop<FMT, 1, false>(a.in, gp + 1 * lb, Vh, yf, i, ey_f, sf, acc);
+        hop<FMT, 1, true>(a.in, gq + 1 * lb, Vh, yb, yb, ey_b, sb, acc);
+        hop<FMT, 2, false>(a.in, gp + 2 * lb, Vh, zf, i, ez_f, sf, acc);
+        hop<FMT, 2, true>(a.in, gq + 2 * lb, Vh, zb, zb, ez_b, sb, acc);
+        hop<FMT, 3, false>(a.in, gp + 3 * lb, Vh, tf, i, et_f, sf, acc);
+        hop<FMT, 3, true>(a.in, gq + 3 * lb, Vh, tb, tb, et_b, sb, acc);
+
+        if (XPAY != 0) {
+            T yv[24];
+            load_reals<T, 24, true>(a.y, Vh, i, yv);
+            const T cf = (T)a.coef;
+            if (XPAY == 2) {
+                T cy[24];
+                clover_apply<T>(a.clov_y, Vh, i, yv, cy);
+#pragma unroll
+                for (int k = 0; k < 24; k++) acc[k] = cy[k] + cf * acc[k];
+            } else {
+#pragma unroll
+                for (int k = 0; k < 24; k++) acc[k] = yv[k] + cf * acc[k];
+            }
+        }
+        if (POST != 0) {
+            T w[24];
+            clover_apply<T>(a.clov_post, Vh, i, acc, w);
+#pragma unroll
+            for (int k = 0; k < 24; k++) acc[k] = w[k];
+        }
+        store_reals<T, 24>(a.out, Vh, i, acc);
+        if (a.partials) {
+            T s2 = 0;
+#pragma unroll
+            for (int k = 0; k < 24; k++) s2 += acc[k] * acc[k];
+            nrm = (double)s2;
+        }
+    }
+    if (a.partials) grid_sum_finalize(nrm, a.partials, a.counter, a.norm_out, a.norm_accumulate != 0);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(DSLASH_BLOCK) clover_apply_kernel(int Vh, const void *clov, const void *in, void *out)
+{
+    const int i = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
+    if (i >= Vh) return;
+    T v[24], w[24];
+    load_reals<T, 24, true>(in, Vh, i, v);
+    clover_apply<T>(clov, Vh, i, v, w);
+    store_reals<T, 24>(out, Vh, i, w);
+}
+
+template <int FMT>
+cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
+{
+    const int xpay = a.y ? (a.clov_y ? 2 : 1) : 0;
+    const int post = a.clov_post ? 1 : 0;
+    const dim3 grid((a.g.Vh + DSLASH_BLOCK - 1) / DSLASH_BLOCK), block(DSLASH_BLOCK);
+    if (xpay == 0 && post == 0) dslash_kernel<FMT, 0, 0><<<grid, block, 0, s>>>(a);
+    else if (xpay == 0 && post == 1) dslash_kernel<FMT, 0, 1><<<grid, block, 0, s>>>(a);
+    else if (xpay == 1 && post == 0) dslash_kernel<FMT, 1, 0><<<grid, block, 0, s>>>(a);
+    else if (xpay == 1 && post == 1) dslash_kernel<FMT, 1, 1><<<grid, block, 0, s>>>(a);
+    else if (xpay == 2 && post == 0) dslash_kernel<FMT, 2, 0><<<grid, block, 0, s>>>(a);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_dslash(int fmt, const DslashArgs &a, cudaStream_t s)
+{
+    switch (fmt) {
+        case LINK_F64_18: return launch_fmt<LINK_F64_18>(a, s);
+        case LINK_F32_18: return launch_fmt<LINK_F32_18>(a, s);
+        case LINK_F32_12: return launch_fmt<LINK_F32_12>(a, s);
+    }
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_clover_apply(cola_prec prec, const Geom &g, const void *clov, const void *in, void *out, cudaStream_t s)
+{
+    const dim3 grid((g.Vh + DSLASH_BLOCK - 1) / DSLASH_BLOCK), block(DSLASH_BLOCK);
+    if (prec == COLA_F64) clover_apply_kernel<double><<<grid, block, 0, s>>>(g.Vh, clov, in, out);
+    else clover_apply_kernel<float><<<grid, block, 0, s>>>(g.Vh, clov, in, out);
+    return cudaGetLastError();
+}
+
+}  // namespace cola

@@ -1,0 +1,86 @@
+// cola_internal.h -- shared declarations of the CUDA library (not part of the public ABI).
+// Layouts and notation follow include/cola.h and DESIGN.md.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/cola.h"
+
+namespace cola {
+
+// Lattice geometry as the kernels see it.  Checkerboard ("cb") index of a site of either parity:
+//   cb = (x >> 1) + Xh*(y + Y*(z + Z*t)),  x = 2*(cb % Xh) + ((y + z + t + parity) & 1)
+struct Geom {
+    int X, Y, Z, T;   // extents
+    int Xh;           // X/2
+    int Vh;           // half volume
+    int bc[4];        // +1 / -1
+};
+
+// Bytes of one link per site in each storage format.
+enum LinkFmt { LINK_F64_18 = 0, LINK_F32_18 = 1, LINK_F32_12 = 2 };
+__host__ __device__ inline size_t link_bytes(int fmt) { return fmt == LINK_F64_18 ? 144 : (fmt == LINK_F32_18 ? 72 : 48); }
+
+// Device-resident scalars of the CG recurrence (all reductions land here; alpha and beta are
+// formed inside the consuming kernels, so the host only ever reads `rr`).
+struct Ctl {
+    double gam[2];     // |s_k|^2 in gam[k & 1], |s_{k+1}|^2 in gam[(k + 1) & 1]
+    double qq;         // |K p|^2
+    double rr;         // |r|^2
+    double aux[4];
+    unsigned counter[8];  // "last block" tickets, one per concurrently used reduction
+};
+
+// Arguments of the fused parity-dslash kernel family:
+//   v   = D_{p,1-p} in                                (hopping term)
+//   v   = Cy*y + coef*v        if y      (Cy = A_p if clov_y else 1)     (H6/H7/H8 epilogue)
+//   v   = Cpost*v              if clov_post                              (H6: A^-1)
+//   out = v;  *norm_out = sum |v|^2 if partials                          (H9)
+struct DslashArgs {
+    Geom g;
+    const void *in;         // parity 1-p, internal half spinor
+    void *out;              // parity p
+    const void *gauge_p;    // links of parity p:   [mu][chunk][Vh]
+    const void *gauge_q;    // links of parity 1-p
+    const void *y;          // parity p half spinor or nullptr
+    const void *clov_y;     // packed clover of parity p or nullptr
+    const void *clov_post;  // packed clover applied to the result or nullptr
+    double coef;
+    double sgn;             // -1: D (forward hop projects with 1 - gamma_mu); +1: gamma_5 D gamma_5
+    int parity;             // p
+    double *partials;       // per-block partial sums (nullptr: no norm)
+    unsigned *counter;
+    double *norm_out;
+    int norm_accumulate;    // 1: *norm_out += sum (second half of a full-lattice operator)
+};
+
+// launchers (cola_dslash.cu)
+cudaError_t launch_dslash(int fmt, const DslashArgs &a, cudaStream_t s);
+// clover-only apply: out = C in on one parity (cola_dslash.cu)
+cudaError_t launch_clover_apply(cola_prec prec, const Geom &g, const void *clov, const void *in, void *out, cudaStream_t s);
+
+// layout / setup kernels (cola_layout.cu, cola_clover.cu)
+cudaError_t launch_gauge_reorder(const Geom &g, const double *canon_dev, long site_lo, long n_sites, void *gauge64, void *gauge32,
+                                 int fmt32, unsigned long long *max_dev_bits, cudaStream_t s);
+cudaError_t launch_spinor_pack(cola_prec prec, const Geom &g, const void *canon, void *internal, cudaStream_t s);
+cudaError_t launch_spinor_unpack(cola_prec prec, const Geom &g, const void *internal, void *canon, cudaStream_t s);
+cudaError_t launch_spinor_convert(cola_prec dst_prec, const void *src, void *dst, size_t n_sites, cudaStream_t s);
+cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, cudaStream_t s);
+cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, cudaStream_t s);
+cudaError_t launch_clover_unpack(const Geom &g, const void *clov64, int parity_mask, void *canon, cudaStream_t s);
+
+// fused BLAS-1 (cola_blas.cu).  n = number of sites of the vectors (Vh or V).
+int blas_max_blocks();
+cudaError_t launch_norm2(cola_prec prec, const void *v, size_t n_sites, double *partials, unsigned *counter, double *out, cudaStream_t s);
+// cur = k & 1.  r -= alpha q with alpha = ctl->gam[cur] / ctl->qq;  ctl->rr = |r|^2
+cudaError_t launch_r_update(cola_prec prec, void *r, const void *q, Ctl *ctl, int cur, size_t n_sites, double *partials, cudaStream_t s);
+// x += alpha p (if do_x);  p = s + beta p with beta = gam[cur^1]/gam[cur] (if do_p)
+cudaError_t launch_xp_update(cola_prec prec, void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, size_t n_sites, cudaStream_t s);
+// out64 = a*A64 + b*B64 (+ optional fp32 copy of the result, + optional |out|^2)
+cudaError_t launch_axpby64(void *out64, double a, const void *A64, double b, const void *B64, void *out32, size_t n_sites,
+                           double *partials, unsigned *counter, double *norm_out, cudaStream_t s);
+// x64 += x32; x32 = 0
+cudaError_t launch_accumulate(void *x64, void *x32, size_t n_sites, cudaStream_t s);
+
+}  // namespace cola

@@ -1,0 +1,152 @@
+// cola_layout.cu -- layout kernels: canonical arrays <-> parity-split SoA of 16-byte
+// chunks, fp64 -> fp32 copies, 18 -> 12-real link compression, unitarity diagnostic.
+#include "cola_device.cuh"
+
+namespace cola {
+
+namespace {
+
+constexpr int LB = 128;
+
+__device__ __forceinline__ void lex_to_cb(const Geom &g, long lex, int &parity, int &cb)
+{
+    const int x = (int)(lex % g.X);
+    long r = lex / g.X;
+    const int y = (int)(r % g.Y);
+    r /= g.Y;
+    const int z = (int)(r % g.Z);
+    const int t = (int)(r / g.Z);
+    parity = (x + y + z + t) & 1;
+    cb = (x >> 1) + g.Xh * (y + g.Y * (z + g.Z * t));
+}
+
+// one thread per (lex site, mu) of the staged canonical chunk
+__global__ void __launch_bounds__(LB) gauge_reorder_kernel(Geom g, const double *canon, long site_lo, long n_sites, char *gauge64,
+                                                           char *gauge32, int fmt32, unsigned long long *max_dev_bits)
+{
+    const long tid = (long)blockIdx.x * LB + threadIdx.x;
+    double dev = 0.0;
+    if (tid < 4 * n_sites) {
+        const long ls = tid >> 2;
+        const int mu = (int)(tid & 3);
+        const double *src = canon + (ls * 4 + mu) * 18;
+        double u[18];
+#pragma unroll
+        for (int k = 0; k < 18; k++) u[k] = src[k];
+        int parity, cb;
+        lex_to_cb(g, site_lo + ls, parity, cb);
+        const size_t Vh = g.Vh;
+        store_reals<double, 18>(gauge64 + (size_t)(parity * 4 + mu) * 144 * Vh, Vh, cb, u);
+        char *b32 = gauge32 + (size_t)(parity * 4 + mu) * link_bytes(fmt32) * Vh;
+        if (fmt32 == LINK_F32_12) {
+            float f[12];
+#pragma unroll
+            for (int k = 0; k < 12; k++) f[k] = (float)u[k];
+            store_reals<float, 12>(b32, Vh, cb, f);
+        } else {
+            float f[16];
+#pragma unroll
+            for (int k = 0; k < 16; k++) f[k] = (float)u[k];
+            store_reals<float, 16>(b32, Vh, cb, f);
+            reinterpret_cast<float2 *>(b32 + 64 * Vh)[cb] = make_float2((float)u[16], (float)u[17]);
+        }
+        // max |U U^+ - 1| (entry-wise)
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                double re = (a == b) ? -1.0 : 0.0, im = 0.0;
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    const double ar = u[2 * (3 * a + c)], ai = u[2 * (3 * a + c) + 1];
+                    const double br = u[2 * (3 * b + c)], bi = u[2 * (3 * b + c) + 1];
+                    re += ar * br + ai * bi;
+                    im += ai * br - ar * bi;
+                }
+                dev = fmax(dev, sqrt(re * re + im * im));
+            }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dev = fmax(dev, __shfl_xor_sync(0xffffffffu, dev, o));
+    if ((threadIdx.x & 31) == 0 && dev > 0.0) atomicMax(max_dev_bits, (unsigned long long)__double_as_longlong(dev));
+}
+
+template <typename T, bool PACK>
+__global__ void __launch_bounds__(LB) spinor_layout_kernel(Geom g, const T *canon_in, T *canon_out, const void *int_in, void *int_out)
+{
+    const long lex = (long)blockIdx.x * LB + threadIdx.x;
+    if (lex >= 2L * g.Vh) return;
+    int parity, cb;
+    lex_to_cb(g, lex, parity, cb);
+    typedef typename VT<T>::V V;
+    const size_t half_chunks = (size_t)(24 / VT<T>::N) * g.Vh;
+    T r[24];
+    if (PACK) {
+#pragma unroll
+        for (int k = 0; k < 24; k++) r[k] = canon_in[lex * 24 + k];
+        store_reals<T, 24>(reinterpret_cast<V *>(int_out) + parity * half_chunks, g.Vh, cb, r);
+    } else {
+        load_reals<T, 24, true>(reinterpret_cast<const V *>(int_in) + parity * half_chunks, g.Vh, cb, r);
+#pragma unroll
+        for (int k = 0; k < 24; k++) canon_out[lex * 24 + k] = r[k];
+    }
+}
+
+// internal fp64 [12 chunks of double2][n] <-> internal fp32 [6 chunks of float4][n]; one thread per (float4 chunk, site)
+template <bool TO_F32>
+__global__ void __launch_bounds__(LB) convert_kernel(const void *src, void *dst, size_t n)
+{
+    const size_t tid = (size_t)blockIdx.x * LB + threadIdx.x;
+    if (tid >= 6 * n) return;
+    const size_t k = tid / n, i = tid - k * n;
+    if (TO_F32) {
+        const double2 *s = reinterpret_cast<const double2 *>(src);
+        const double2 a = s[(2 * k) * n + i], b = s[(2 * k + 1) * n + i];
+        reinterpret_cast<float4 *>(dst)[k * n + i] = make_float4((float)a.x, (float)a.y, (float)b.x, (float)b.y);
+    } else {
+        const float4 v = reinterpret_cast<const float4 *>(src)[k * n + i];
+        double2 *d = reinterpret_cast<double2 *>(dst);
+        d[(2 * k) * n + i] = make_double2(v.x, v.y);
+        d[(2 * k + 1) * n + i] = make_double2(v.z, v.w);
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_gauge_reorder(const Geom &g, const double *canon_dev, long site_lo, long n_sites, void *gauge64, void *gauge32,
+                                 int fmt32, unsigned long long *max_dev_bits, cudaStream_t s)
+{
+    const long n = 4 * n_sites;
+    gauge_reorder_kernel<<<(unsigned)((n + LB - 1) / LB), LB, 0, s>>>(g, canon_dev, site_lo, n_sites, (char *)gauge64, (char *)gauge32,
+                                                                     fmt32, max_dev_bits);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_spinor_pack(cola_prec prec, const Geom &g, const void *canon, void *internal, cudaStream_t s)
+{
+    const long n = 2L * g.Vh;
+    const unsigned grid = (unsigned)((n + LB - 1) / LB);
+    if (prec == COLA_F64) spinor_layout_kernel<double, true><<<grid, LB, 0, s>>>(g, (const double *)canon, nullptr, nullptr, internal);
+    else spinor_layout_kernel<float, true><<<grid, LB, 0, s>>>(g, (const float *)canon, nullptr, nullptr, internal);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_spinor_unpack(cola_prec prec, const Geom &g, const void *internal, void *canon, cudaStream_t s)
+{
+    const long n = 2L * g.Vh;
+    const unsigned grid = (unsigned)((n + LB - 1) / LB);
+    if (prec == COLA_F64) spinor_layout_kernel<double, false><<<grid, LB, 0, s>>>(g, nullptr, (double *)canon, internal, nullptr);
+    else spinor_layout_kernel<float, false><<<grid, LB, 0, s>>>(g, nullptr, (float *)canon, internal, nullptr);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_spinor_convert(cola_prec dst_prec, const void *src, void *dst, size_t n_sites, cudaStream_t s)
+{
+    const size_t n = 6 * n_sites;
+    const unsigned grid = (unsigned)((n + LB - 1) / LB);
+    if (dst_prec == COLA_F32) convert_kernel<true><<<grid, LB, 0, s>>>(src, dst, n_sites);
+    else convert_kernel<false><<<grid, LB, 0, s>>>(src, dst, n_sites);
+    return cudaGetLastError();
+}
+
+}  // namespace cola
