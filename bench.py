@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""Benchmark of the COLA hot path on B200 (contract: see the task statement).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+
+One STEP = one pass of the whole hot path over one source: a mixed-precision (fp32 inner, fp64 reliable
+updates) even-odd CGNR solve of M x = b to |r| <= 1e-10 |b|, i.e. source preparation, ~2 Schur-operator
+applications (4 fused dslash+clover kernels) and 2 fused BLAS-1 kernels per iteration, reliable updates in
+fp64, reconstruction of the odd sites and the fp64 true residual -- SURVEY.md 8(a) H3-H12.  The gauge upload
++ clover build/inversion (H0-H2) is setup and is timed separately ("setup_s").
+
+metric  = Dirac-operator GFLOP/s sustained over the solve, counted flops (1320/site hopping term, 504/site
+          clover, 48/site xpay) / device time, whole job over all ranks (BASELINE.json "metric").
+e2e     = the same through cola_cg_solve_host: b in pinned HOST memory, x returned to pinned HOST memory.
+roofline= the dominant kernel (fused dslash + clover + xpay, fp32 with 12-real links) timed alone with CUDA
+          events: algorithmic bytes per launch / average launch time, against MEASURED_PEAKS.json hbm_gbs.
+N > 1   : replicas only (the path has no inter-GPU exchange): every rank solves its own
+          source on its own GPU; value = all ranks' flops / max-over-ranks time ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+from paper_2302_00850_b200 import inputs  # noqa: E402
+
+# algorithmic bytes per output site, fp32 with 12-real links; fp64 x18 in the second column
+BYTES = {
+    "dslash": {"f32x12": 576, "f32x18": 768, "f64x18": 1536},          # 8 links + 1 spinor in + 1 out
+    "dslash_clover_inv": {"f32x12": 864, "f32x18": 1056, "f64x18": 2112},   # + 72 reals clover
+    "dslash_clover_xpay": {"f32x12": 960, "f32x18": 1152, "f64x18": 2304},  # + 72 clover + 24 (x)
+}
+FLOPS = {"dslash": 1320, "dslash_clover_inv": 1824, "dslash_clover_xpay": 1872}
+NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star's denominator, reported beside the measured one
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (torch copy, read+write)"
+    return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md; MEASURED_PEAKS.json absent)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([f.strip() for f in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        pw = [float(r[2]) for r in self.rows if len(r) >= 7 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def aggregate_over_ranks(local_ms: float, local_units: float, device=None):
+    """(max-over-ranks time, sum-over-ranks units).  Works on any initialised process group (nccl or gloo)."""
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()):
+        return local_ms, local_units
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def time_launches(fn, n_warm, n_timed):
+    """Average device time (ms) of fn() over n_timed calls, CUDA events on the current stream."""
+    for _ in range(n_warm):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(n_timed):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / n_timed
+
+
+def operator_table(ctx, fmt32, n_warm=20, n_timed=200):
+    """Per-kernel throughput of the operator family, each timed alone (inputs larger than L2)."""
+    peak, _ = measured_peaks()
+    out = {}
+    Vh = ctx.Vh
+    for prec, fmt in ((torch.float32, fmt32), (torch.float64, "f64x18")):
+        full = ctx.empty_internal(prec, full=True).normal_()
+        dst = ctx.empty_internal(prec, full=True)
+        rows = {
+            "dslash_even": ("dslash", 1, lambda: ctx.dslash_apply(0, full[1], out=dst[0])),
+            "dslash_odd": ("dslash", 1, lambda: ctx.dslash_apply(1, full[0], out=dst[1])),
+            "fermion_matrix": ("dslash_clover_xpay", 2, lambda: ctx.fermion_matrix_apply(full, out=dst)),
+            "schur": (None, 2, lambda: ctx.schur_apply(full[0], out=dst[0])),
+        }
+        for name, (kind, launches, fn) in rows.items():
+            ms = time_launches(fn, n_warm, n_timed)
+            if kind is None:   # Schur = dslash+A^-1 then dslash+A+xpay
+                nbytes = (BYTES["dslash_clover_inv"][fmt] + BYTES["dslash_clover_xpay"][fmt]) * Vh
+                flops = (FLOPS["dslash_clover_inv"] + FLOPS["dslash_clover_xpay"]) * Vh
+            else:
+                nbytes = BYTES[kind][fmt] * Vh * launches
+                flops = FLOPS[kind] * Vh * launches
+            gbs = nbytes / (ms * 1e-3) / 1e9
+            out[f"{name}_{fmt}"] = {"ms": round(ms, 5), "launches": launches, "GB/s": round(gbs, 1), "GFLOP/s": round(flops / (ms * 1e-3) / 1e9, 1),
+                                    "frac_measured": round(gbs / peak, 4), "frac_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4)}
+        del full, dst
+    return out
+
+
+def cpu_baseline_sample(cfg, U_cpu, n_pairs=2):
+    """The oracle as it stands on the host cores: n_pairs x (S, S^dagger) applications on the same lattice."""
+    import numpy as np
+
+    import oracle
+
+    dims, kappa, csw = cfg["dims"], cfg["kappa"], cfg["csw"]
+    Un = U_cpu.numpy()
+    A = oracle.clover(dims, Un, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    x = (inputs.source_gaussian(dims, 77) * torch.from_numpy(oracle.parity_mask(dims) == 0)[..., None, None]).numpy()
+    Vh = inputs.volume(dims) // 2
+    t0 = time.time()
+    for _ in range(n_pairs):
+        y = oracle.schur(dims, inputs.BC, Un, A, Ainv, kappa, x)
+        x = oracle.schur(dims, inputs.BC, Un, A, Ainv, kappa, y, dagger=True)
+        x = x / np.linalg.norm(x.ravel())
+    dt = time.time() - t0
+    flops = n_pairs * 2 * 3696.0 * Vh
+    return {"value": round(flops / dt / 1e9, 3), "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{n_pairs} x (S, S^dagger) oracle applications on the full {dims} lattice = the operator work of {n_pairs} CGLS iterations, {dt:.1f} s",
+            "seconds": round(dt, 2)}
+
+
+def reference_arm(args, cfg, workload):
+    """--impl reference: the CPU oracle (this tier's reference arm) on the host cores, rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+
+    import oracle
+
+    dims, kappa, csw = cfg["dims"], cfg["kappa"], cfg["csw"]
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    U = inputs.make_links(args.config, device=dev).cpu()
+    Un = U.numpy()
+    A = oracle.clover(dims, Un, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    x = (inputs.source_gaussian(dims, 77) * torch.from_numpy(oracle.parity_mask(dims) == 0)[..., None, None]).numpy()
+    Vh = inputs.volume(dims) // 2
+
+    def step(x):
+        y = oracle.schur(dims, inputs.BC, Un, A, Ainv, kappa, x)
+        x = oracle.schur(dims, inputs.BC, Un, A, Ainv, kappa, y, dagger=True)
+        return x / np.linalg.norm(x.ravel())
+
+    for _ in range(args.warmup):
+        x = step(x)
+    t0 = time.time()
+    for _ in range(args.steps):
+        x = step(x)
+    dt = time.time() - t0
+    val = args.steps * 2 * 3696.0 * Vh / dt / 1e9
+    sample = f"each step = one (S, S^dagger) oracle application pair on the full {dims} lattice (operator work of one CGLS iteration)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": round(val, 3), "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": round(dt / args.steps * 1e3, 2), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload,
+        "cpu_baseline": {"value": round(val, 3), "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": round(val, 3), "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+METRIC = "Dirac-op GFLOP/s (counted flops) sustained over a mixed-precision even-odd CGNR solve to 1e-10"
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[K] (default 2: 32^3x64, fp32 12-real links)")
+    ap.add_argument("--impl", default="cola", choices=["cola", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-operator-table", action="store_true")
+    args = ap.parse_args()
+
+    cfg = inputs.CONFIGS[args.config]
+    dims = cfg["dims"]
+    workload = {
+        "workload": f"BASELINE.json configs[{args.config}]: {dims[0]}x{dims[1]}x{dims[2]}x{dims[3]} lattice, links exp(i*{cfg['eps']}*H) seeded, "
+                    f"kappa={cfg['kappa']}, csw={cfg['csw']}, bc=(+,+,+,-), Gaussian source, fp32 links stored as 12 reals; "
+                    "step = mixed-precision (fp32 inner / fp64 reliable updates, delta=0.1) even-odd CGNR to 1e-10",
+        "lattice": list(dims), "kappa": cfg["kappa"], "csw": cfg["csw"], "tol": 1e-10, "parallelism": f"replicas x{args.gpus}",
+        "l2": "inputs larger than L2 (fp32 gauge+clover alone are > 1 GB per operator application at 32^3x64)",
+    }
+    if args.impl == "reference":
+        return reference_arm(args, cfg, workload)
+
+    from paper_2302_00850_b200 import binding   # raises if libcola.so is missing: no CPU fallback
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the COLA hot path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+
+    # ---- setup (H0-H2), not part of a step
+    U = inputs.make_links(args.config, device=dev)
+    b = inputs.source_gaussian(dims, inputs.config_seed_source(args.config) + rank, device=dev)
+    ctx = binding.Cola(dims, cfg["kappa"], cfg["csw"], bc=inputs.BC, compress12=True, device=local)
+    torch.cuda.synchronize()
+    t0 = time.time()
+    ctx.gauge_upload(U)
+    torch.cuda.synchronize()
+    setup_s = time.time() - t0
+    U_cpu = U.cpu() if (rank == 0 and world == 1 and not args.no_cpu_baseline) else None
+    del U
+    torch.cuda.empty_cache()
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident steps
+    for _ in range(args.warmup):
+        x, info = ctx.cg_solve(b, tol=1e-10, even_odd=True, mixed=True)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    flops = 0.0
+    for _ in range(args.steps):
+        x, info = ctx.cg_solve(b, tol=1e-10, even_odd=True, mixed=True)
+        flops += info["op_flops"]
+    e1.record()
+    barrier()
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop()
+    ms_local = e0.elapsed_time(e1)
+    ms, flops_all = aggregate_over_ranks(ms_local, flops, device=dev)
+    value = flops_all / (ms * 1e-3) / 1e9
+
+    # ---- end to end: host buffers through cola_cg_solve_host
+    b_host = b.cpu().pin_memory()
+    x_host = torch.empty_like(b_host).pin_memory()
+    ctx.cg_solve(b_host, tol=1e-10, even_odd=True, mixed=True, x=x_host)
+    barrier()
+    e0.record()
+    flops_e = 0.0
+    for _ in range(args.steps):
+        _, info_e = ctx.cg_solve(b_host, tol=1e-10, even_odd=True, mixed=True, x=x_host)
+        flops_e += info_e["op_flops"]
+    e1.record()
+    barrier()
+    ms_e, flops_e_all = aggregate_over_ranks(e0.elapsed_time(e1), flops_e, device=dev)
+    nbytes = b_host.numel() * b_host.element_size()
+
+    if rank != 0:
+        if world > 1:
+            torch.distributed.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel + operator table (rank 0, kernels timed alone)
+    peak, peak_src = measured_peaks()
+    table = {} if args.no_operator_table else operator_table(ctx, "f32x12")
+    roof = None
+    if table:
+        k = table["fermion_matrix_f32x12"]   # two launches of the fused dslash + clover + xpay kernel
+        per_launch_bytes = BYTES["dslash_clover_xpay"]["f32x12"] * ctx.Vh
+        roof = {"kernel": "dslash_kernel<F32x12, XPAY=A*y+c*v> (Schur kernel 2 / M), timed alone through cola_fermion_matrix_apply (2 launches per call)",
+                "bound": "hbm", "achieved": k["GB/s"], "peak": peak, "unit": "GB/s", "frac": round(k["GB/s"] / peak, 4),
+                "frac_of_nominal_8TBs": round(k["GB/s"] / NOMINAL_HBM_GBS, 4), "peak_source": peak_src + " (burst figure; kernel timed alone)",
+                "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": round(k["ms"] / 2, 5), "traffic": None}
+        prof = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(prof):
+            roof["traffic"] = json.load(open(prof)).get("dslash_clover_xpay_f32x12_bytes_per_launch")
+    cpu = None
+    if U_cpu is not None:
+        cpu = cpu_baseline_sample(cfg, U_cpu)
+
+    line = {
+        "metric": METRIC, "value": round(value, 1), "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": round(ms / args.steps, 3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": workload,
+        "solve": {"iters": info["iters"], "reliable_updates": info["reliable_updates"], "true_residual": info["true_residual"],
+                  "time_to_solution_s": round(ms / args.steps * 1e-3, 5), "converged": info["converged"]},
+        "setup_s": round(setup_s, 3),
+        "e2e": {"value": round(flops_e_all / (ms_e * 1e-3) / 1e9, 1), "unit": "GFLOP/s", "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                "ms_per_step": round(ms_e / args.steps, 3)},
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "cpu_baseline": cpu, "operators": table,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
