@@ -42,6 +42,9 @@ BYTES = {
     "dslash_clover_xpay": {"f32x12": 960, "f32x18": 1152, "f64x18": 2304},  # + 72 clover + 24 (x)
 }
 FLOPS = {"dslash": 1320, "dslash_clover_inv": 1824, "dslash_clover_xpay": 1872}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of dslash_kernel<F32x12, XPAY=2> from the committed
+# ncu --set full capture (a number read from a profile, never a timing taken under the profiler)
+NCU_TRAFFIC = {(32, 32, 32, 64): {"bytes_per_launch": 980312832, "source": "profiles/r1_dslash_f32x12_full.txt (909.34 MB read + 70.98 MB write)"}}
 NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star's denominator, reported beside the measured one
 
 
@@ -322,9 +325,9 @@ def main():
                 "bound": "hbm", "achieved": k["GB/s"], "peak": peak, "unit": "GB/s", "frac": round(k["GB/s"] / peak, 4),
                 "frac_of_nominal_8TBs": round(k["GB/s"] / NOMINAL_HBM_GBS, 4), "peak_source": peak_src + " (burst figure; kernel timed alone)",
                 "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": round(k["ms"] / 2, 5), "traffic": None}
-        prof = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(prof):
-            roof["traffic"] = json.load(open(prof)).get("dslash_clover_xpay_f32x12_bytes_per_launch")
+        if tuple(dims) in NCU_TRAFFIC:
+            roof["traffic"] = NCU_TRAFFIC[tuple(dims)]["bytes_per_launch"]
+            roof["traffic_source"] = NCU_TRAFFIC[tuple(dims)]["source"]
     cpu = None
     if U_cpu is not None:
         cpu = cpu_baseline_sample(cfg, U_cpu)
