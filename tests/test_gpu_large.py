@@ -1,0 +1,151 @@
+"""Full-size parity at BASELINE.json configs 2, 3, 4 (32^3x64, 48^3x96, 64^3x128), in the launch configuration
+bench.py times.  The oracle cannot sweep these lattices in seconds, so:
+  * operators are compared on sampled output sites the oracle evaluates one by one (>= 4096 seeded random sites
+    per parity, all 16 lattice corners, a strip of the boundary time-slices that exercises wrap and BC);
+  * the 32^3x64 solve is compared with the stored oracle solve (tests/golden/solver_golden.json: iterations,
+    sampled solution values, norm);
+  * larger solves are checked through the residual b - M x evaluated by the ORACLE at sampled sites and through
+    the global residual norm the library reports.
+Links are generated on the GPU with the seeded generator (same integer hash as on the CPU, floating point equal
+to rounding) and copied to the host for the oracle.
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2302_00850_b200 import inputs
+
+pytestmark = [pytest.mark.gpu, pytest.mark.large]
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "solver_golden.json")
+TOL = {torch.float64: 1e-12, torch.float32: 2e-6}
+
+
+def sample_sites(dims, n_random, seed):
+    lx, ly, lz, lt = dims
+    V = lx * ly * lz * lt
+    rng = np.random.default_rng(seed)
+    sites = set(int(s) for s in rng.integers(0, V, size=2 * n_random + 64))
+    for cx in (0, lx - 1):
+        for cy in (0, ly - 1):
+            for cz in (0, lz - 1):
+                for ct in (0, lt - 1):
+                    sites.add(cx + lx * (cy + ly * (cz + lz * ct)))
+    # a strip of both boundary time-slices (first x-y plane at z = 0 and z = Lz-1)
+    for ct in (0, lt - 1):
+        for cz in (0, lz - 1):
+            base = lx * ly * (cz + lz * ct)
+            sites.update(range(base, base + lx * ly))
+    return np.array(sorted(sites), dtype=np.int64)
+
+
+def parity_of(dims, sites):
+    lx, ly, lz, lt = dims
+    x = sites % lx
+    y = (sites // lx) % ly
+    z = (sites // (lx * ly)) % lz
+    t = sites // (lx * ly * lz)
+    return (x + y + z + t) & 1
+
+
+def rel(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+class Big:
+    def __init__(self, k):
+        from paper_2302_00850_b200 import binding
+
+        self.k = k
+        self.cfg = inputs.CONFIGS[k]
+        self.dims = self.cfg["dims"]
+        U = inputs.make_links(k, device="cuda")
+        self.ctx = binding.Cola(self.dims, self.cfg["kappa"], self.cfg["csw"], bc=inputs.BC, compress12=True)
+        self.ctx.gauge_upload(U)
+        self.Un = U.cpu().numpy()
+        del U
+        torch.cuda.empty_cache()
+        self.sites = sample_sites(self.dims, 4096, 7000 + k)
+        self.par = parity_of(self.dims, self.sites)
+
+    def close(self):
+        self.ctx.close()
+        torch.cuda.empty_cache()
+
+
+@pytest.fixture(scope="module", params=[2, 3, 4])
+def big(request):
+    b = Big(request.param)
+    yield b
+    b.close()
+
+
+def at_sites(canon, sites):
+    return canon.reshape(-1, 4, 3)[torch.from_numpy(sites).to(canon.device)].cpu().numpy()
+
+
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64])
+def test_operators_on_sampled_sites(big, dtype):
+    c, dims, cfg = big.ctx, big.dims, big.cfg
+    assert len(big.sites) >= 8192 and (big.par == 0).sum() >= 4096 and (big.par == 1).sum() >= 4096
+    psi = inputs.source_gaussian(dims, 4242 + big.k, device="cuda")
+    psin = psi.cpu().numpy()
+    ct = torch.complex128 if dtype == torch.float64 else torch.complex64
+    internal = c.spinor_pack(psi.to(ct))
+    args = (dims, inputs.BC, big.Un, cfg["kappa"], cfg["csw"])
+    # full hopping term = the two parity dslashes
+    out = torch.empty_like(internal)
+    c.dslash_apply(0, internal[1], out=out[0])
+    c.dslash_apply(1, internal[0], out=out[1])
+    got = at_sites(c.spinor_unpack(out), big.sites)
+    assert rel(got, oracle.apply_sites(*args, "D", psin, big.sites)) < TOL[dtype]
+    for which, dagger in (("M", False), ("Mdag", True)):
+        got = at_sites(c.spinor_unpack(c.fermion_matrix_apply(internal, dagger=dagger)), big.sites)
+        assert rel(got, oracle.apply_sites(*args, which, psin, big.sites)) < TOL[dtype]
+    even = big.sites[big.par == 0]
+    for which, dagger in (("S", False), ("Sdag", True)):
+        out.zero_()
+        c.schur_apply(internal[0], dagger=dagger, out=out[0])
+        got = at_sites(c.spinor_unpack(out), even)
+        assert rel(got, oracle.apply_sites(*args, which, psin, even)) < TOL[dtype]
+
+
+def test_mixed_precision_solve(big):
+    c, dims, cfg, k = big.ctx, big.dims, big.cfg, big.k
+    if cfg["source"] == "point":
+        b = inputs.source_point(dims, 1, 2, device="cuda")        # one of BJ:c3's 12 spin-colour sources
+    else:
+        b = inputs.source_gaussian(dims, inputs.config_seed_source(k), device="cuda")
+    x, info = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=True)
+    assert info["converged"] and info["true_residual"] <= 1.05e-10 and info["reliable_updates"] >= 2
+    # residual evaluated by the ORACLE at the sampled sites vs the library's own residual field there
+    xn, bn = x.cpu().numpy(), b.cpu().numpy()
+    Mx = oracle.apply_sites(dims, inputs.BC, big.Un, cfg["kappa"], cfg["csw"], "M", xn, big.sites)
+    r_or = bn.reshape(-1, 4, 3)[big.sites] - Mx
+    Mx_gpu = c.spinor_unpack(c.fermion_matrix_apply(c.spinor_pack(x)))
+    r_gpu = at_sites(b - Mx_gpu, big.sites)
+    bnorm = float(torch.linalg.vector_norm(b).item())
+    # per-site residuals agree to fp64 rounding of the operator (|M x| ~ |b| locally)
+    assert np.abs(r_or - r_gpu).max() <= 1e-12 * max(1.0, np.abs(Mx).max())
+    # the sampled sites carry their share of a 1e-10 residual: rms over the sample extrapolated to the volume
+    V = inputs.volume(dims)
+    est = math.sqrt(float((np.abs(r_or) ** 2).sum()) * V / len(big.sites)) / bnorm
+    if cfg["source"] != "point":
+        assert est <= 3e-10
+    glob = float(torch.linalg.vector_norm(b - Mx_gpu).item()) / bnorm
+    assert abs(glob - info["true_residual"]) <= 1e-3 * glob + 1e-14
+    if k == 2:
+        g = json.load(open(GOLD))["2"]["eo"]
+        assert abs(info["iters"] - g["iters"]) <= max(1, math.ceil(0.02 * g["iters"]))
+        xs = xn.reshape(-1, 12)[np.array(g["sites"])]
+        want = np.array(g["x_re"]) + 1j * np.array(g["x_im"])
+        assert np.linalg.norm(xs - want) / np.linalg.norm(want) < 5e-8
+        assert abs(np.linalg.norm(xn.ravel()) - g["x_norm"]) / g["x_norm"] < 1e-8
+        # pure fp64 solve: same count
+        x64, info64 = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=False)
+        assert info64["converged"] and abs(info64["iters"] - g["iters"]) <= max(1, math.ceil(0.02 * g["iters"]))
+        assert rel(x64.cpu().numpy(), xn) < 5e-9
