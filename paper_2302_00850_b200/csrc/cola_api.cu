@@ -22,13 +22,16 @@ struct cola_ctx {
     char *clovA64, *clovA32;        // [parity][chunk][Vh]
     char *clovI64, *clovI32;        // odd parity only
     char *tmp64, *tmp32;            // odd half-lattice temporaries of the Schur operator
-    double *partials;
+    ReduceWs red;                   // deterministic-reduction buffers
+    size_t red_blocks;              // max grid size of a reducing launch
     char *scratch;                  // solver vectors / staging
     size_t scratch_bytes;
     // owned
     Ctl *ctl;                       // device
     unsigned long long *max_dev_bits;   // device (inside the same allocation)
     double *h_pinned;               // pinned host scalars
+    HostStatus *h_status;           // mapped pinned host memory the device publishes the iteration status to
+    HostStatus *d_status;           // device alias of h_status
     cudaEvent_t ev0, ev1;
     int ready;
     double max_unitarity_dev;
@@ -77,7 +80,11 @@ static Carve carve(const cola_ctx *c)
     k.clovI32 = take(288 * Vh);
     k.tmp64 = take(192 * Vh);
     k.tmp32 = take(96 * Vh);
-    k.partials = take(((Vh + 127) / 128 + 4096) * sizeof(double));
+    {
+        size_t nb = dslash_grid_blocks(Vh);
+        if (nb < (size_t)blas_max_blocks()) nb = (size_t)blas_max_blocks();
+        k.partials = take((nb + reduce_groups(nb)) * sizeof(double) + reduce_groups(nb) * sizeof(unsigned));
+    }
     k.scratch = take(SCRATCH_HALF64 * 192 * Vh);
     k.total = off;
     return k;
@@ -114,9 +121,13 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     char *blk = nullptr;
     cudaError_t e = cudaMalloc(&blk, 4096);
     if (e == cudaSuccess) e = cudaMemset(blk, 0, 4096);
-    if (e == cudaSuccess) e = cudaHostAlloc(&c->h_pinned, 256, cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaHostAlloc(&c->h_pinned, 1024, cudaHostAllocMapped);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    if (e == cudaSuccess) {
+        c->h_status = reinterpret_cast<HostStatus *>(reinterpret_cast<char *>(c->h_pinned) + 256);
+        e = cudaHostGetDevicePointer(reinterpret_cast<void **>(&c->d_status), c->h_status, 0);
+    }
     if (e != cudaSuccess) {
         fail(nullptr, COLA_ECUDA, "cola_create: %s", cudaGetErrorString(e));
         if (blk) cudaFree(blk);
@@ -172,7 +183,16 @@ cola_status cola_set_workspace(cola_ctx *c, void *dev_ptr, size_t bytes)
     c->clovA64 = c->ws + k.clovA64; c->clovA32 = c->ws + k.clovA32;
     c->clovI64 = c->ws + k.clovI64; c->clovI32 = c->ws + k.clovI32;
     c->tmp64 = c->ws + k.tmp64; c->tmp32 = c->ws + k.tmp32;
-    c->partials = (double *)(c->ws + k.partials);
+    {
+        size_t nb = dslash_grid_blocks(c->Vh);
+        if (nb < (size_t)blas_max_blocks()) nb = (size_t)blas_max_blocks();
+        c->red_blocks = nb;
+        c->red.partials = (double *)(c->ws + k.partials);
+        c->red.gpart = c->red.partials + nb;
+        c->red.gticket = (unsigned *)(c->red.gpart + reduce_groups(nb));
+        cudaError_t e = cudaMemsetAsync(c->red.gticket, 0, reduce_groups(nb) * sizeof(unsigned), c->stream);
+        if (e != cudaSuccess) return fail(c, COLA_ECUDA, "cola_set_workspace: %s", cudaGetErrorString(e));
+    }
     c->scratch = c->ws + k.scratch;
     c->scratch_bytes = SCRATCH_HALF64 * 192 * c->Vh;
     return COLA_OK;
@@ -205,7 +225,7 @@ static char *tmp_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64
 
 // out_p = [post] ( [A] y + coef * D_{p,1-p} in ), optional |out|^2 -> norm_out
 static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, const void *in, void *out, const void *y, int clov_on_y,
-                          double coef, int post_inv, double *norm_out, int norm_accumulate)
+                          double coef, int post_inv, double *norm_out, int norm_accumulate, const int *skip = nullptr)
 {
     DslashArgs a;
     memset(&a, 0, sizeof(a));
@@ -220,8 +240,9 @@ static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, c
     a.coef = coef;
     a.sgn = dagger ? +1.0 : -1.0;
     a.parity = parity;
+    a.skip = skip;
     if (norm_out) {
-        a.partials = c->partials;
+        a.red = c->red;
         a.counter = &c->ctl->counter[0];
         a.norm_out = norm_out;
         a.norm_accumulate = norm_accumulate;
@@ -233,22 +254,22 @@ static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, c
 }
 
 // out_e = S in_e  (2 launches; norm of the result optional)
-static cola_status schur(cola_ctx *c, cola_prec prec, int dagger, const void *in_e, void *out_e, double *norm_out)
+static cola_status schur(cola_ctx *c, cola_prec prec, int dagger, const void *in_e, void *out_e, double *norm_out, const int *skip = nullptr)
 {
     const double k = c->p.kappa;
-    ST(dslash(c, prec, 1, dagger, in_e, tmp_of(c, prec), nullptr, 0, 0.0, 1, nullptr, 0));          // t_o = A_oo^-1 D_oe x_e
-    ST(dslash(c, prec, 0, dagger, tmp_of(c, prec), out_e, in_e, 1, -k * k, 0, norm_out, 0));        // A_ee x_e - k^2 D_eo t_o
+    ST(dslash(c, prec, 1, dagger, in_e, tmp_of(c, prec), nullptr, 0, 0.0, 1, nullptr, 0, skip));          // t_o = A_oo^-1 D_oe x_e
+    ST(dslash(c, prec, 0, dagger, tmp_of(c, prec), out_e, in_e, 1, -k * k, 0, norm_out, 0, skip));        // A_ee x_e - k^2 D_eo t_o
     return COLA_OK;
 }
 
 // out = M in on the full lattice (2 launches)
-static cola_status fmatrix(cola_ctx *c, cola_prec prec, int dagger, const void *in, void *out, double *norm_out)
+static cola_status fmatrix(cola_ctx *c, cola_prec prec, int dagger, const void *in, void *out, double *norm_out, const int *skip = nullptr)
 {
     const size_t hb = half_bytes(c, prec);
     const char *in_e = (const char *)in, *in_o = in_e + hb;
     char *out_e = (char *)out, *out_o = out_e + hb;
-    ST(dslash(c, prec, 0, dagger, in_o, out_e, in_e, 1, -c->p.kappa, 0, norm_out, 0));
-    ST(dslash(c, prec, 1, dagger, in_e, out_o, in_o, 1, -c->p.kappa, 0, norm_out, 1));
+    ST(dslash(c, prec, 0, dagger, in_o, out_e, in_e, 1, -c->p.kappa, 0, norm_out, 0, skip));
+    ST(dslash(c, prec, 1, dagger, in_e, out_o, in_o, 1, -c->p.kappa, 0, norm_out, 1, skip));
     return COLA_OK;
 }
 
@@ -262,7 +283,7 @@ static cola_status read_scalar(cola_ctx *c, const double *dev, double *host)
 
 static cola_status norm2(cola_ctx *c, cola_prec prec, const void *v, size_t n_sites, double *dev_out)
 {
-    CK(launch_norm2(prec, v, n_sites, c->partials, &c->ctl->counter[2], dev_out, c->stream));
+    CK(launch_norm2(prec, v, n_sites, c->red, &c->ctl->counter[2], dev_out, c->stream));
     c->launches++;
     return COLA_OK;
 }
@@ -321,9 +342,65 @@ struct System {            // K x = rhs on n_sites sites; K = S (even_odd) or M
     size_t n_sites;
 };
 
-cola_status apply_K(cola_ctx *c, const System &sy, cola_prec prec, int dagger, const void *in, void *out, double *norm_out)
+cola_status apply_K(cola_ctx *c, const System &sy, cola_prec prec, int dagger, const void *in, void *out, double *norm_out, const int *skip = nullptr)
 {
-    return sy.even_odd ? schur(c, prec, dagger, in, out, norm_out) : fmatrix(c, prec, dagger, in, out, norm_out);
+    return sy.even_odd ? schur(c, prec, dagger, in, out, norm_out, skip) : fmatrix(c, prec, dagger, in, out, norm_out, skip);
+}
+
+// (re)arm the device-side decision state: rmax2, target2, delta2, flag = 0, iters
+cola_status set_decision_state(cola_ctx *c, double rmax2, double target2, double delta2, int iters)
+{
+    struct { double rmax2, target2, delta2; int flag, iters; } st = {rmax2, target2, delta2, 0, iters};
+    static_assert(sizeof(st) == 32, "decision block layout");
+    static_assert(offsetof(Ctl, iters) - offsetof(Ctl, rmax2) == 28, "decision block layout");
+    // pageable source: the runtime stages it before returning, so the stack buffer may die
+    CK(cudaMemcpyAsync(&c->ctl->rmax2, &st, sizeof(st), cudaMemcpyHostToDevice, c->stream));
+    return COLA_OK;
+}
+
+// Wait until iteration k's r_update has published its status (slot k & 1, sequence number k + 1).  The device
+// writes straight into mapped pinned memory, so this is a poll on host memory, not a stream synchronisation;
+// the stream is queried now and then so that a faulted kernel cannot hang the caller.
+cola_status wait_status(cola_ctx *c, int k, HostStatus *out)
+{
+    volatile HostStatus *m = c->h_status + (k & 1);
+    for (unsigned long spins = 0;; spins++) {
+        if (m->iters == k + 1) break;
+        if ((spins & 0xfff) == 0xfff) {
+            cudaError_t e = cudaStreamQuery(c->stream);
+            if (e == cudaSuccess) {
+                if (m->iters == k + 1) break;
+                return fail(c, COLA_ECUDA, "cola_cg_solve: the stream drained without iteration status (internal error)");
+            }
+            if (e != cudaErrorNotReady) return fail(c, COLA_ECUDA, "cola_cg_solve: %s", cudaGetErrorString(e));
+        }
+        __builtin_ia32_pause();
+    }
+    __sync_synchronize();
+    out->rr = m->rr;
+    out->flag = m->flag;
+    out->iters = m->iters;
+    return COLA_OK;
+}
+
+// iteration k, first half:  q = K p (|q|^2),  r -= alpha q (|r|^2, decision, status -> mapped host slot k & 1)
+cola_status first_half(cola_ctx *c, const System &sy, cola_prec P, int k, char *ri, char *pi, char *qi)
+{
+    Ctl *ctl = c->ctl;
+    ST(apply_K(c, sy, P, 0, pi, qi, &ctl->qq, &ctl->flag));
+    CK(launch_r_update(P, ri, qi, ctl, k & 1, k + 1, &ctl->flag, c->d_status + (k & 1), sy.n_sites, c->red, c->stream));
+    c->launches++;
+    return COLA_OK;
+}
+
+// iteration k, second half:  s = K^+ r (|s|^2),  x += alpha p (do_x),  p = s + beta p
+cola_status second_half(cola_ctx *c, const System &sy, cola_prec P, int k, int do_x, char *xi, char *ri, char *pi, char *qi)
+{
+    Ctl *ctl = c->ctl;
+    ST(apply_K(c, sy, P, 1, ri, qi, &ctl->gam[(k & 1) ^ 1], &ctl->flag));
+    CK(launch_xp_update(P, xi, pi, qi, ctl, k & 1, do_x, 1, &ctl->flag, sy.n_sites, c->stream));
+    c->launches++;
+    return COLA_OK;
 }
 
 size_t vec_bytes(const cola_ctx *c, const System &sy, cola_prec prec) { return half_bytes(c, prec) * (sy.even_odd ? 1 : 2); }
@@ -401,89 +478,71 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
             ST(dslash(c, COLA_F64, 0, 0, c->tmp64, rhs, B, 0, kappa, 0, nullptr, 0));
             flops += (504.0 + 1320.0 + 48.0) * (double)c->Vh;
         }
-        const double target = sp->tol * bnorm;
-        if (!sp->mixed) {
-            // ---- fp64 CGLS
-            CK(cudaMemcpyAsync(r, rhs, nv64, cudaMemcpyDeviceToDevice, c->stream));
-            ST(apply_K(c, sy, COLA_F64, 1, r, qs, &ctl->gam[0]));
-            CK(cudaMemcpyAsync(p, qs, nv64, cudaMemcpyDeviceToDevice, c->stream));
-            flops += flops_K;
-            ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
-            ST(read_scalar(c, &ctl->rr, &rr));
-            status_conv = sqrt(rr) <= target;
-            for (int k = 0; !status_conv && k < sp->max_iter; k++) {
-                const int cur = k & 1;
-                ST(apply_K(c, sy, COLA_F64, 0, p, qs, &ctl->qq));
-                CK(launch_r_update(COLA_F64, r, qs, ctl, cur, sy.n_sites, c->partials, c->stream));
-                c->launches++;
-                ST(read_scalar(c, &ctl->rr, &rr));
-                iters = k + 1;
-                flops += flops_K;
-                if (sqrt(rr) <= target) {
-                    CK(launch_xp_update(COLA_F64, xsol, p, qs, ctl, cur, 1, 0, sy.n_sites, c->stream));
-                    c->launches++;
-                    status_conv = 1;
-                    break;
-                }
-                ST(apply_K(c, sy, COLA_F64, 1, r, qs, &ctl->gam[cur ^ 1]));
-                flops += flops_K;
-                const int last = (k + 1 == sp->max_iter);
-                CK(launch_xp_update(COLA_F64, xsol, p, qs, ctl, cur, 1, last ? 0 : 1, sy.n_sites, c->stream));
-                c->launches++;
-            }
-        } else {
-            // ---- mixed precision: fp32 CGLS with fp64 reliable updates, search direction kept
+        // CGLS; with `mixed` the inner vectors are fp32 and the fp64 residual is recomputed at reliable
+        // updates that keep the search direction.  The stop / reliable-update decision is taken on
+        // the device (r_update's last block raises ctl->flag); every kernel of the iteration is a no-op while the
+        // flag is up, so the host queues half an iteration ahead and reads the status with a lag instead of
+        // draining the stream once per iteration.
+        const double target2 = (sp->tol * bnorm) * (sp->tol * bnorm);
+        const double delta2 = sp->mixed ? delta * delta : 0.0;
+        const cola_prec P = sp->mixed ? COLA_F32 : COLA_F64;
+        char *xi = sp->mixed ? x32 : xsol, *ri = sp->mixed ? r32 : r, *pi = sp->mixed ? p32 : p, *qi = sp->mixed ? qs32 : qs;
+        const size_t nvi = sp->mixed ? nv32 : nv64;
+        const int nh = sy.even_odd ? 1 : 2;
+        if (sp->mixed) {
             CK(cudaMemsetAsync(x32, 0, nv32, c->stream));
             ST(axpby64(c, sy, r, 1.0, rhs, 0.0, nullptr, r32));         // r64 = rhs, r32 = float(r64)
-            ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
-            ST(read_scalar(c, &ctl->rr, &rr));
-            double rmax = sqrt(rr);
-            status_conv = sqrt(rr) <= target;
-            if (!status_conv) {
-                ST(apply_K(c, sy, COLA_F32, 1, r32, qs32, &ctl->gam[0]));
-                CK(cudaMemcpyAsync(p32, qs32, nv32, cudaMemcpyDeviceToDevice, c->stream));
-                flops += flops_K;
-            }
-            for (int k = 0; !status_conv && k < sp->max_iter; k++) {
-                const int cur = k & 1;
-                ST(apply_K(c, sy, COLA_F32, 0, p32, qs32, &ctl->qq));
-                CK(launch_r_update(COLA_F32, r32, qs32, ctl, cur, sy.n_sites, c->partials, c->stream));
-                c->launches++;
-                ST(read_scalar(c, &ctl->rr, &rr));
+        } else {
+            CK(cudaMemcpyAsync(r, rhs, nv64, cudaMemcpyDeviceToDevice, c->stream));
+        }
+        ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
+        ST(read_scalar(c, &ctl->rr, &rr));
+        status_conv = rr <= target2;
+        if (!status_conv) {
+            ST(set_decision_state(c, rr, target2, delta2, 0));
+            ST(apply_K(c, sy, P, 1, ri, qi, &ctl->gam[0]));             // s0 = K^+ r0, gamma_0
+            CK(cudaMemcpyAsync(pi, qi, nvi, cudaMemcpyDeviceToDevice, c->stream));
+            flops += flops_K;
+            c->h_status[0].iters = c->h_status[1].iters = 0;
+            ST(first_half(c, sy, P, 0, ri, pi, qi));
+            for (int k = 0;; k++) {
+                const int more = (k + 1 < sp->max_iter);
+                ST(second_half(c, sy, P, k, 1, xi, ri, pi, qi));        // speculative: skipped if iteration k raises the flag
+                if (more) ST(first_half(c, sy, P, k + 1, ri, pi, qi));
+                HostStatus hs;
+                ST(wait_status(c, k, &hs));
+                const HostStatus *st = &hs;
+                rr = st->rr;
                 iters = k + 1;
                 flops += flops_K;
-                double rn = sqrt(rr);
-                if (rn > rmax) rmax = rn;
-                int x_done = 0;
-                if (rn < delta * rmax || rn <= target) {
-                    // reliable update: x64 += x32 (+ the pending alpha p), r64 = rhs - K x64 in fp64
-                    CK(launch_xp_update(COLA_F32, x32, p32, qs32, ctl, cur, 1, 0, sy.n_sites, c->stream));
-                    c->launches++;
-                    x_done = 1;
-                    for (int h = 0; h < (sy.even_odd ? 1 : 2); h++) {
-                        CK(launch_accumulate(xsol + h * h64, x32 + h * h32, c->Vh, c->stream));
-                        c->launches++;
-                    }
-                    ST(apply_K(c, sy, COLA_F64, 0, xsol, qs, nullptr));
+                if (!st->flag) {
                     flops += flops_K;
-                    ST(axpby64(c, sy, r, 1.0, rhs, -1.0, qs, r32));
-                    ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
-                    ST(read_scalar(c, &ctl->rr, &rr));
-                    rn = sqrt(rr);
-                    rmax = rn;
-                    updates++;
-                    if (rn <= target) { status_conv = 1; break; }
+                    if (!more) break;
+                    continue;
                 }
-                ST(apply_K(c, sy, COLA_F32, 1, r32, qs32, &ctl->gam[cur ^ 1]));
-                flops += flops_K;
-                const int last = (k + 1 == sp->max_iter);
-                if (!x_done || !last) {
-                    CK(launch_xp_update(COLA_F32, x32, p32, qs32, ctl, cur, x_done ? 0 : 1, last ? 0 : 1, sy.n_sites, c->stream));
+                // iteration k converged (inner residual) or asks for a reliable update; x has not received alpha_k p_k yet
+                CK(launch_xp_update(P, xi, pi, qi, ctl, k & 1, 1, 0, nullptr, sy.n_sites, c->stream));
+                c->launches++;
+                if (!sp->mixed) { status_conv = 1; break; }
+                for (int h = 0; h < nh; h++) {
+                    CK(launch_accumulate(xsol + h * h64, x32 + h * h32, c->Vh, c->stream));   // x64 += x32, x32 = 0
                     c->launches++;
                 }
+                ST(apply_K(c, sy, COLA_F64, 0, xsol, qs, nullptr));
+                flops += flops_K;
+                ST(axpby64(c, sy, r, 1.0, rhs, -1.0, qs, r32));          // r64 = rhs - K x64, r32 = float(r64)
+                ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
+                ST(read_scalar(c, &ctl->rr, &rr));
+                updates++;
+                if (rr <= target2) { status_conv = 1; break; }
+                if (!more) break;
+                ST(set_decision_state(c, rr, target2, delta2, k + 1)); // rmax = |r64|, flag down
+                ST(second_half(c, sy, P, k, 0, xi, ri, pi, qi));        // same search direction: p = s + beta p
+                flops += flops_K;
+                ST(first_half(c, sy, P, k + 1, ri, pi, qi));
             }
-            if (!status_conv) {   // max_iter: fold the fp32 part into the fp64 iterate
-                for (int h = 0; h < (sy.even_odd ? 1 : 2); h++) {
+            if (!status_conv && sp->mixed) {   // max_iter: fold the fp32 part into the fp64 iterate
+                for (int h = 0; h < nh; h++) {
                     CK(launch_accumulate(xsol + h * h64, x32 + h * h32, c->Vh, c->stream));
                     c->launches++;
                 }
@@ -505,7 +564,7 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
         flops += 1872.0 * (double)c->V;
         double tr = 0.0;
         for (int h = 0; h < 2; h++) {
-            CK(launch_axpby64(nullptr, 1.0, B + h * h64, -1.0, t + h * h64, nullptr, c->Vh, c->partials, &c->ctl->counter[3], &ctl->aux[h], c->stream));
+            CK(launch_axpby64(nullptr, 1.0, B + h * h64, -1.0, t + h * h64, nullptr, c->Vh, &c->red, &c->ctl->counter[3], &ctl->aux[h], c->stream));
             c->launches++;
         }
         double a0, a1;

@@ -23,17 +23,18 @@ __device__ __forceinline__ float4 axpy(float a, const float4 &x, const float4 &y
 __device__ __forceinline__ double2 axpy(double a, const double2 &x, const double2 &y) { return make_double2(y.x + a * x.x, y.y + a * x.y); }
 
 template <typename T>
-__global__ void __launch_bounds__(BB) norm2_kernel(const typename VT<T>::V *v, size_t n, double *partials, unsigned *counter, double *out)
+__global__ void __launch_bounds__(BB) norm2_kernel(const typename VT<T>::V *v, size_t n, ReduceWs red, unsigned *counter, double *out)
 {
     double acc = 0.0;
     for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) acc += sq(v[k]);
-    grid_sum_finalize(acc, partials, counter, out);
+    grid_sum_finalize(acc, red, counter, out);
 }
 
 // r -= alpha q, alpha = gamma / qq;  rr = |r|^2
 template <typename T>
-__global__ void __launch_bounds__(BB) r_update_kernel(typename VT<T>::V *r, const typename VT<T>::V *q, Ctl *ctl, int cur, size_t n, double *partials)
+__global__ void __launch_bounds__(BB) r_update_kernel(typename VT<T>::V *r, const typename VT<T>::V *q, Ctl *ctl, int cur, int iter, const int *skip, HostStatus *mirror, size_t n, ReduceWs red)
 {
+    if (skip && *skip) return;
     const T ma = (T)(-(ctl->gam[cur] / ctl->qq));
     double acc = 0.0;
     for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) {
@@ -41,13 +42,29 @@ __global__ void __launch_bounds__(BB) r_update_kernel(typename VT<T>::V *r, cons
         r[k] = v;
         acc += sq(v);
     }
-    grid_sum_finalize(acc, partials, &ctl->counter[1], &ctl->rr);
+    double rr;
+    if (grid_sum_last(acc, red, &ctl->counter[1], &rr)) {
+        ctl->rr = rr;
+        ctl->iters = iter;
+        const double rmax2 = fmax(ctl->rmax2, rr);
+        ctl->rmax2 = rmax2;
+        const int flag = (rr <= ctl->target2 || rr < ctl->delta2 * rmax2) ? 1 : 0;
+        if (flag) ctl->flag = 1;
+        if (mirror) {   // publish to the host without a DMA copy in the stream
+            volatile HostStatus *m = mirror;
+            m->rr = rr;
+            m->flag = flag;
+            __threadfence_system();
+            m->iters = iter;
+        }
+    }
 }
 
 // x += alpha p (DO_X);  p = s + beta p (DO_P);  alpha = gamma/qq, beta = gamma_new/gamma
 template <typename T, bool DO_X, bool DO_P>
-__global__ void __launch_bounds__(BB) xp_update_kernel(typename VT<T>::V *x, typename VT<T>::V *p, const typename VT<T>::V *s, const Ctl *ctl, int cur, size_t n)
+__global__ void __launch_bounds__(BB) xp_update_kernel(typename VT<T>::V *x, typename VT<T>::V *p, const typename VT<T>::V *s, const Ctl *ctl, int cur, const int *skip, size_t n)
 {
+    if (skip && *skip) return;
     const T alpha = (T)(ctl->gam[cur] / ctl->qq);
     const T beta = (T)(ctl->gam[cur ^ 1] / ctl->gam[cur]);
     for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) {
@@ -60,7 +77,7 @@ __global__ void __launch_bounds__(BB) xp_update_kernel(typename VT<T>::V *x, typ
 // out64 = a*A + b*B; optional fp32 copy (internal fp32 layout needs chunk pairing, so this kernel works
 // per site-chunk pair: thread handles double2 chunks 2k, 2k+1 of site i = one float4 chunk k)
 __global__ void __launch_bounds__(BB) axpby64_kernel(double2 *out, double a, const double2 *A, double b, const double2 *B, float4 *out32,
-                                                     size_t n_sites, double *partials, unsigned *counter, double *norm_out)
+                                                     size_t n_sites, ReduceWs red, unsigned *counter, double *norm_out)
 {
     double acc = 0.0;
     const size_t n = 6 * n_sites;
@@ -84,7 +101,7 @@ __global__ void __launch_bounds__(BB) axpby64_kernel(double2 *out, double a, con
         if (out32) out32[k * n_sites + i] = make_float4((float)v0.x, (float)v0.y, (float)v1.x, (float)v1.y);
         acc += sq(v0) + sq(v1);
     }
-    if (partials) grid_sum_finalize(acc, partials, counter, norm_out);
+    if (red.partials) grid_sum_finalize(acc, red, counter, norm_out);
 }
 
 // x64 += x32; x32 = 0
@@ -107,52 +124,53 @@ __global__ void __launch_bounds__(BB) accumulate_kernel(double2 *x64, float4 *x3
 
 int blas_max_blocks() { return MAX_BLOCKS; }
 
-cudaError_t launch_norm2(cola_prec prec, const void *v, size_t n_sites, double *partials, unsigned *counter, double *out, cudaStream_t s)
+cudaError_t launch_norm2(cola_prec prec, const void *v, size_t n_sites, const ReduceWs &red, unsigned *counter, double *out, cudaStream_t s)
 {
     if (prec == COLA_F64) {
         const size_t n = 12 * n_sites;
-        norm2_kernel<double><<<blas_grid(n), BB, 0, s>>>((const double2 *)v, n, partials, counter, out);
+        norm2_kernel<double><<<blas_grid(n), BB, 0, s>>>((const double2 *)v, n, red, counter, out);
     } else {
         const size_t n = 6 * n_sites;
-        norm2_kernel<float><<<blas_grid(n), BB, 0, s>>>((const float4 *)v, n, partials, counter, out);
+        norm2_kernel<float><<<blas_grid(n), BB, 0, s>>>((const float4 *)v, n, red, counter, out);
     }
     return cudaGetLastError();
 }
 
-cudaError_t launch_r_update(cola_prec prec, void *r, const void *q, Ctl *ctl, int cur, size_t n_sites, double *partials, cudaStream_t s)
+cudaError_t launch_r_update(cola_prec prec, void *r, const void *q, Ctl *ctl, int cur, int iter, const int *skip, HostStatus *mirror, size_t n_sites, const ReduceWs &red, cudaStream_t s)
 {
     if (prec == COLA_F64) {
         const size_t n = 12 * n_sites;
-        r_update_kernel<double><<<blas_grid(n), BB, 0, s>>>((double2 *)r, (const double2 *)q, ctl, cur, n, partials);
+        r_update_kernel<double><<<blas_grid(n), BB, 0, s>>>((double2 *)r, (const double2 *)q, ctl, cur, iter, skip, mirror, n, red);
     } else {
         const size_t n = 6 * n_sites;
-        r_update_kernel<float><<<blas_grid(n), BB, 0, s>>>((float4 *)r, (const float4 *)q, ctl, cur, n, partials);
+        r_update_kernel<float><<<blas_grid(n), BB, 0, s>>>((float4 *)r, (const float4 *)q, ctl, cur, iter, skip, mirror, n, red);
     }
     return cudaGetLastError();
 }
 
 template <typename T>
-static void xp_dispatch(void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, size_t n, cudaStream_t s)
+static void xp_dispatch(void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, const int *skip, size_t n, cudaStream_t s)
 {
     typedef typename VT<T>::V V;
     const unsigned grid = blas_grid(n);
-    if (do_x && do_p) xp_update_kernel<T, true, true><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, n);
-    else if (do_x) xp_update_kernel<T, true, false><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, n);
-    else if (do_p) xp_update_kernel<T, false, true><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, n);
+    if (do_x && do_p) xp_update_kernel<T, true, true><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
+    else if (do_x) xp_update_kernel<T, true, false><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
+    else if (do_p) xp_update_kernel<T, false, true><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
 }
 
-cudaError_t launch_xp_update(cola_prec prec, void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, size_t n_sites, cudaStream_t s)
+cudaError_t launch_xp_update(cola_prec prec, void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, const int *skip, size_t n_sites, cudaStream_t s)
 {
-    if (prec == COLA_F64) xp_dispatch<double>(x, p, sv, ctl, cur, do_x, do_p, 12 * n_sites, s);
-    else xp_dispatch<float>(x, p, sv, ctl, cur, do_x, do_p, 6 * n_sites, s);
+    if (prec == COLA_F64) xp_dispatch<double>(x, p, sv, ctl, cur, do_x, do_p, skip, 12 * n_sites, s);
+    else xp_dispatch<float>(x, p, sv, ctl, cur, do_x, do_p, skip, 6 * n_sites, s);
     return cudaGetLastError();
 }
 
 cudaError_t launch_axpby64(void *out64, double a, const void *A64, double b, const void *B64, void *out32, size_t n_sites,
-                           double *partials, unsigned *counter, double *norm_out, cudaStream_t s)
+                           const ReduceWs *red, unsigned *counter, double *norm_out, cudaStream_t s)
 {
+    ReduceWs none = {nullptr, nullptr, nullptr};
     axpby64_kernel<<<blas_grid(6 * n_sites), BB, 0, s>>>((double2 *)out64, a, (const double2 *)A64, b, (const double2 *)B64, (float4 *)out32,
-                                                        n_sites, partials, counter, norm_out);
+                                                        n_sites, red ? *red : none, counter, norm_out);
     return cudaGetLastError();
 }
 

@@ -178,28 +178,54 @@ __device__ __forceinline__ double block_sum(double v, double *sm /* >= 32 double
     return sm[0];
 }
 
-__device__ __forceinline__ void grid_sum_finalize(double v, double *partials, unsigned *counter, double *result, bool accumulate = false)
+// Workspace of one grid-wide reduction: per-block partials, then per-group partials, then per-group tickets.
+// Blocks are grouped by REDUCE_GROUP consecutive block indices; the last block of a group to arrive adds the group's
+// partials in index order, the last group to finish adds the group sums in index order.  Two short dependent steps
+// instead of one block walking over every partial, and still bitwise deterministic (fixed order at each level).
+// Returns true in thread 0 of the block that completes the reduction, with the grid-wide sum in *total.
+// `counter` is the top-level ticket (self-resetting).  All threads of every block must call it.
+__device__ __forceinline__ bool grid_sum_last(double v, const ReduceWs &ws, unsigned *counter, double *total)
 {
     __shared__ double sm[33];
-    __shared__ int is_last;
+    __shared__ int stage;
+    const unsigned group = blockIdx.x / REDUCE_GROUP;
+    const unsigned ngroups = (gridDim.x + REDUCE_GROUP - 1) / REDUCE_GROUP;
+    const unsigned first = group * REDUCE_GROUP;
+    const unsigned gsize = min(REDUCE_GROUP, gridDim.x - first);
     double s = block_sum(v, sm);
     if (threadIdx.x == 0) {
-        partials[blockIdx.x] = s;
+        ws.partials[blockIdx.x] = s;
         __threadfence();
-        unsigned t = atomicAdd(counter, 1u);
-        is_last = (t == gridDim.x - 1);
+        stage = (atomicAdd(ws.gticket + group, 1u) == gsize - 1) ? 1 : 0;
     }
     __syncthreads();
-    if (is_last) {
+    if (!stage) return false;
+    __threadfence();
+    double a = 0.0;
+    for (unsigned k = threadIdx.x; k < gsize; k += blockDim.x) a += __ldcg(ws.partials + first + k);
+    a = block_sum(a, sm);
+    if (threadIdx.x == 0) {
+        ws.gticket[group] = 0u;
+        ws.gpart[group] = a;
         __threadfence();
-        double a = 0.0;
-        for (unsigned k = threadIdx.x; k < gridDim.x; k += blockDim.x) a += __ldcg(partials + k);
-        a = block_sum(a, sm);
-        if (threadIdx.x == 0) {
-            *result = accumulate ? *result + a : a;
-            *counter = 0u;
-        }
+        stage = (atomicAdd(counter, 1u) == ngroups - 1) ? 2 : 0;
     }
+    __syncthreads();
+    if (stage != 2) return false;
+    __threadfence();
+    a = 0.0;
+    for (unsigned k = threadIdx.x; k < ngroups; k += blockDim.x) a += __ldcg(ws.gpart + k);
+    a = block_sum(a, sm);
+    if (threadIdx.x != 0) return false;
+    *counter = 0u;
+    *total = a;
+    return true;
+}
+
+__device__ __forceinline__ void grid_sum_finalize(double v, const ReduceWs &ws, unsigned *counter, double *result, bool accumulate = false)
+{
+    double a;
+    if (grid_sum_last(v, ws, counter, &a)) *result = accumulate ? *result + a : a;
 }
 
 }  // namespace cola

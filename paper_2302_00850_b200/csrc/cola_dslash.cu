@@ -16,7 +16,21 @@ namespace cola {
 
 namespace {
 
-constexpr int DSLASH_BLOCK = 128;
+// Tuning knobs (compile-time).  Defaults = best of the round-1 sweep on B200: 64 threads
+// per block; fp32 kernels capped at 80 registers (12 blocks = 24 warps per SM), fp64 kernels at 168 registers
+// (6 blocks = 12 warps per SM).  The kernels are bound by bytes in flight: fewer registers than this spill, more
+// registers cost occupancy, and both lose bandwidth.
+#ifndef COLA_DSLASH_BLOCK
+#define COLA_DSLASH_BLOCK 64
+#endif
+#ifndef COLA_DSLASH_MINB_F32
+#define COLA_DSLASH_MINB_F32 12
+#endif
+#ifndef COLA_DSLASH_MINB_F64
+#define COLA_DSLASH_MINB_F64 6
+#endif
+constexpr int DSLASH_BLOCK = COLA_DSLASH_BLOCK;
+template <int FMT> struct MinBlocks { static constexpr int value = (FMT == LINK_F64_18) ? COLA_DSLASH_MINB_F64 : COLA_DSLASH_MINB_F32; };
 
 // h (2 spins x 3 colours, complex) = upper + s * A_mu * lower of the 24-real spinor p
 template <int MU, typename T>
@@ -123,9 +137,10 @@ __device__ __forceinline__ void hop(const void *in, const char *gauge_mu, size_t
 
 // XPAY: 0 none, 1 v = y + coef v, 2 v = A y + coef v.   POST: 0 none, 1 v = Cpost v.
 template <int FMT, int XPAY, int POST>
-__global__ void __launch_bounds__(DSLASH_BLOCK) dslash_kernel(const __grid_constant__ DslashArgs a)
+__global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
 {
     typedef typename LinkT<FMT>::T T;
+    if (a.skip && *a.skip) return;
     const Geom &g = a.g;
     const size_t Vh = g.Vh;
     const int i = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
@@ -197,14 +212,14 @@ __global__ void __launch_bounds__(DSLASH_BLOCK) dslash_kernel(const __grid_const
             for (int k = 0; k < 24; k++) acc[k] = w[k];
         }
         store_reals<T, 24>(a.out, Vh, i, acc);
-        if (a.partials) {
+        if (a.red.partials) {
             T s2 = 0;
 #pragma unroll
             for (int k = 0; k < 24; k++) s2 += acc[k] * acc[k];
             nrm = (double)s2;
         }
     }
-    if (a.partials) grid_sum_finalize(nrm, a.partials, a.counter, a.norm_out, a.norm_accumulate != 0);
+    if (a.red.partials) grid_sum_finalize(nrm, a.red, a.counter, a.norm_out, a.norm_accumulate != 0);
 }
 
 template <typename T>
@@ -234,6 +249,8 @@ cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
 }
 
 }  // namespace
+
+size_t dslash_grid_blocks(size_t Vh) { return (Vh + DSLASH_BLOCK - 1) / DSLASH_BLOCK; }
 
 cudaError_t launch_dslash(int fmt, const DslashArgs &a, cudaStream_t s)
 {

@@ -29,7 +29,31 @@ struct Ctl {
     double qq;         // |K p|^2
     double rr;         // |r|^2
     double aux[4];
+    // decision state of the iteration (written by r_update's last block, read by the host with a lag)
+    double rmax2;      // max |r|^2 since the last reliable update
+    double target2;    // (tol |b|)^2
+    double delta2;     // delta^2 of the reliable-update test; 0 = pure-precision solve
+    int flag;          // 1: iteration `iters` converged or asked for a reliable update -> later kernels skip
+    int iters;         // CGLS passes completed
     unsigned counter[8];  // "last block" tickets, one per concurrently used reduction
+};
+
+constexpr unsigned REDUCE_GROUP = 256;
+__host__ __device__ inline size_t reduce_groups(size_t nblocks) { return (nblocks + REDUCE_GROUP - 1) / REDUCE_GROUP; }
+
+// Buffers of one deterministic grid-wide reduction (see grid_sum_last in cola_device.cuh)
+struct ReduceWs {
+    double *partials;     // [max blocks]
+    double *gpart;        // [max groups]
+    unsigned *gticket;    // [max groups], zero before first use, self-resetting
+};
+
+// What r_update's last block publishes for the host: written straight into mapped pinned host memory
+// (rr and flag first, then a system fence, then `iters` as the sequence number the host polls).
+struct HostStatus {
+    double rr;
+    int flag;
+    int iters;
 };
 
 // Arguments of the fused parity-dslash kernel family:
@@ -49,13 +73,15 @@ struct DslashArgs {
     double coef;
     double sgn;             // -1: D (forward hop projects with 1 - gamma_mu); +1: gamma_5 D gamma_5
     int parity;             // p
-    double *partials;       // per-block partial sums (nullptr: no norm)
+    ReduceWs red;           // reduction buffers (red.partials == nullptr: no norm)
     unsigned *counter;
     double *norm_out;
     int norm_accumulate;    // 1: *norm_out += sum (second half of a full-lattice operator)
+    const int *skip;        // if non-null and *skip != 0 the launch is a no-op (speculatively queued iteration)
 };
 
 // launchers (cola_dslash.cu)
+size_t dslash_grid_blocks(size_t Vh);   // blocks a dslash launch uses = partial sums it may write
 cudaError_t launch_dslash(int fmt, const DslashArgs &a, cudaStream_t s);
 // clover-only apply: out = C in on one parity (cola_dslash.cu)
 cudaError_t launch_clover_apply(cola_prec prec, const Geom &g, const void *clov, const void *in, void *out, cudaStream_t s);
@@ -72,14 +98,15 @@ cudaError_t launch_clover_unpack(const Geom &g, const void *clov64, int parity_m
 
 // fused BLAS-1 (cola_blas.cu).  n = number of sites of the vectors (Vh or V).
 int blas_max_blocks();
-cudaError_t launch_norm2(cola_prec prec, const void *v, size_t n_sites, double *partials, unsigned *counter, double *out, cudaStream_t s);
+cudaError_t launch_norm2(cola_prec prec, const void *v, size_t n_sites, const ReduceWs &red, unsigned *counter, double *out, cudaStream_t s);
 // cur = k & 1.  r -= alpha q with alpha = ctl->gam[cur] / ctl->qq;  ctl->rr = |r|^2
-cudaError_t launch_r_update(cola_prec prec, void *r, const void *q, Ctl *ctl, int cur, size_t n_sites, double *partials, cudaStream_t s);
+// and the stop / reliable-update decision: ctl->iters = iter; ctl->flag = 1 if |r|^2 <= target2 or < delta2*rmax2
+cudaError_t launch_r_update(cola_prec prec, void *r, const void *q, Ctl *ctl, int cur, int iter, const int *skip, HostStatus *mirror, size_t n_sites, const ReduceWs &red, cudaStream_t s);
 // x += alpha p (if do_x);  p = s + beta p with beta = gam[cur^1]/gam[cur] (if do_p)
-cudaError_t launch_xp_update(cola_prec prec, void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, size_t n_sites, cudaStream_t s);
+cudaError_t launch_xp_update(cola_prec prec, void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, const int *skip, size_t n_sites, cudaStream_t s);
 // out64 = a*A64 + b*B64 (+ optional fp32 copy of the result, + optional |out|^2)
 cudaError_t launch_axpby64(void *out64, double a, const void *A64, double b, const void *B64, void *out32, size_t n_sites,
-                           double *partials, unsigned *counter, double *norm_out, cudaStream_t s);
+                           const ReduceWs *red, unsigned *counter, double *norm_out, cudaStream_t s);
 // x64 += x32; x32 = 0
 cudaError_t launch_accumulate(void *x64, void *x32, size_t n_sites, cudaStream_t s);
 
