@@ -112,6 +112,9 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     c->p = *p;
     c->g.X = p->dims[0]; c->g.Y = p->dims[1]; c->g.Z = p->dims[2]; c->g.T = p->dims[3];
     c->g.Xh = p->dims[0] / 2;
+    c->g.dXh = make_fastdiv((unsigned)c->g.Xh);
+    c->g.dY = make_fastdiv((unsigned)c->g.Y);
+    c->g.dZ = make_fastdiv((unsigned)c->g.Z);
     c->V = (size_t)vol;
     c->Vh = c->V / 2;
     c->g.Vh = (int)c->Vh;

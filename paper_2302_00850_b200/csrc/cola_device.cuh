@@ -39,6 +39,11 @@ __device__ __forceinline__ double2 ld_stream(const double2 *p)
 __device__ __forceinline__ float4 ld_cached(const float4 *p) { return __ldg(p); }
 __device__ __forceinline__ double2 ld_cached(const double2 *p) { return __ldg(p); }
 
+// Explicit fused multiply-add chains: without fast-math the compiler may not reassociate `re += a*b - c*d`
+// into two dependent FMAs (it emits FMUL + FFMA + FADD), and the fp32 kernels are close to issue-bound.
+__device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
+
 __device__ __forceinline__ void unpack(const float4 &v, float *r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
 __device__ __forceinline__ void unpack(const double2 &v, double *r) { r[0] = v.x; r[1] = v.y; }
 __device__ __forceinline__ float4 pack(const float *r) { return make_float4(r[0], r[1], r[2], r[3]); }
@@ -77,10 +82,11 @@ __device__ __forceinline__ void reconstruct_row3(T (&u)[18])
     for (int c = 0; c < 3; c++) {
         const int a = (c + 1) % 3, b = (c + 2) % 3;
         // U_2c = conj(U_0a U_1b - U_0b U_1a)
-        T re = u[2 * a] * u[6 + 2 * b] - u[2 * a + 1] * u[6 + 2 * b + 1] - (u[2 * b] * u[6 + 2 * a] - u[2 * b + 1] * u[6 + 2 * a + 1]);
-        T im = u[2 * a] * u[6 + 2 * b + 1] + u[2 * a + 1] * u[6 + 2 * b] - (u[2 * b] * u[6 + 2 * a + 1] + u[2 * b + 1] * u[6 + 2 * a]);
-        u[12 + 2 * c] = re;
-        u[12 + 2 * c + 1] = -im;
+        const T ar = u[2 * a], ai = u[2 * a + 1], br = u[2 * b], bi = u[2 * b + 1];                  // row 1
+        const T cr = u[6 + 2 * b], ci = u[6 + 2 * b + 1], dr = u[6 + 2 * a], di = u[6 + 2 * a + 1];  // row 2
+        // re = ar cr - ai ci - br dr + bi di;  -im = -(ar ci + ai cr - br di - bi dr)
+        u[12 + 2 * c] = fma_(bi, di, fma_(-br, dr, fma_(-ai, ci, ar * cr)));
+        u[12 + 2 * c + 1] = fma_(bi, dr, fma_(br, di, fma_(-ai, cr, -(ar * ci))));
     }
 }
 
@@ -130,11 +136,11 @@ __device__ __forceinline__ void clover_block_mul(const T *c, const T *v, T *w)
             const int k = 6 + 2 * (i * (i - 1) / 2 + j);
             const T ar = c[k], ai = c[k + 1];
             // w_i += a v_j
-            w[2 * i] += ar * v[2 * j] - ai * v[2 * j + 1];
-            w[2 * i + 1] += ar * v[2 * j + 1] + ai * v[2 * j];
+            w[2 * i] = fma_(-ai, v[2 * j + 1], fma_(ar, v[2 * j], w[2 * i]));
+            w[2 * i + 1] = fma_(ai, v[2 * j], fma_(ar, v[2 * j + 1], w[2 * i + 1]));
             // w_j += conj(a) v_i
-            w[2 * j] += ar * v[2 * i] + ai * v[2 * i + 1];
-            w[2 * j + 1] += ar * v[2 * i + 1] - ai * v[2 * i];
+            w[2 * j] = fma_(ai, v[2 * i + 1], fma_(ar, v[2 * i], w[2 * j]));
+            w[2 * j + 1] = fma_(-ai, v[2 * i], fma_(ar, v[2 * i + 1], w[2 * j + 1]));
         }
     }
 }

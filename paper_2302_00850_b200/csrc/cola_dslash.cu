@@ -114,8 +114,13 @@ __device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&
                 const T ur = DAG ? u[2 * (3 * b + a)] : u[2 * (3 * a + b)];
                 const T ui = DAG ? -u[2 * (3 * b + a) + 1] : u[2 * (3 * a + b) + 1];
                 const T hr = h[6 * sp + 2 * b], hi = h[6 * sp + 2 * b + 1];
-                re += ur * hr - ui * hi;
-                im += ur * hi + ui * hr;
+                if (b == 0) {
+                    re = fma_(-ui, hi, ur * hr);
+                    im = fma_(ui, hr, ur * hi);
+                } else {
+                    re = fma_(-ui, hi, fma_(ur, hr, re));
+                    im = fma_(ui, hr, fma_(ur, hi, im));
+                }
             }
             g[6 * sp + 2 * a] = re;
             g[6 * sp + 2 * a + 1] = im;
@@ -147,12 +152,8 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
     double nrm = 0.0;
     if (i < g.Vh) {
         // coordinates of the output site
-        const int xh = i % g.Xh;
-        int r = i / g.Xh;
-        const int y = r % g.Y;
-        r /= g.Y;
-        const int z = r % g.Z;
-        const int t = r / g.Z;
+        const unsigned r1 = g.dXh.div((unsigned)i), r2 = g.dY.div(r1), r3 = g.dZ.div(r2);
+        const int xh = i - (int)r1 * g.Xh, y = (int)r1 - (int)r2 * g.Y, z = (int)r2 - (int)r3 * g.Z, t = (int)r3;
         const int odd = (y + z + t + a.parity) & 1;     // x = 2*xh + odd
         const int sY = g.Xh, sZ = g.Xh * g.Y, sT = g.Xh * g.Y * g.Z;
 

@@ -11,11 +11,32 @@ namespace cola {
 
 // Lattice geometry as the kernels see it.  Checkerboard ("cb") index of a site of either parity:
 //   cb = (x >> 1) + Xh*(y + Y*(z + Z*t)),  x = 2*(cb % Xh) + ((y + z + t + parity) & 1)
+// Division of a site index n < 2^31 by a run-time extent d without the hardware's ~30-instruction
+// integer-division sequence: floor(n/d) = umulhi(n, m) >> sh with m = ceil(2^(32+sh)/d), sh = ceil(log2 d) - 1
+// (exact for n < 2^31 because m*d - 2^(32+sh) < d <= 2^(sh+1)); d = 1 is the identity.
+struct FastDiv {
+    unsigned d, m, sh;
+#ifdef __CUDACC__
+    __device__ __forceinline__ unsigned div(unsigned n) const { return d == 1u ? n : (__umulhi(n, m) >> sh); }
+#endif
+};
+inline FastDiv make_fastdiv(unsigned d)
+{
+    FastDiv f = {d, 0u, 0u};
+    if (d <= 1u) return f;
+    unsigned L = 0;
+    while ((1ull << L) < d) L++;
+    f.sh = L - 1;
+    f.m = (unsigned)((((unsigned long long)1 << (31 + L)) + d - 1) / d);
+    return f;
+}
+
 struct Geom {
     int X, Y, Z, T;   // extents
     int Xh;           // X/2
     int Vh;           // half volume
     int bc[4];        // +1 / -1
+    FastDiv dXh, dY, dZ;   // index decomposition of the dslash kernels
 };
 
 // Bytes of one link per site in each storage format.
