@@ -44,7 +44,7 @@ BYTES = {
 FLOPS = {"dslash": 1320, "dslash_clover_inv": 1824, "dslash_clover_xpay": 1872}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of dslash_kernel<F32x12, XPAY=2> from the committed
 # ncu --set full capture (a number read from a profile, never a timing taken under the profiler)
-NCU_TRAFFIC = {(32, 32, 32, 64): {"bytes_per_launch": 980312832, "source": "profiles/r1_dslash_f32x12_full.txt (909.34 MB read + 70.98 MB write)"}}
+NCU_TRAFFIC = {(32, 32, 32, 64): {"bytes_per_launch": 980280000, "source": "profiles/r1b_operators_full.txt (909.4 MB read + 70.88 MB write)"}}
 NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star's denominator, reported beside the measured one
 
 
@@ -227,6 +227,10 @@ def main():
     ap.add_argument("--impl", default="cola", choices=["cola", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-operator-table", action="store_true")
+    ap.add_argument("--operators-only", action="store_true",
+                    help="profiling aid: skip the solves, run only the operator table (few launches: --op-warm/--op-timed) and print it")
+    ap.add_argument("--op-warm", type=int, default=20)
+    ap.add_argument("--op-timed", type=int, default=200)
     args = ap.parse_args()
 
     cfg = inputs.CONFIGS[args.config]
@@ -273,6 +277,11 @@ def main():
             torch.distributed.barrier()
         torch.cuda.synchronize()
 
+    if args.operators_only:   # not a bench line: a short launch sequence for ncu captures of each operator kernel
+        print(json.dumps({"operators_only": True, "lattice": list(dims),
+                          "operators": operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed)}))
+        return
+
     # ---- device-resident steps
     for _ in range(args.warmup):
         x, info = ctx.cg_solve(b, tol=1e-10, even_odd=True, mixed=True)
@@ -316,7 +325,7 @@ def main():
 
     # ---- roofline of the dominant kernel + operator table (rank 0, kernels timed alone)
     peak, peak_src = measured_peaks()
-    table = {} if args.no_operator_table else operator_table(ctx, "f32x12")
+    table = {} if args.no_operator_table else operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed)
     roof = None
     if table:
         k = table["fermion_matrix_f32x12"]   # two launches of the fused dslash + clover + xpay kernel
