@@ -149,6 +149,31 @@ cola_status cola_dslash_apply_host(cola_ctx *c, cola_prec prec, cola_parity out_
 cola_status cola_fermion_matrix_apply_host(cola_ctx *c, cola_prec prec, int dagger, const void *in_canon_host, void *out_canon_host);
 cola_status cola_cg_solve_host(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_host, void *x_canon_host, cola_solve_info *info);
 
+/* ---- Multi-right-hand-side operators and batched solver (BJ:c3 has 12 sources per gauge
+ * field, one per spin-colour component).  The operators act on nrhs (1..16) vectors in ONE pass over the links and
+ * the clover field: a thread block covers the sites of a single-rhs block for several right-hand sides, so gauge and
+ * clover traffic is paid once per launch instead of once per vector (trade work for global-memory traffic).
+ * Per vector the arithmetic, its order and hence the result are those of the single-rhs entry points.
+ * "nrhs vectors" = nrhs internal buffers of the stated size stored back to back.
+ *
+ * Workspace: a second caller-owned DEVICE buffer holding, per right-hand side, the Schur temporaries and the vectors
+ * of the batched solver (5.5 fp64 half-lattice vectors).  Borrowed until cola_destroy / the next call. */
+size_t cola_mrhs_workspace_bytes(const cola_ctx *c, int nrhs);
+cola_status cola_set_mrhs_workspace(cola_ctx *c, void *dev_ptr, size_t bytes, int nrhs);
+/* out_p[n] = D_{p,1-p} in[n]: nrhs half-lattice internal DEVICE vectors each, no overlap. */
+cola_status cola_dslash_apply_mrhs(cola_ctx *c, cola_prec prec, cola_parity out_parity, int nrhs, const void *in_dev, void *out_dev);
+/* out[n] = M in[n] (M^+ if dagger): nrhs full internal DEVICE vectors each. */
+cola_status cola_fermion_matrix_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int nrhs, const void *in_full_dev, void *out_full_dev);
+/* out_e[n] = S in_e[n] (S^+ if dagger): nrhs half-lattice (even) internal DEVICE vectors each. */
+cola_status cola_schur_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int nrhs, const void *in_even_dev, void *out_even_dev);
+/* Batched solve of M x_n = b_n, n < nrhs, by mixed-precision even-odd CGNR (sp->even_odd and sp->mixed must be 1):
+ * the systems advance in lock step, each with its own alpha, beta, stopping test and reliable-update schedule
+ * (SURVEY O7/O8 per system); a system that has converged drops out of the batch.  b_canon_dev / x_canon_dev: nrhs
+ * canonical complex128 DEVICE arrays back to back; infos: HOST array of nrhs entries (seconds = time of the whole
+ * batch).  COLA_ENOCONV if any system hit max_iter (its info has the last residual).  COLA_ENOTREADY without a
+ * multi-rhs workspace for nrhs systems. */
+cola_status cola_cg_solve_mrhs(cola_ctx *c, const cola_solve_params *sp, int nrhs, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *infos);
+
 /* Benchmark aid: number of kernels this context has launched since creation. */
 unsigned long long cola_launch_count(const cola_ctx *c);
 

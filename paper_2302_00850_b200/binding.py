@@ -26,6 +26,8 @@ EXPORTS = [
     "cola_spinor_convert", "cola_dslash_apply", "cola_fermion_matrix_apply", "cola_schur_apply",
     "cola_cg_solve", "cola_dslash_apply_host", "cola_fermion_matrix_apply_host", "cola_cg_solve_host",
     "cola_launch_count",
+    "cola_mrhs_workspace_bytes", "cola_set_mrhs_workspace", "cola_dslash_apply_mrhs", "cola_fermion_matrix_apply_mrhs",
+    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs",
 ]
 
 
@@ -85,9 +87,16 @@ def _load():
     lib.cola_cg_solve_host.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo)]
     lib.cola_launch_count.argtypes = [vp]
     lib.cola_launch_count.restype = ctypes.c_ulonglong
+    lib.cola_mrhs_workspace_bytes.argtypes = [vp, ci]
+    lib.cola_mrhs_workspace_bytes.restype = ctypes.c_size_t
+    lib.cola_set_mrhs_workspace.argtypes = [vp, vp, ctypes.c_size_t, ci]
+    lib.cola_dslash_apply_mrhs.argtypes = [vp, ci, ci, ci, vp, vp]
+    lib.cola_fermion_matrix_apply_mrhs.argtypes = [vp, ci, ci, ci, vp, vp]
+    lib.cola_schur_apply_mrhs.argtypes = [vp, ci, ci, ci, vp, vp]
+    lib.cola_cg_solve_mrhs.argtypes = [vp, ctypes.POINTER(ColaSolveParams), ci, vp, vp, ctypes.POINTER(ColaSolveInfo)]
     for name in EXPORTS:
         fn = getattr(lib, name)
-        if name not in ("cola_last_error", "cola_spinor_bytes", "cola_workspace_bytes", "cola_launch_count"):
+        if name not in ("cola_last_error", "cola_spinor_bytes", "cola_workspace_bytes", "cola_launch_count", "cola_mrhs_workspace_bytes"):
             fn.restype = ci
     return lib
 
@@ -115,6 +124,8 @@ class Cola:
         self.device = torch.device("cuda", device)
         self._h = ctypes.c_void_p()
         self._ws = None
+        self._mws = None
+        self._mws_nrhs = 0
         p = ColaParams()
         p.dims[:] = self.dims
         p.kappa, p.csw = float(kappa), float(csw)
@@ -142,6 +153,7 @@ class Cola:
             _lib.cola_destroy(self._h)
             self._h = ctypes.c_void_p()
             self._ws = None
+            self._mws = None
 
     def __del__(self):
         try:
@@ -300,3 +312,71 @@ class Cola:
             out = torch.empty_like(inp, pin_memory=True)
         self._ck(_lib.cola_fermion_matrix_apply_host(self._h, pr, int(bool(dagger)), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
+
+    # ---- multi-right-hand-side operators and batched solver
+    def mrhs_workspace_bytes(self, nrhs: int) -> int:
+        return int(_lib.cola_mrhs_workspace_bytes(self._h, int(nrhs)))
+
+    def set_mrhs_workspace(self, nrhs: int, tensor: torch.Tensor | None = None):
+        """Lend the per-right-hand-side workspace (allocated here with torch if not given)."""
+        if tensor is None:
+            tensor = torch.empty(self.mrhs_workspace_bytes(nrhs), dtype=torch.uint8, device=self.device)
+        self._ck(_lib.cola_set_mrhs_workspace(self._h, ctypes.c_void_p(tensor.data_ptr()), tensor.numel() * tensor.element_size(), int(nrhs)))
+        self._mws, self._mws_nrhs = tensor, int(nrhs)
+        return tensor
+
+    def _need_mrhs(self, nrhs):
+        if self._mws is None or self._mws_nrhs < nrhs:
+            self.set_mrhs_workspace(nrhs)
+
+    def empty_internal_mrhs(self, nrhs, prec, full=True) -> torch.Tensor:
+        """nrhs internal buffers back to back: shape (nrhs,) + the shape of empty_internal."""
+        one = self.empty_internal(prec, full=full)
+        return torch.empty((int(nrhs),) + tuple(one.shape), dtype=one.dtype, device=self.device)
+
+    def dslash_apply_mrhs(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        pr, nrhs = _PREC[inp.dtype], inp.shape[0]
+        assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.Vh * 24
+        self._need_mrhs(nrhs)
+        if out is None:
+            out = torch.empty_like(inp)
+        self._ck(_lib.cola_dslash_apply_mrhs(self._h, pr, int(out_parity), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def fermion_matrix_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
+        pr, nrhs = _PREC[inp.dtype], inp.shape[0]
+        assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.V * 24
+        self._need_mrhs(nrhs)
+        if out is None:
+            out = torch.empty_like(inp)
+        self._ck(_lib.cola_fermion_matrix_apply_mrhs(self._h, pr, int(bool(dagger)), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def schur_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
+        pr, nrhs = _PREC[inp.dtype], inp.shape[0]
+        assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.Vh * 24
+        self._need_mrhs(nrhs)
+        if out is None:
+            out = torch.empty_like(inp)
+        self._ck(_lib.cola_schur_apply_mrhs(self._h, pr, int(bool(dagger)), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def cg_solve_mrhs(self, b: torch.Tensor, tol=1e-10, max_iter=20000, delta=0.1, x: torch.Tensor | None = None):
+        """b: nrhs canonical complex128 sources, shape (nrhs, t, z, y, x, 4, 3), on the device.
+        Returns (x, [info dict per system])."""
+        assert b.is_cuda and b.dtype == torch.complex128 and b.dim() == 7 and b[0].numel() == self.V * 12
+        b = b.contiguous()
+        nrhs = b.shape[0]
+        self._need_mrhs(nrhs)
+        if x is None:
+            x = torch.empty_like(b)
+        sp = self._solve_params(tol, max_iter, True, True, delta)
+        infos = (ColaSolveInfo * nrhs)()
+        st = _lib.cola_cg_solve_mrhs(self._h, ctypes.byref(sp), nrhs, ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), infos)
+        self._ck(st, ok=(COLA_OK, COLA_ENOCONV))
+        out = []
+        for n in range(nrhs):
+            d = self._info_dict(infos[n], COLA_OK)
+            d["converged"] = bool(d["iterated_residual"] <= tol) or st == COLA_OK
+            out.append(d)
+        return x, out

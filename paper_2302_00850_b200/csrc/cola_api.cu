@@ -32,6 +32,16 @@ struct cola_ctx {
     double *h_pinned;               // pinned host scalars
     HostStatus *h_status;           // mapped pinned host memory the device publishes the iteration status to
     HostStatus *d_status;           // device alias of h_status
+    // multi-right-hand-side workspace (borrowed, cola_set_mrhs_workspace) and control state
+    int m_nrhs;                     // capacity in right-hand sides (0: none)
+    char *m_tmp32;                  // [m_nrhs] odd half temporaries of the fp32 Schur operator
+    char *m_r64;                    // [m_nrhs] fp64 half vectors: Schur temporary of the operator API; r of the batched solver
+    char *m_rhs, *m_qs;             // [m_nrhs] fp64 half vectors: prepared sources, K x of the reliable updates
+    char *m_x32, *m_r32, *m_p32, *m_q32;   // [m_nrhs] fp32 half vectors of the inner iteration
+    double *m_partials;             // [m_nrhs][m_nsb]
+    int m_nsb;
+    CtlM *ctlm;                     // device, inside the control block
+    HostStatusM *h_statusm, *d_statusm;   // mapped pinned host memory and its device alias
     cudaEvent_t ev0, ev1;
     int ready;
     double max_unitarity_dev;
@@ -124,12 +134,15 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     char *blk = nullptr;
     cudaError_t e = cudaMalloc(&blk, 4096);
     if (e == cudaSuccess) e = cudaMemset(blk, 0, 4096);
-    if (e == cudaSuccess) e = cudaHostAlloc(&c->h_pinned, 1024, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostAlloc(&c->h_pinned, 2048, cudaHostAllocMapped);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
     if (e == cudaSuccess) {
         c->h_status = reinterpret_cast<HostStatus *>(reinterpret_cast<char *>(c->h_pinned) + 256);
         e = cudaHostGetDevicePointer(reinterpret_cast<void **>(&c->d_status), c->h_status, 0);
+        c->h_statusm = reinterpret_cast<HostStatusM *>(reinterpret_cast<char *>(c->h_pinned) + 512);
+        c->d_statusm = reinterpret_cast<HostStatusM *>(reinterpret_cast<char *>(c->d_status) + 256);
+        static_assert(2 * sizeof(HostStatusM) <= 1536 && sizeof(Ctl) <= 512 && sizeof(CtlM) <= 1536, "control block layout");
     }
     if (e != cudaSuccess) {
         fail(nullptr, COLA_ECUDA, "cola_create: %s", cudaGetErrorString(e));
@@ -138,6 +151,7 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
         return COLA_ECUDA;
     }
     c->ctl = reinterpret_cast<Ctl *>(blk);
+    c->ctlm = reinterpret_cast<CtlM *>(blk + 512);
     c->max_dev_bits = reinterpret_cast<unsigned long long *>(blk + 2048);
     *out = c;
     return COLA_OK;
@@ -590,6 +604,327 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
     return COLA_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// multi-right-hand-side operators and batched solver
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+struct CarveM {
+    size_t tmp32, r64, rhs, qs, x32, r32, p32, q32, partials, total;
+    int nsb;
+};
+
+CarveM carve_m(const cola_ctx *c, int nrhs)
+{
+    CarveM k;
+    size_t off = 0;
+    const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32), n = (size_t)nrhs;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    k.tmp32 = take(n * h32);
+    k.r64 = take(n * h64);
+    k.rhs = take(n * h64);
+    k.qs = take(n * h64);
+    k.x32 = take(n * h32);
+    k.r32 = take(n * h32);
+    k.p32 = take(n * h32);
+    k.q32 = take(n * h32);
+    size_t nsb = (size_t)mrhs_site_blocks(c->g);
+    const size_t nb32 = (size_t)blas_mrhs_blocks(c->Vh, COLA_F32), nb64 = (size_t)blas_mrhs_blocks(c->Vh, COLA_F64);
+    if (nsb < nb32) nsb = nb32;
+    if (nsb < nb64) nsb = nb64;
+    k.nsb = (int)nsb;
+    k.partials = take(n * nsb * sizeof(double));
+    k.total = off;
+    return k;
+}
+
+MrhsList list_of(const int *v, int n)
+{
+    MrhsList l;
+    for (int k = 0; k < MRHS_MAX; k++) l.v[k] = k < n ? v[k] : 0;
+    return l;
+}
+
+cola_status need_mrhs(cola_ctx *c, const char *who, int nrhs)
+{
+    ST(need_ready(c, who));
+    if (nrhs < 1 || nrhs > MRHS_MAX) return fail(c, COLA_EINVAL, "%s: nrhs must be 1..16", who);
+    if (c->m_nrhs < nrhs) return fail(c, COLA_ENOTREADY, "%s: no multi-rhs workspace for that many right-hand sides (call cola_set_mrhs_workspace)", who);
+    return COLA_OK;
+}
+
+// batched  out_p[n] = [post] ( [A] y[n] + coef * D_{p,1-p} in[n] )  for the vectors list.v[0..nrhs);  optional |out[n]|^2 -> norm_out[n]
+cola_status dslash_m(cola_ctx *c, cola_prec prec, int parity, int dagger, const MrhsList &list, int nrhs, const void *in, size_t in_stride, void *out,
+                     size_t out_stride, const void *y, size_t y_stride, int clov_on_y, double coef, int post_inv, double *norm_out, int norm_accumulate,
+                     const int *skip)
+{
+    MrhsArgs m;
+    memset(&m, 0, sizeof(m));
+    DslashArgs &a = m.d;
+    a.g = c->g;
+    a.in = in;
+    a.out = out;
+    a.gauge_p = gauge_of(c, prec, parity);
+    a.gauge_q = gauge_of(c, prec, 1 - parity);
+    a.y = y;
+    a.clov_y = (y && clov_on_y) ? clovA_of(c, prec, parity) : nullptr;
+    a.clov_post = post_inv ? clovI_of(c, prec) : nullptr;
+    a.coef = coef;
+    a.sgn = dagger ? +1.0 : -1.0;
+    a.parity = parity;
+    a.skip = skip;
+    m.nrhs = nrhs;
+    m.in_stride = in_stride;
+    m.out_stride = out_stride;
+    m.y_stride = y_stride;
+    for (int k = 0; k < MRHS_MAX; k++) m.list[k] = list.v[k];
+    m.partials = norm_out ? c->m_partials : nullptr;
+    if (post_inv && parity != 1) return fail(c, COLA_EINVAL, "internal: A^-1 is stored on the odd parity only");
+    CK(launch_dslash_mrhs(fmt_of(c, prec), m, c->stream));
+    c->launches++;
+    if (norm_out) {
+        CK(launch_mrhs_reduce(c->m_partials, m.nsb, nrhs, list.v, norm_out, norm_accumulate, skip, c->stream));
+        c->launches++;
+    }
+    return COLA_OK;
+}
+
+// batched Schur: out_e[n] = S in_e[n]; tmp = nrhs odd half vectors of precision prec (stride = half_bytes)
+cola_status schur_m(cola_ctx *c, cola_prec prec, int dagger, const MrhsList &list, int nrhs, const void *in, size_t in_stride, void *tmp, void *out,
+                    size_t out_stride, double *norm_out, const int *skip)
+{
+    const double k = c->p.kappa;
+    const size_t hb = half_bytes(c, prec);
+    ST(dslash_m(c, prec, 1, dagger, list, nrhs, in, in_stride, tmp, hb, nullptr, 0, 0, 0.0, 1, nullptr, 0, skip));
+    ST(dslash_m(c, prec, 0, dagger, list, nrhs, tmp, hb, out, out_stride, in, in_stride, 1, -k * k, 0, norm_out, 0, skip));
+    return COLA_OK;
+}
+
+}  // namespace
+
+namespace {
+
+cola_status wait_status_m(cola_ctx *c, int k, HostStatusM *out)
+{
+    volatile HostStatusM *m = c->h_statusm + (k & 1);
+    for (unsigned long spins = 0;; spins++) {
+        if (m->iters == k + 1) break;
+        if ((spins & 0xfff) == 0xfff) {
+            cudaError_t e = cudaStreamQuery(c->stream);
+            if (e == cudaSuccess) {
+                if (m->iters == k + 1) break;
+                return fail(c, COLA_ECUDA, "cola_cg_solve_mrhs: the stream drained without iteration status (internal error)");
+            }
+            if (e != cudaErrorNotReady) return fail(c, COLA_ECUDA, "cola_cg_solve_mrhs: %s", cudaGetErrorString(e));
+        }
+        __builtin_ia32_pause();
+    }
+    __sync_synchronize();
+    for (int n = 0; n < MRHS_MAX; n++) out->rr[n] = m->rr[n];
+    out->trig = m->trig;
+    out->flag = m->flag;
+    out->iters = m->iters;
+    return COLA_OK;
+}
+
+// iteration k of the batch, first half:  q = S p (|q|^2),  r -= alpha q (|r|^2), decision -> mapped host slot k & 1
+cola_status first_half_m(cola_ctx *c, int k, const MrhsList &A, int na)
+{
+    CtlM *cm = c->ctlm;
+    const size_t h32 = half_bytes(c, COLA_F32);
+    const int nb = blas_mrhs_blocks(c->Vh, COLA_F32);
+    ST(schur_m(c, COLA_F32, 0, A, na, c->m_p32, h32, c->m_tmp32, c->m_q32, h32, cm->qq, &cm->flag));
+    CK(launch_r_update_mrhs(COLA_F32, c->m_r32, c->m_q32, h32, cm, k & 1, A, na, &cm->flag, c->Vh, c->m_partials, c->stream));
+    CK(launch_mrhs_reduce(c->m_partials, nb, na, A.v, cm->rr, 0, &cm->flag, c->stream));
+    CK(launch_decide_mrhs(cm, A, na, k + 1, &cm->flag, c->d_statusm + (k & 1), c->stream));
+    c->launches += 3;
+    return COLA_OK;
+}
+
+// second half:  s = S^+ r (|s|^2 -> gam[next]),  x += alpha p (do_x),  p = s + beta p
+cola_status second_half_m(cola_ctx *c, int k, int do_x, const MrhsList &A, int na)
+{
+    CtlM *cm = c->ctlm;
+    const size_t h32 = half_bytes(c, COLA_F32);
+    ST(schur_m(c, COLA_F32, 1, A, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[(k & 1) ^ 1], &cm->flag));
+    CK(launch_xp_update_mrhs(COLA_F32, c->m_x32, c->m_p32, c->m_q32, h32, cm, k & 1, A, na, do_x, 1, &cm->flag, c->Vh, c->stream));
+    c->launches++;
+    return COLA_OK;
+}
+
+}  // namespace
+
+// Batched mixed-precision even-odd CGNR: nrhs independent systems M x_n = b_n advance in lock step so that every
+// pass over the links and the clover field serves all of them.  Each system keeps its own alpha, beta, residual
+// history and reliable-update schedule (SURVEY O7/O8 per system): the device raises one flag when ANY active system
+// converges in the inner precision or asks for a reliable update; the host then updates exactly those systems
+// (fp64 true residual, search direction kept), drops the ones that have converged and re-queues the rest.
+// Storage: the internal x_n lives in the caller's x_n buffer during the solve (same size) and is unpacked in place
+// at the end through the context's scratch.
+static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int nrhs, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *infos)
+{
+    ST(need_mrhs(c, "cola_cg_solve_mrhs", nrhs));
+    if (!sp || !b_canon_dev || !x_canon_dev || !infos) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: NULL argument");
+    if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: tol must be > 0 and max_iter >= 1");
+    if (!sp->even_odd || !sp->mixed) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd solver is batched (even_odd = 1, mixed = 1)");
+    CK(cudaSetDevice(c->p.device));
+    const double delta = sp->delta > 0 ? sp->delta : 0.1, kappa = c->p.kappa;
+    const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32), f64 = 2 * h64;
+    const double flops_K = 3696.0 * (double)c->Vh;
+    Ctl *ctl = c->ctl;
+    CtlM *cm = c->ctlm;
+    char *Bt = c->scratch, *Tt = Bt + f64;      // packed source of one system; full-lattice temporary
+    char *Xall = (char *)x_canon_dev;
+    const char *Ball = (const char *)b_canon_dev;
+    double bb[MRHS_MAX], bnorm[MRHS_MAX], target2[MRHS_MAX], rr[MRHS_MAX], flops[MRHS_MAX];
+    int conv[MRHS_MAX], iters[MRHS_MAX], updates[MRHS_MAX];
+    memset(infos, 0, sizeof(cola_solve_info) * nrhs);
+    CK(cudaEventRecord(c->ev0, c->stream));
+
+    // ---- source preparation, one system at a time (once per solve)
+    for (int n = 0; n < nrhs; n++) {
+        conv[n] = iters[n] = updates[n] = 0;
+        flops[n] = rr[n] = target2[n] = 0.0;
+        char *X = Xall + (size_t)n * f64;
+        CK(launch_spinor_pack(COLA_F64, c->g, Ball + (size_t)n * f64, Bt, c->stream));
+        c->launches++;
+        ST(norm2(c, COLA_F64, Bt, c->V, &ctl->aux[2]));
+        ST(read_scalar(c, &ctl->aux[2], &bb[n]));
+        bnorm[n] = sqrt(bb[n]);
+        CK(cudaMemsetAsync(X, 0, f64, c->stream));
+        CK(cudaMemsetAsync(c->m_x32 + (size_t)n * h32, 0, h32, c->stream));
+        if (!(bb[n] > 0.0)) { conv[n] = 1; continue; }
+        char *rhs = c->m_rhs + (size_t)n * h64, *r = c->m_r64 + (size_t)n * h64;
+        CK(launch_clover_apply(COLA_F64, c->g, c->clovI64, Bt + h64, c->tmp64, c->stream));
+        c->launches++;
+        ST(dslash(c, COLA_F64, 0, 0, c->tmp64, rhs, Bt, 0, kappa, 0, nullptr, 0));                       // bhat_e = b_e + kappa D_eo A_oo^-1 b_o
+        flops[n] += (504.0 + 1320.0 + 48.0) * (double)c->Vh;
+        CK(launch_axpby64(r, 1.0, rhs, 0.0, nullptr, c->m_r32 + (size_t)n * h32, c->Vh, &c->red, &ctl->counter[3], &cm->rr[n], c->stream));
+        c->launches++;
+    }
+    CK(cudaMemcpyAsync(c->h_pinned, cm->rr, sizeof(double) * MRHS_MAX, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    int A[MRHS_MAX], na = 0;
+    for (int n = 0; n < nrhs; n++) {
+        if (conv[n]) continue;
+        rr[n] = c->h_pinned[n];
+        target2[n] = (sp->tol * bnorm[n]) * (sp->tol * bnorm[n]);
+        if (rr[n] <= target2[n]) conv[n] = 1;
+        else A[na++] = n;
+    }
+
+    if (na > 0) {
+        CtlM st;
+        memset(&st, 0, sizeof(st));
+        for (int n = 0; n < nrhs; n++) { st.rmax2[n] = rr[n]; st.target2[n] = target2[n]; }
+        st.delta2 = delta * delta;
+        CK(cudaMemcpyAsync(cm, &st, sizeof(st), cudaMemcpyHostToDevice, c->stream));
+        MrhsList L = list_of(A, na);
+        ST(schur_m(c, COLA_F32, 1, L, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[0], nullptr));    // s0 = S^+ r0, gamma_0
+        CK(cudaMemcpyAsync(c->m_p32, c->m_q32, (size_t)nrhs * h32, cudaMemcpyDeviceToDevice, c->stream));
+        for (int j = 0; j < na; j++) flops[A[j]] += flops_K;
+        c->h_statusm[0].iters = c->h_statusm[1].iters = 0;
+        ST(first_half_m(c, 0, L, na));
+        for (int k = 0;; k++) {
+            const int more = (k + 1 < sp->max_iter);
+            ST(second_half_m(c, k, 1, L, na));                          // speculative: skipped if iteration k raises the flag
+            if (more) ST(first_half_m(c, k + 1, L, na));
+            HostStatusM hs;
+            ST(wait_status_m(c, k, &hs));
+            for (int j = 0; j < na; j++) { rr[A[j]] = hs.rr[A[j]]; iters[A[j]] = k + 1; flops[A[j]] += flops_K; }
+            if (!hs.flag) {
+                for (int j = 0; j < na; j++) flops[A[j]] += flops_K;
+                if (!more) break;
+                continue;
+            }
+            // some systems converged in fp32 or ask for a reliable update; no x has received alpha_k p_k yet
+            CK(launch_xp_update_mrhs(COLA_F32, c->m_x32, c->m_p32, c->m_q32, h32, cm, k & 1, L, na, 1, 0, nullptr, c->Vh, c->stream));
+            c->launches++;
+            int S[MRHS_MAX], ns = 0;
+            for (int j = 0; j < na; j++) if (hs.trig & (1u << A[j])) S[ns++] = A[j];
+            if (ns == 0) return fail(c, COLA_ECUDA, "cola_cg_solve_mrhs: flag raised without a triggering system (internal error)");
+            for (int j = 0; j < ns; j++) {
+                CK(launch_accumulate(Xall + (size_t)S[j] * f64, c->m_x32 + (size_t)S[j] * h32, c->Vh, c->stream));   // x64 += x32, x32 = 0
+                c->launches++;
+            }
+            const MrhsList LS = list_of(S, ns);
+            ST(schur_m(c, COLA_F64, 0, LS, ns, Xall, f64, c->m_r64, c->m_qs, h64, nullptr, nullptr));     // r64 is dead here: it is the Schur temporary
+            for (int j = 0; j < ns; j++) {
+                const size_t n = (size_t)S[j];
+                CK(launch_axpby64(c->m_r64 + n * h64, 1.0, c->m_rhs + n * h64, -1.0, c->m_qs + n * h64, c->m_r32 + n * h32, c->Vh, &c->red,
+                                  &ctl->counter[3], &cm->rr[n], c->stream));                                  // r64 = rhs - S x64, r32 = float(r64)
+                c->launches++;
+            }
+            CK(cudaMemcpyAsync(c->h_pinned, cm->rr, sizeof(double) * MRHS_MAX, cudaMemcpyDeviceToHost, c->stream));
+            CK(cudaStreamSynchronize(c->stream));
+            int na2 = 0;
+            for (int j = 0; j < na; j++) {
+                const int n = A[j];
+                if (hs.trig & (1u << n)) {
+                    rr[n] = c->h_pinned[n];
+                    updates[n]++;
+                    flops[n] += flops_K;
+                    if (rr[n] <= target2[n]) { conv[n] = 1; continue; }
+                    CK(cudaMemcpyAsync(&cm->rmax2[n], &rr[n], sizeof(double), cudaMemcpyHostToDevice, c->stream));   // rmax = |r64|
+                }
+                A[na2++] = n;
+            }
+            na = na2;
+            if (na == 0 || !more) break;
+            struct { int flag, iters; unsigned trig; } rearm = {0, k + 1, 0u};
+            static_assert(offsetof(CtlM, trig) - offsetof(CtlM, flag) == 8, "CtlM decision block layout");
+            CK(cudaMemcpyAsync(&cm->flag, &rearm, sizeof(rearm), cudaMemcpyHostToDevice, c->stream));
+            L = list_of(A, na);
+            ST(second_half_m(c, k, 0, L, na));                          // same search directions: p = s + beta p
+            for (int j = 0; j < na; j++) flops[A[j]] += flops_K;
+            ST(first_half_m(c, k + 1, L, na));
+        }
+        for (int j = 0; j < na; j++) {   // max_iter: fold the fp32 parts into the fp64 iterates
+            CK(launch_accumulate(Xall + (size_t)A[j] * f64, c->m_x32 + (size_t)A[j] * h32, c->Vh, c->stream));
+            c->launches++;
+        }
+    }
+
+    // ---- reconstruction of the odd sites, fp64 true residual and unpacking, one system at a time
+    int all_conv = 1;
+    for (int n = 0; n < nrhs; n++) {
+        char *X = Xall + (size_t)n * f64;
+        double tr = 0.0;
+        if (bb[n] > 0.0) {
+            CK(launch_spinor_pack(COLA_F64, c->g, Ball + (size_t)n * f64, Bt, c->stream));
+            c->launches++;
+            ST(dslash(c, COLA_F64, 1, 0, X, X + h64, Bt + h64, 0, kappa, 1, nullptr, 0));               // x_o = A_oo^-1 (b_o + kappa D_oe x_e)
+            flops[n] += (1320.0 + 48.0 + 504.0) * (double)c->Vh;
+            ST(fmatrix(c, COLA_F64, 0, X, Tt, nullptr));
+            flops[n] += 1872.0 * (double)c->V;
+            for (int h = 0; h < 2; h++) {
+                CK(launch_axpby64(nullptr, 1.0, Bt + h * h64, -1.0, Tt + h * h64, nullptr, c->Vh, &c->red, &ctl->counter[3], &ctl->aux[h], c->stream));
+                c->launches++;
+            }
+            double a0, a1;
+            ST(read_scalar(c, &ctl->aux[0], &a0));
+            ST(read_scalar(c, &ctl->aux[1], &a1));
+            tr = a0 + a1;
+        }
+        CK(launch_spinor_unpack(COLA_F64, c->g, X, Tt, c->stream));
+        c->launches++;
+        CK(cudaMemcpyAsync(X, Tt, f64, cudaMemcpyDeviceToDevice, c->stream));
+        infos[n].iters = iters[n];
+        infos[n].reliable_updates = updates[n];
+        infos[n].iterated_residual = bb[n] > 0 ? sqrt(rr[n]) / bnorm[n] : 0.0;
+        infos[n].true_residual = bb[n] > 0 ? sqrt(tr) / bnorm[n] : 0.0;
+        infos[n].op_flops = flops[n];
+        if (!conv[n]) all_conv = 0;
+    }
+    CK(cudaEventRecord(c->ev1, c->stream));
+    CK(cudaEventSynchronize(c->ev1));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+    for (int n = 0; n < nrhs; n++) infos[n].seconds = ms * 1e-3;
+    if (!all_conv) return fail(c, COLA_ENOCONV, "cola_cg_solve_mrhs: max_iter reached before |r| <= tol*|b| for every system");
+    return COLA_OK;
+}
+
 extern "C" {
 
 cola_status cola_gauge_upload(cola_ctx *c, const double *host_links) { return gauge_upload_impl(c, host_links, 1); }
@@ -726,6 +1061,73 @@ cola_status cola_cg_solve_host(cola_ctx *c, const cola_solve_params *sp, const v
     CK(cudaMemcpyAsync(x_canon_host, stage, fb, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return st;
+}
+
+// ---- multi-right-hand-side entry points
+size_t cola_mrhs_workspace_bytes(const cola_ctx *c, int nrhs)
+{
+    if (!c || nrhs < 1 || nrhs > MRHS_MAX) return 0;
+    return carve_m(c, nrhs).total;
+}
+
+cola_status cola_set_mrhs_workspace(cola_ctx *c, void *dev_ptr, size_t bytes, int nrhs)
+{
+    if (!c) return COLA_EINVAL;
+    c->m_nrhs = 0;
+    if (nrhs < 1 || nrhs > MRHS_MAX) return fail(c, COLA_EINVAL, "cola_set_mrhs_workspace: nrhs must be 1..16");
+    if (!dev_ptr || ((uintptr_t)dev_ptr & 255)) return fail(c, COLA_EINVAL, "cola_set_mrhs_workspace: pointer must be non-NULL and 256-byte aligned");
+    const CarveM k = carve_m(c, nrhs);
+    if (bytes < k.total) return fail(c, COLA_ENOMEM, "cola_set_mrhs_workspace: workspace smaller than cola_mrhs_workspace_bytes()");
+    char *w = (char *)dev_ptr;
+    c->m_tmp32 = w + k.tmp32; c->m_r64 = w + k.r64; c->m_rhs = w + k.rhs; c->m_qs = w + k.qs;
+    c->m_x32 = w + k.x32; c->m_r32 = w + k.r32; c->m_p32 = w + k.p32; c->m_q32 = w + k.q32;
+    c->m_partials = (double *)(w + k.partials);
+    c->m_nsb = k.nsb;
+    c->m_nrhs = nrhs;
+    return COLA_OK;
+}
+
+static MrhsList identity_list(int nrhs)
+{
+    int v[MRHS_MAX];
+    for (int k = 0; k < MRHS_MAX; k++) v[k] = k;
+    return list_of(v, nrhs);
+}
+
+cola_status cola_dslash_apply_mrhs(cola_ctx *c, cola_prec prec, cola_parity out_parity, int nrhs, const void *in_dev, void *out_dev)
+{
+    ST(need_mrhs(c, "cola_dslash_apply_mrhs", nrhs));
+    if (!in_dev || !out_dev || in_dev == out_dev) return fail(c, COLA_EINVAL, "cola_dslash_apply_mrhs: NULL or aliased buffers");
+    if (out_parity != COLA_EVEN && out_parity != COLA_ODD) return fail(c, COLA_EINVAL, "cola_dslash_apply_mrhs: bad parity");
+    const size_t hb = half_bytes(c, prec);
+    return dslash_m(c, prec, (int)out_parity, 0, identity_list(nrhs), nrhs, in_dev, hb, out_dev, hb, nullptr, 0, 0, 0.0, 0, nullptr, 0, nullptr);
+}
+
+cola_status cola_fermion_matrix_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int nrhs, const void *in_full_dev, void *out_full_dev)
+{
+    ST(need_mrhs(c, "cola_fermion_matrix_apply_mrhs", nrhs));
+    if (!in_full_dev || !out_full_dev || in_full_dev == out_full_dev) return fail(c, COLA_EINVAL, "cola_fermion_matrix_apply_mrhs: NULL or aliased buffers");
+    const size_t hb = half_bytes(c, prec), fb = 2 * hb;
+    const char *in_e = (const char *)in_full_dev, *in_o = in_e + hb;
+    char *out_e = (char *)out_full_dev, *out_o = out_e + hb;
+    const MrhsList L = identity_list(nrhs);
+    const int dg = dagger ? 1 : 0;
+    ST(dslash_m(c, prec, 0, dg, L, nrhs, in_o, fb, out_e, fb, in_e, fb, 1, -c->p.kappa, 0, nullptr, 0, nullptr));
+    ST(dslash_m(c, prec, 1, dg, L, nrhs, in_e, fb, out_o, fb, in_o, fb, 1, -c->p.kappa, 0, nullptr, 0, nullptr));
+    return COLA_OK;
+}
+
+cola_status cola_schur_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int nrhs, const void *in_even_dev, void *out_even_dev)
+{
+    ST(need_mrhs(c, "cola_schur_apply_mrhs", nrhs));
+    if (!in_even_dev || !out_even_dev || in_even_dev == out_even_dev) return fail(c, COLA_EINVAL, "cola_schur_apply_mrhs: NULL or aliased buffers");
+    const size_t hb = half_bytes(c, prec);
+    return schur_m(c, prec, dagger ? 1 : 0, identity_list(nrhs), nrhs, in_even_dev, hb, prec == COLA_F64 ? c->m_r64 : c->m_tmp32, out_even_dev, hb, nullptr, nullptr);
+}
+
+cola_status cola_cg_solve_mrhs(cola_ctx *c, const cola_solve_params *sp, int nrhs, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *infos)
+{
+    return solve_mrhs_impl(c, sp, nrhs, b_canon_dev, x_canon_dev, infos);
 }
 
 unsigned long long cola_launch_count(const cola_ctx *c) { return c ? c->launches : 0; }

@@ -120,9 +120,132 @@ __global__ void __launch_bounds__(BB) accumulate_kernel(double2 *x64, float4 *x3
     }
 }
 
+// ---- batched (multi-right-hand-side) variants: blockIdx.y = position in the list, same arithmetic per vector
+inline unsigned mrhs_grid(size_t n_chunks)
+{
+    size_t b = (n_chunks + BB - 1) / BB;
+    return (unsigned)(b < (size_t)(MAX_BLOCKS / 4) ? b : (size_t)(MAX_BLOCKS / 4));
+}
+
+template <typename T>
+__global__ void __launch_bounds__(BB) r_update_mrhs_kernel(char *r0, const char *q0, size_t stride, const CtlM *ctl, int cur, const __grid_constant__ MrhsList list,
+                                                           const int *skip, size_t n, double *partials)
+{
+    typedef typename VT<T>::V V;
+    if (skip && *skip) return;
+    __shared__ double sm[33];
+    const int vec = list.v[blockIdx.y];
+    V *r = reinterpret_cast<V *>(r0 + (size_t)vec * stride);
+    const V *q = reinterpret_cast<const V *>(q0 + (size_t)vec * stride);
+    const T ma = (T)(-(ctl->gam[cur][vec] / ctl->qq[vec]));
+    double acc = 0.0;
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) {
+        const V v = axpy(ma, q[k], r[k]);
+        r[k] = v;
+        acc += sq(v);
+    }
+    acc = block_sum(acc, sm);
+    if (threadIdx.x == 0) partials[(size_t)vec * gridDim.x + blockIdx.x] = acc;
+}
+
+// one block, one thread per list entry: rmax2, trigger, flag, host mirror
+__global__ void __launch_bounds__(32) decide_mrhs_kernel(CtlM *ctl, const __grid_constant__ MrhsList list, int nrhs, int iter, const int *skip, HostStatusM *mirror)
+{
+    if (skip && *skip) return;
+    const int k = threadIdx.x;
+    bool trig = false;
+    int vec = 0;
+    double rr = 0.0;
+    if (k < nrhs) {
+        vec = list.v[k];
+        rr = ctl->rr[vec];
+        const double rmax2 = fmax(ctl->rmax2[vec], rr);
+        ctl->rmax2[vec] = rmax2;
+        trig = rr <= ctl->target2[vec] || rr < ctl->delta2 * rmax2;
+    }
+    unsigned mask = 0;
+    for (int j = 0; j < 32; j++) {
+        const int tj = __shfl_sync(0xffffffffu, trig ? 1 : 0, j);
+        const int vj = __shfl_sync(0xffffffffu, vec, j);
+        if (tj) mask |= 1u << vj;
+    }
+    if (mirror && k < nrhs) (reinterpret_cast<volatile double *>(mirror->rr))[vec] = rr;
+    __syncwarp();
+    if (k == 0) {
+        ctl->iters = iter;
+        ctl->trig = mask;
+        if (mask) ctl->flag = 1;
+        if (mirror) {
+            volatile HostStatusM *m = mirror;
+            m->trig = mask;
+            m->flag = mask ? 1 : 0;
+            __threadfence_system();
+            m->iters = iter;
+        }
+    }
+}
+
+template <typename T, bool DO_X, bool DO_P>
+__global__ void __launch_bounds__(BB) xp_update_mrhs_kernel(char *x0, char *p0, const char *s0, size_t stride, const CtlM *ctl, int cur, const __grid_constant__ MrhsList list,
+                                                            const int *skip, size_t n)
+{
+    typedef typename VT<T>::V V;
+    if (skip && *skip) return;
+    const int vec = list.v[blockIdx.y];
+    V *x = reinterpret_cast<V *>(x0 + (size_t)vec * stride);
+    V *p = reinterpret_cast<V *>(p0 + (size_t)vec * stride);
+    const V *s = reinterpret_cast<const V *>(s0 + (size_t)vec * stride);
+    const T alpha = (T)(ctl->gam[cur][vec] / ctl->qq[vec]);
+    const T beta = (T)(ctl->gam[cur ^ 1][vec] / ctl->gam[cur][vec]);
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) {
+        const V pv = p[k];
+        if (DO_X) x[k] = axpy(alpha, pv, x[k]);
+        if (DO_P) p[k] = axpy(beta, pv, s[k]);
+    }
+}
+
 }  // namespace
 
 int blas_max_blocks() { return MAX_BLOCKS; }
+
+int blas_mrhs_blocks(size_t n_sites, cola_prec prec) { return (int)mrhs_grid((prec == COLA_F64 ? 12 : 6) * n_sites); }
+
+cudaError_t launch_r_update_mrhs(cola_prec prec, void *r, const void *q, size_t stride, const CtlM *ctl, int cur, const MrhsList &list, int nrhs,
+                                 const int *skip, size_t n_sites, double *partials, cudaStream_t s)
+{
+    const size_t n = (prec == COLA_F64 ? 12 : 6) * n_sites;
+    const dim3 grid(mrhs_grid(n), nrhs);
+    if (prec == COLA_F64) r_update_mrhs_kernel<double><<<grid, BB, 0, s>>>((char *)r, (const char *)q, stride, ctl, cur, list, skip, n, partials);
+    else r_update_mrhs_kernel<float><<<grid, BB, 0, s>>>((char *)r, (const char *)q, stride, ctl, cur, list, skip, n, partials);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_decide_mrhs(CtlM *ctl, const MrhsList &list, int nrhs, int iter, const int *skip, HostStatusM *mirror, cudaStream_t s)
+{
+    decide_mrhs_kernel<<<1, 32, 0, s>>>(ctl, list, nrhs, iter, skip, mirror);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_xp_update_mrhs(cola_prec prec, void *x, void *p, const void *sv, size_t stride, const CtlM *ctl, int cur, const MrhsList &list, int nrhs,
+                                  int do_x, int do_p, const int *skip, size_t n_sites, cudaStream_t s)
+{
+    const size_t n = (prec == COLA_F64 ? 12 : 6) * n_sites;
+    const dim3 grid(mrhs_grid(n), nrhs);
+    char *x0 = (char *)x, *p0 = (char *)p;
+    const char *s0 = (const char *)sv;
+#define COLA_XP(T, X, P) xp_update_mrhs_kernel<T, X, P><<<grid, BB, 0, s>>>(x0, p0, s0, stride, ctl, cur, list, skip, n)
+    if (prec == COLA_F64) {
+        if (do_x && do_p) COLA_XP(double, true, true);
+        else if (do_x) COLA_XP(double, true, false);
+        else if (do_p) COLA_XP(double, false, true);
+    } else {
+        if (do_x && do_p) COLA_XP(float, true, true);
+        else if (do_x) COLA_XP(float, true, false);
+        else if (do_p) COLA_XP(float, false, true);
+    }
+#undef COLA_XP
+    return cudaGetLastError();
+}
 
 cudaError_t launch_norm2(cola_prec prec, const void *v, size_t n_sites, const ReduceWs &red, unsigned *counter, double *out, cudaStream_t s)
 {

@@ -96,23 +96,26 @@ template <> struct LinkT<LINK_F32_18> { typedef float T; };
 template <> struct LinkT<LINK_F32_12> { typedef float T; };
 
 // base = start of the [chunk][Vh] block of one (parity, mu)
-template <int FMT>
+// STREAM: read-once data, no L1 allocation (single right-hand side); !STREAM: the same link is read by the
+// threads of several right-hand sides of one block, so it is kept in L1.
+template <int FMT, bool STREAM = true>
 __device__ __forceinline__ void load_link(const char *base, size_t Vh, size_t i, typename LinkT<FMT>::T (&u)[18])
 {
     if constexpr (FMT == LINK_F64_18) {
-        load_reals<double, 18, true>(base, Vh, i, u);
+        load_reals<double, 18, STREAM>(base, Vh, i, u);
     } else if constexpr (FMT == LINK_F32_12) {
         float r[12];
-        load_reals<float, 12, true>(base, Vh, i, r);
+        load_reals<float, 12, STREAM>(base, Vh, i, r);
 #pragma unroll
         for (int k = 0; k < 12; k++) u[k] = r[k];
         reconstruct_row3(u);
     } else {
         float r[16];
-        load_reals<float, 16, true>(base, Vh, i, r);
+        load_reals<float, 16, STREAM>(base, Vh, i, r);
 #pragma unroll
         for (int k = 0; k < 16; k++) u[k] = r[k];
-        float2 t = ld_stream(reinterpret_cast<const float2 *>(base + 64 * Vh) + i);
+        const float2 *tp = reinterpret_cast<const float2 *>(base + 64 * Vh) + i;
+        float2 t = STREAM ? ld_stream(tp) : __ldg(tp);
         u[16] = t.x;
         u[17] = t.y;
     }
@@ -146,7 +149,7 @@ __device__ __forceinline__ void clover_block_mul(const T *c, const T *v, T *w)
 }
 
 // w = C(site i) v on the full 24-real spinor; clov = [72/N chunks][Vh]
-template <typename T>
+template <typename T, bool STREAM = true>
 __device__ __forceinline__ void clover_apply(const void *clov, size_t Vh, size_t i, const T (&v)[24], T (&w)[24])
 {
     typedef typename VT<T>::V V;
@@ -154,7 +157,7 @@ __device__ __forceinline__ void clover_apply(const void *clov, size_t Vh, size_t
 #pragma unroll
     for (int b = 0; b < 2; b++) {
         T c[36];
-        load_reals<T, 36, true>(reinterpret_cast<const V *>(clov) + (size_t)b * (36 / N) * Vh, Vh, i, c);
+        load_reals<T, 36, STREAM>(reinterpret_cast<const V *>(clov) + (size_t)b * (36 / N) * Vh, Vh, i, c);
         clover_block_mul(c, &v[12 * b], &w[12 * b]);
     }
 }

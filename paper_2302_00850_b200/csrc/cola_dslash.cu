@@ -129,28 +129,28 @@ __device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&
 }
 
 // one hop: neighbour index nb (parity 1-p), link at site li of the given gauge block
-template <int FMT, int MU, bool BACK, typename T>
+template <int FMT, int MU, bool BACK, bool STREAM, typename T>
 __device__ __forceinline__ void hop(const void *in, const char *gauge_mu, size_t Vh, int nb, int li, T eta, T s, T (&acc)[24])
 {
     T psi[24], h[12], g[12], u[18];
     load_reals<T, 24, false>(in, Vh, nb, psi);
-    load_link<FMT>(gauge_mu, Vh, li, u);
+    load_link<FMT, STREAM>(gauge_mu, Vh, li, u);
     project<MU>(psi, s, h);
     su3_mul<BACK>(u, h, g);
     reconstruct_accumulate<MU>(g, eta, s, acc);
 }
 
-// XPAY: 0 none, 1 v = y + coef v, 2 v = A y + coef v.   POST: 0 none, 1 v = Cpost v.
-template <int FMT, int XPAY, int POST>
-__global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
+// One output site i of parity a.parity:  v = D in;  v = [A] y + coef v (XPAY);  v = Cpost v (POST);  out = v.
+// Returns |v|^2 if want_norm.  XPAY: 0 none, 1 v = y + coef v, 2 v = A y + coef v.   POST: 0 none, 1 v = Cpost v.
+// STREAM: links and clover are read once (no L1 allocation); !STREAM: they are shared by the right-hand sides of a block.
+template <int FMT, int XPAY, int POST, bool STREAM>
+__device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, const void *in, const void *yin, void *out, const bool want_norm)
 {
     typedef typename LinkT<FMT>::T T;
-    if (a.skip && *a.skip) return;
     const Geom &g = a.g;
     const size_t Vh = g.Vh;
-    const int i = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
     double nrm = 0.0;
-    if (i < g.Vh) {
+    {
         // coordinates of the output site
         const unsigned r1 = g.dXh.div((unsigned)i), r2 = g.dY.div(r1), r3 = g.dZ.div(r2);
         const int xh = i - (int)r1 * g.Xh, y = (int)r1 - (int)r2 * g.Y, z = (int)r2 - (int)r3 * g.Z, t = (int)r3;
@@ -183,22 +183,22 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
 #pragma unroll
         for (int k = 0; k < 24; k++) acc[k] = 0;
 
-        hop<FMT, 0, false>(a.in, gp + 0 * lb, Vh, xf, i, ex_f, sf, acc);
-        hop<FMT, 0, true>(a.in, gq + 0 * lb, Vh, xb, xb, ex_b, sb, acc);
-        hop<FMT, 1, false>(a.in, gp + 1 * lb, Vh, yf, i, ey_f, sf, acc);
-        hop<FMT, 1, true>(a.in, gq + 1 * lb, Vh, yb, yb, ey_b, sb, acc);
-        hop<FMT, 2, false>(a.in, gp + 2 * lb, Vh, zf, i, ez_f, sf, acc);
-        hop<FMT, 2, true>(a.in, gq + 2 * lb, Vh, zb, zb, ez_b, sb, acc);
-        hop<FMT, 3, false>(a.in, gp + 3 * lb, Vh, tf, i, et_f, sf, acc);
-        hop<FMT, 3, true>(a.in, gq + 3 * lb, Vh, tb, tb, et_b, sb, acc);
+        hop<FMT, 0, false, STREAM>(in, gp + 0 * lb, Vh, xf, i, ex_f, sf, acc);
+        hop<FMT, 0, true, STREAM>(in, gq + 0 * lb, Vh, xb, xb, ex_b, sb, acc);
+        hop<FMT, 1, false, STREAM>(in, gp + 1 * lb, Vh, yf, i, ey_f, sf, acc);
+        hop<FMT, 1, true, STREAM>(in, gq + 1 * lb, Vh, yb, yb, ey_b, sb, acc);
+        hop<FMT, 2, false, STREAM>(in, gp + 2 * lb, Vh, zf, i, ez_f, sf, acc);
+        hop<FMT, 2, true, STREAM>(in, gq + 2 * lb, Vh, zb, zb, ez_b, sb, acc);
+        hop<FMT, 3, false, STREAM>(in, gp + 3 * lb, Vh, tf, i, et_f, sf, acc);
+        hop<FMT, 3, true, STREAM>(in, gq + 3 * lb, Vh, tb, tb, et_b, sb, acc);
 
         if (XPAY != 0) {
             T yv[24];
-            load_reals<T, 24, true>(a.y, Vh, i, yv);
+            load_reals<T, 24, true>(yin, Vh, i, yv);
             const T cf = (T)a.coef;
             if (XPAY == 2) {
                 T cy[24];
-                clover_apply<T>(a.clov_y, Vh, i, yv, cy);
+                clover_apply<T, STREAM>(a.clov_y, Vh, i, yv, cy);
 #pragma unroll
                 for (int k = 0; k < 24; k++) acc[k] = cy[k] + cf * acc[k];
             } else {
@@ -208,19 +208,102 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
         }
         if (POST != 0) {
             T w[24];
-            clover_apply<T>(a.clov_post, Vh, i, acc, w);
+            clover_apply<T, STREAM>(a.clov_post, Vh, i, acc, w);
 #pragma unroll
             for (int k = 0; k < 24; k++) acc[k] = w[k];
         }
-        store_reals<T, 24>(a.out, Vh, i, acc);
-        if (a.red.partials) {
+        store_reals<T, 24>(out, Vh, i, acc);
+        if (want_norm) {
             T s2 = 0;
 #pragma unroll
             for (int k = 0; k < 24; k++) s2 += acc[k] * acc[k];
             nrm = (double)s2;
         }
     }
-    if (a.red.partials) grid_sum_finalize(nrm, a.red, a.counter, a.norm_out, a.norm_accumulate != 0);
+    return nrm;
+}
+
+template <int FMT, int XPAY, int POST>
+__global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
+{
+    if (a.skip && *a.skip) return;
+    const int i = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
+    const bool want_norm = a.red.partials != nullptr;
+    double nrm = 0.0;
+    if (i < a.g.Vh) nrm = dslash_site<FMT, XPAY, POST, true>(a, i, a.in, a.y, a.out, want_norm);
+    if (want_norm) grid_sum_finalize(nrm, a.red, a.counter, a.norm_out, a.norm_accumulate != 0);
+}
+
+// ---- multi-right-hand-side variant (MrhsArgs in cola_internal.h)
+#ifndef COLA_MRHS_PER_BLOCK_F32
+#define COLA_MRHS_PER_BLOCK_F32 4
+#endif
+#ifndef COLA_MRHS_PER_BLOCK_F64
+#define COLA_MRHS_PER_BLOCK_F64 2
+#endif
+#ifndef COLA_MRHS_MINB
+#define COLA_MRHS_MINB 3
+#endif
+#ifndef COLA_MRHS_SITES
+#define COLA_MRHS_SITES 64
+#endif
+#ifndef COLA_MRHS_TILE_X
+#define COLA_MRHS_TILE_X 16
+#endif
+constexpr int MSITES = COLA_MRHS_SITES;
+template <int FMT> struct MrhsCfg { static constexpr int NRB = (FMT == LINK_F64_18) ? COLA_MRHS_PER_BLOCK_F64 : COLA_MRHS_PER_BLOCK_F32; };
+
+template <int FMT, int XPAY, int POST>
+__global__ void __launch_bounds__(MSITES * MrhsCfg<FMT>::NRB, COLA_MRHS_MINB) dslash_mrhs_kernel(const __grid_constant__ MrhsArgs m)
+{
+    constexpr int NRB = MrhsCfg<FMT>::NRB;
+    if (m.d.skip && *m.d.skip) return;
+    const Geom &g = m.d.g;
+    const Tile &tl = m.tile;
+    const unsigned sb = blockIdx.x / (unsigned)m.ngroups, grp = blockIdx.x - sb * (unsigned)m.ngroups;
+    const int k = (int)grp * NRB + (int)threadIdx.y;
+    // site of this thread: tile origin (block-uniform) + position inside the tile
+    const unsigned b1 = tl.nb[0].div(sb), b2 = tl.nb[1].div(b1), b3 = tl.nb[2].div(b2);
+    const unsigned l = threadIdx.x;
+    const int s0 = tl.sh[0], s1 = tl.sh[1], s2 = tl.sh[2];
+    const int xh = (int)((sb - b1 * tl.nb[0].d) << s0) + (int)(l & ((1u << s0) - 1u));
+    const int y = (int)((b1 - b2 * tl.nb[1].d) << s1) + (int)((l >> s0) & ((1u << s1) - 1u));
+    const int z = (int)((b2 - b3 * tl.nb[2].d) << s2) + (int)((l >> (s0 + s1)) & ((1u << s2) - 1u));
+    const int t = (int)(b3 << tl.sh[3]) + (int)(l >> (s0 + s1 + s2));
+    const int i = xh + g.Xh * (y + g.Y * (z + g.Z * t));
+    const bool want_norm = m.partials != nullptr;
+    const bool live = k < m.nrhs && (int)l < tl.vol;
+    const size_t vec = k < m.nrhs ? (size_t)m.list[k] : 0;
+    double nrm = 0.0;
+    if (live)
+        nrm = dslash_site<FMT, XPAY, POST, false>(m.d, i, reinterpret_cast<const char *>(m.d.in) + vec * m.in_stride,
+                                                  reinterpret_cast<const char *>(m.d.y) + vec * m.y_stride,
+                                                  reinterpret_cast<char *>(m.d.out) + vec * m.out_stride, want_norm);
+    if (want_norm) {   // one partial per (vector, site block): the warps of a row (threadIdx.y) hold one right-hand side
+        __shared__ double sm[NRB][MSITES / 32];
+        const double w = warp_sum(nrm);
+        if ((threadIdx.x & 31) == 0) sm[threadIdx.y][threadIdx.x >> 5] = w;
+        __syncthreads();
+        if (threadIdx.x == 0 && k < m.nrhs) {
+            double tsum = 0.0;
+#pragma unroll
+            for (int q = 0; q < MSITES / 32; q++) tsum += sm[threadIdx.y][q];
+            m.partials[vec * (size_t)m.nsb + sb] = tsum;
+        }
+    }
+}
+
+// out[vec] (+)= sum over site blocks of partials[vec][.], one block per right-hand side, fixed order
+__global__ void __launch_bounds__(256) mrhs_reduce_kernel(const double *partials, int nsb, const __grid_constant__ MrhsList list, const int *skip, double *out, int accumulate)
+{
+    if (skip && *skip) return;
+    __shared__ double sm[33];
+    const int vec = list.v[blockIdx.x];
+    const double *p = partials + (size_t)vec * nsb;
+    double a = 0.0;
+    for (int k = threadIdx.x; k < nsb; k += 256) a += p[k];
+    a = block_sum(a, sm);
+    if (threadIdx.x == 0) out[vec] = accumulate ? out[vec] + a : a;
 }
 
 template <typename T>
@@ -249,7 +332,87 @@ cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
     return cudaGetLastError();
 }
 
+template <int FMT>
+cudaError_t launch_mrhs_fmt(MrhsArgs &m, cudaStream_t s)
+{
+    constexpr int NRB = MrhsCfg<FMT>::NRB;
+    const int xpay = m.d.y ? (m.d.clov_y ? 2 : 1) : 0;
+    const int post = m.d.clov_post ? 1 : 0;
+    m.tile = make_tile(m.d.g, MSITES, COLA_MRHS_TILE_X);
+    m.nsb = m.tile.ntiles;
+    m.ngroups = (m.nrhs + NRB - 1) / NRB;
+    const dim3 grid((unsigned)m.nsb * (unsigned)m.ngroups), block(MSITES, NRB);
+    if (xpay == 0 && post == 0) dslash_mrhs_kernel<FMT, 0, 0><<<grid, block, 0, s>>>(m);
+    else if (xpay == 0 && post == 1) dslash_mrhs_kernel<FMT, 0, 1><<<grid, block, 0, s>>>(m);
+    else if (xpay == 1 && post == 0) dslash_mrhs_kernel<FMT, 1, 0><<<grid, block, 0, s>>>(m);
+    else if (xpay == 1 && post == 1) dslash_mrhs_kernel<FMT, 1, 1><<<grid, block, 0, s>>>(m);
+    else if (xpay == 2 && post == 0) dslash_mrhs_kernel<FMT, 2, 0><<<grid, block, 0, s>>>(m);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
 }  // namespace
+
+// Tile = the largest power-of-two box of at most max_sites sites whose extents divide the lattice extents: x first, up
+// to max_x checkerboard sites (coalescing), then y, z, t doubled in turn so the tile stays close to a hypercube.
+Tile make_tile(const Geom &g, int max_sites, int max_x)
+{
+    Tile t;
+    const int ext[4] = {g.Xh, g.Y, g.Z, g.T};
+    int vol = 1;
+    for (int k = 0; k < 4; k++) t.sh[k] = 0;
+    while (vol * 2 <= max_sites && (1 << (t.sh[0] + 1)) <= max_x && ext[0] % (1 << (t.sh[0] + 1)) == 0) {
+        t.sh[0]++;
+        vol *= 2;
+    }
+#ifdef COLA_MRHS_TILE_LINEAR   // tuning experiment: fill y completely, then z, then t (a contiguous run of sites)
+    for (int k = 1; k < 4; k++)
+        while (vol * 2 <= max_sites && ext[k] % (1 << (t.sh[k] + 1)) == 0) {
+            t.sh[k]++;
+            vol *= 2;
+        }
+#endif
+    for (bool grown = true; grown && vol * 2 <= max_sites;) {
+        grown = false;
+        for (int k = 1; k < 4 && vol * 2 <= max_sites; k++) {
+            if (ext[k] % (1 << (t.sh[k] + 1)) == 0) {
+                t.sh[k]++;
+                vol *= 2;
+                grown = true;
+            }
+        }
+    }
+    while (vol * 2 <= max_sites && ext[0] % (1 << (t.sh[0] + 1)) == 0) {   // y, z, t exhausted (tiny lattice): give x the rest
+        t.sh[0]++;
+        vol *= 2;
+    }
+    t.vol = vol;
+    t.ntiles = g.Vh / vol;
+    for (int k = 0; k < 3; k++) t.nb[k] = make_fastdiv((unsigned)(ext[k] >> t.sh[k]));
+    return t;
+}
+
+int mrhs_site_blocks(const Geom &g) { return make_tile(g, MSITES, COLA_MRHS_TILE_X).ntiles; }
+
+cudaError_t launch_dslash_mrhs(int fmt, MrhsArgs &m, cudaStream_t s)
+{
+    if (m.nrhs < 1 || m.nrhs > MRHS_MAX) return cudaErrorInvalidValue;
+    switch (fmt) {
+        case LINK_F64_18: return launch_mrhs_fmt<LINK_F64_18>(m, s);
+        case LINK_F32_18: return launch_mrhs_fmt<LINK_F32_18>(m, s);
+        case LINK_F32_12: return launch_mrhs_fmt<LINK_F32_12>(m, s);
+    }
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_mrhs_reduce(const double *partials, int nsb, int nrhs, const int *list, double *out, int accumulate, const int *skip, cudaStream_t s)
+{
+    if (nrhs < 1 || nrhs > MRHS_MAX) return cudaErrorInvalidValue;
+    MrhsList l;
+    for (int k = 0; k < MRHS_MAX; k++) l.v[k] = k < nrhs ? list[k] : 0;
+    mrhs_reduce_kernel<<<nrhs, 256, 0, s>>>(partials, nsb, l, skip, out, accumulate);
+    return cudaGetLastError();
+}
 
 size_t dslash_grid_blocks(size_t Vh) { return (Vh + DSLASH_BLOCK - 1) / DSLASH_BLOCK; }
 

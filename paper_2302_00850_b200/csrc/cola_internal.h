@@ -59,6 +59,32 @@ struct Ctl {
     unsigned counter[8];  // "last block" tickets, one per concurrently used reduction
 };
 
+constexpr int MRHS_MAX = 16;   // right-hand sides per batched launch / solve
+
+// Device-resident scalars of the batched (multi-right-hand-side) CGLS: one entry per vector.  Lives in the control
+// block next to Ctl.  `flag` stops the whole batch (every queued kernel becomes a no-op) when any active system asks
+// for a reliable update or converges; `trig` says which ones.
+struct CtlM {
+    double gam[2][MRHS_MAX];
+    double qq[MRHS_MAX];
+    double rr[MRHS_MAX];
+    double rmax2[MRHS_MAX];
+    double target2[MRHS_MAX];
+    double delta2;
+    int flag;
+    int iters;
+    unsigned trig;        // bit n: vector n raised the flag in iteration `iters`
+};
+// What the decision kernel publishes into mapped pinned host memory (rr, trig, flag first; `iters` last, after a
+// system fence: it is the sequence number the host polls).
+struct HostStatusM {
+    double rr[MRHS_MAX];
+    unsigned trig;
+    int flag;
+    int iters;
+};
+struct MrhsList { int v[MRHS_MAX]; };
+
 constexpr unsigned REDUCE_GROUP = 256;
 __host__ __device__ inline size_t reduce_groups(size_t nblocks) { return (nblocks + REDUCE_GROUP - 1) / REDUCE_GROUP; }
 
@@ -101,7 +127,40 @@ struct DslashArgs {
     const int *skip;        // if non-null and *skip != 0 the launch is a no-op (speculatively queued iteration)
 };
 
+// Multi-right-hand-side launch of the same kernel family: `nrhs` vectors share one pass over
+// the links and the clover field.  Vector k of the launch is vector list[k] of the caller's arrays: `in`, `out`, `y`
+// of `d` point at vector 0 and consecutive vectors are `*_stride` bytes apart.  A thread block covers the sites of a
+// single-rhs block for MRHS_PER_BLOCK right-hand sides (threadIdx.y), so the link a site needs is fetched from L2
+// once per block and served to the other right-hand sides by L1; blocks of the same sites and different rhs groups
+// are adjacent in the grid, so DRAM sees each link once per launch.
+// 4-D tile of sites covered by one thread block of the multi-rhs kernels: 2^sh[0] x 2^sh[1] x 2^sh[2] x 2^sh[3]
+// (x in checkerboard sites), each extent dividing the lattice extent.  With several right-hand sides per link the
+// kernels are bound by L2-to-L1 traffic, most of it neighbour spinors; a compact tile lets L1 serve the neighbours
+// inside the tile in all four directions (the single-rhs kernels are DRAM-bound and prefer long contiguous runs).
+struct Tile {
+    int sh[4];
+    int vol;          // sites per tile
+    int ntiles;
+    FastDiv nb[3];    // tiles along x, y, z
+};
+Tile make_tile(const Geom &g, int max_sites, int max_x);
+
+struct MrhsArgs {
+    DslashArgs d;
+    Tile tile;           // d.red / d.counter / d.norm_out unused (per-rhs norms go through `partials`)
+    int nrhs;               // right-hand sides of this launch, 1..MRHS_MAX
+    int ngroups;            // rhs groups per site block (filled by the launcher)
+    int nsb;                // site blocks (filled by the launcher)
+    size_t in_stride, out_stride, y_stride;
+    int list[MRHS_MAX];
+    double *partials;       // [vector][nsb] per-block |v|^2, or nullptr; reduce with launch_mrhs_reduce
+};
+
 // launchers (cola_dslash.cu)
+cudaError_t launch_dslash_mrhs(int fmt, MrhsArgs &m, cudaStream_t s);
+int mrhs_site_blocks(const Geom &g);   // site blocks (tiles) of a multi-rhs launch = partial sums per vector
+// out[list[k]] (+)= sum_sb partials[list[k]*nsb + sb], fixed order
+cudaError_t launch_mrhs_reduce(const double *partials, int nsb, int nrhs, const int *list, double *out, int accumulate, const int *skip, cudaStream_t s);
 size_t dslash_grid_blocks(size_t Vh);   // blocks a dslash launch uses = partial sums it may write
 cudaError_t launch_dslash(int fmt, const DslashArgs &a, cudaStream_t s);
 // clover-only apply: out = C in on one parity (cola_dslash.cu)
@@ -130,5 +189,16 @@ cudaError_t launch_axpby64(void *out64, double a, const void *A64, double b, con
                            const ReduceWs *red, unsigned *counter, double *norm_out, cudaStream_t s);
 // x64 += x32; x32 = 0
 cudaError_t launch_accumulate(void *x64, void *x32, size_t n_sites, cudaStream_t s);
+
+// ---- batched BLAS-1 over the vectors list.v[0..nrhs) (cola_blas.cu); vector n of an array starts n*stride bytes in.
+int blas_mrhs_blocks(size_t n_sites, cola_prec prec);   // blocks per vector of a batched BLAS launch = partials per vector
+// r[n] -= alpha_n q[n], alpha_n = gam[cur][n]/qq[n];  partials[n][block] = block sums of |r[n]|^2
+cudaError_t launch_r_update_mrhs(cola_prec prec, void *r, const void *q, size_t stride, const CtlM *ctl, int cur, const MrhsList &list, int nrhs,
+                                 const int *skip, size_t n_sites, double *partials, cudaStream_t s);
+// after launch_mrhs_reduce(partials -> ctl->rr): rmax2, per-vector trigger, ctl->flag, status -> mapped host memory
+cudaError_t launch_decide_mrhs(CtlM *ctl, const MrhsList &list, int nrhs, int iter, const int *skip, HostStatusM *mirror, cudaStream_t s);
+// x[n] += alpha_n p[n] (do_x);  p[n] = s[n] + beta_n p[n], beta_n = gam[cur^1][n]/gam[cur][n] (do_p)
+cudaError_t launch_xp_update_mrhs(cola_prec prec, void *x, void *p, const void *sv, size_t stride, const CtlM *ctl, int cur, const MrhsList &list, int nrhs,
+                                  int do_x, int do_p, const int *skip, size_t n_sites, cudaStream_t s);
 
 }  // namespace cola
