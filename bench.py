@@ -186,7 +186,7 @@ def reference_arm(args, cfg, workload):
 
     dims, kappa, csw = cfg["dims"], cfg["kappa"], cfg["csw"]
     dev = "cuda" if torch.cuda.is_available() else "cpu"
-    U = inputs.make_links(args.config, device=dev).cpu()
+    U = inputs.make_links(args.config, dims=dims, device=dev).cpu()
     Un = U.numpy()
     A = oracle.clover(dims, Un, kappa, csw)
     Ainv = oracle.clover_inverse(A)
@@ -229,16 +229,23 @@ def main():
     ap.add_argument("--no-operator-table", action="store_true")
     ap.add_argument("--operators-only", action="store_true",
                     help="profiling aid: skip the solves, run only the operator table (few launches: --op-warm/--op-timed) and print it")
+    ap.add_argument("--lattice", default="", help="test aid: run the config's recipe on other extents, e.g. 16,16,16,32")
+    ap.add_argument("--no-batched", action="store_true", help="config 3: skip the batched (multi-rhs) solve of the 12 sources")
     ap.add_argument("--op-warm", type=int, default=20)
     ap.add_argument("--op-timed", type=int, default=200)
     args = ap.parse_args()
 
-    cfg = inputs.CONFIGS[args.config]
+    cfg = dict(inputs.CONFIGS[args.config])
+    if args.lattice:   # test aid: the same recipe on other extents (the line's config.lattice says so; not a bench value)
+        cfg["dims"] = tuple(int(v) for v in args.lattice.split(","))
     dims = cfg["dims"]
     workload = {
         "workload": f"BASELINE.json configs[{args.config}]: {dims[0]}x{dims[1]}x{dims[2]}x{dims[3]} lattice, links exp(i*{cfg['eps']}*H) seeded, "
-                    f"kappa={cfg['kappa']}, csw={cfg['csw']}, bc=(+,+,+,-), Gaussian source, fp32 links stored as 12 reals; "
-                    "step = mixed-precision (fp32 inner / fp64 reliable updates, delta=0.1) even-odd CGNR to 1e-10",
+                    f"kappa={cfg['kappa']}, csw={cfg['csw']}, bc=(+,+,+,-), "
+                    + ("12 point sources at the origin (one per spin-colour component) solved one after the other"
+                       if cfg["source"] == "point" else "Gaussian source")
+                    + ", fp32 links stored as 12 reals; step = mixed-precision (fp32 inner / fp64 reliable updates, delta=0.1) "
+                      "even-odd CGNR to 1e-10" + (" for each source" if cfg["source"] == "point" else ""),
         "lattice": list(dims), "kappa": cfg["kappa"], "csw": cfg["csw"], "tol": 1e-10, "parallelism": f"replicas x{args.gpus}",
         "l2": "inputs larger than L2 (fp32 gauge+clover alone are > 1 GB per operator application at 32^3x64)",
     }
@@ -260,8 +267,16 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     # ---- setup (H0-H2), not part of a step
-    U = inputs.make_links(args.config, device=dev)
-    b = inputs.source_gaussian(dims, inputs.config_seed_source(args.config) + rank, device=dev)
+    U = inputs.make_links(args.config, dims=dims, device=dev)
+    point = cfg["source"] == "point"    # BJ:c3: 12 point sources at the origin, one per spin-colour component
+    if point:
+        def source(n):
+            return inputs.source_point(dims, n // 3, n % 3, device=dev)
+        n_src = 12
+    else:
+        def source(n):
+            return inputs.source_gaussian(dims, inputs.config_seed_source(args.config) + rank, device=dev)
+        n_src = 1
     ctx = binding.Cola(dims, cfg["kappa"], cfg["csw"], bc=inputs.BC, compress12=True, device=local)
     torch.cuda.synchronize()
     t0 = time.time()
@@ -282,9 +297,21 @@ def main():
                           "operators": operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed)}))
         return
 
+    def one_step():
+        """One pass of the hot path over the configuration's sources, solved one after the other."""
+        fl, infos = 0.0, []
+        for n in range(n_src):
+            bn = b if n_src == 1 else source(n)
+            xn, info = ctx.cg_solve(bn, tol=1e-10, even_odd=True, mixed=True)
+            fl += info["op_flops"]
+            infos.append(info)
+            del xn
+        return fl, infos
+
+    b = source(0) if n_src == 1 else None
     # ---- device-resident steps
     for _ in range(args.warmup):
-        x, info = ctx.cg_solve(b, tol=1e-10, even_odd=True, mixed=True)
+        one_step()
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
@@ -293,30 +320,70 @@ def main():
     e0.record()
     flops = 0.0
     for _ in range(args.steps):
-        x, info = ctx.cg_solve(b, tol=1e-10, even_odd=True, mixed=True)
-        flops += info["op_flops"]
+        fl, infos = one_step()
+        flops += fl
     e1.record()
     barrier()
     launches = ctx.launch_count() - l0
     clocks = sampler.stop()
+    info = infos[-1]
     ms_local = e0.elapsed_time(e1)
     ms, flops_all = aggregate_over_ranks(ms_local, flops, device=dev)
     value = flops_all / (ms * 1e-3) / 1e9
 
     # ---- end to end: host buffers through cola_cg_solve_host
-    b_host = b.cpu().pin_memory()
+    b_host = source(0).cpu().pin_memory()
     x_host = torch.empty_like(b_host).pin_memory()
-    ctx.cg_solve(b_host, tol=1e-10, even_odd=True, mixed=True, x=x_host)
+
+    def host_step():
+        fl = 0.0
+        for n in range(n_src):
+            if n_src > 1:
+                b_host.zero_()
+                b_host[0, 0, 0, 0, n // 3, n % 3] = 1.0
+            _, info_e = ctx.cg_solve(b_host, tol=1e-10, even_odd=True, mixed=True, x=x_host)
+            fl += info_e["op_flops"]
+        return fl
+
+    host_step()
     barrier()
     e0.record()
     flops_e = 0.0
     for _ in range(args.steps):
-        _, info_e = ctx.cg_solve(b_host, tol=1e-10, even_odd=True, mixed=True, x=x_host)
-        flops_e += info_e["op_flops"]
+        flops_e += host_step()
     e1.record()
     barrier()
     ms_e, flops_e_all = aggregate_over_ranks(e0.elapsed_time(e1), flops_e, device=dev)
-    nbytes = b_host.numel() * b_host.element_size()
+    nbytes = b_host.numel() * b_host.element_size() * n_src
+
+    # ---- the same sources as ONE batched solve (links and clover read once per pass for all)
+    batched = None
+    if n_src > 1 and rank == 0 and not args.no_batched:
+        del b_host, x_host
+        torch.cuda.empty_cache()
+        try:
+            bs = torch.stack([source(n) for n in range(n_src)])
+            xs = torch.empty_like(bs)
+            ctx.set_mrhs_workspace(n_src)
+            for _ in range(min(args.warmup, 1)):
+                ctx.cg_solve_mrhs(bs, tol=1e-10, x=xs)
+            torch.cuda.synchronize()
+            e0.record()
+            fl_b = 0.0
+            for _ in range(args.steps):
+                _, infos_b = ctx.cg_solve_mrhs(bs, tol=1e-10, x=xs)
+                fl_b += sum(i["op_flops"] for i in infos_b)
+            e1.record()
+            torch.cuda.synchronize()
+            ms_b = e0.elapsed_time(e1) / args.steps
+            batched = {"ms_per_step": round(ms_b, 3), "GFLOP/s": round(fl_b / args.steps / (ms_b * 1e-3) / 1e9, 1),
+                       "speedup_vs_sequential": round(ms / args.steps / ms_b, 3), "nrhs": n_src,
+                       "iters": [i["iters"] for i in infos_b], "reliable_updates": [i["reliable_updates"] for i in infos_b],
+                       "max_true_residual": max(i["true_residual"] for i in infos_b)}
+            del bs, xs
+        except (RuntimeError, binding.ColaError) as ex:   # e.g. out of memory for 12 systems at once
+            batched = {"unavailable": str(ex)[:200]}
+        torch.cuda.empty_cache()
 
     if rank != 0:
         if world > 1:
@@ -352,6 +419,11 @@ def main():
                 "ms_per_step": round(ms_e / args.steps, 3)},
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "cpu_baseline": cpu, "operators": table,
     }
+    if n_src > 1:
+        line["solve"]["sources"] = n_src
+        line["solve"]["iters_per_source"] = [i["iters"] for i in infos]
+        line["solve"]["max_true_residual"] = max(i["true_residual"] for i in infos)
+        line["batched"] = batched
     print(json.dumps(line))
     if world > 1:
         torch.distributed.destroy_process_group()
