@@ -45,6 +45,7 @@ FLOPS = {"dslash": 1320, "dslash_clover_inv": 1824, "dslash_clover_xpay": 1872}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of dslash_kernel<F32x12, XPAY=2> from the committed
 # ncu --set full capture (a number read from a profile, never a timing taken under the profiler)
 NCU_TRAFFIC = {(32, 32, 32, 64): {"bytes_per_launch": 980280000, "source": "profiles/r1b_operators_full.txt (909.4 MB read + 70.88 MB write)"}}
+CPU_SAMPLE_MAX_SITES = 1 << 22   # largest lattice the oracle's full fields are built for inside bench.py
 NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star's denominator, reported beside the measured one
 
 
@@ -122,8 +123,9 @@ def time_launches(fn, n_warm, n_timed):
     return e0.elapsed_time(e1) / n_timed
 
 
-def operator_table(ctx, fmt32, n_warm=20, n_timed=200):
-    """Per-kernel throughput of the operator family, each timed alone (inputs larger than L2)."""
+def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
+    """Per-kernel throughput of the operator family, each timed alone (inputs larger than L2).
+    nrhs > 1 adds the multi-right-hand-side Schur operator over nrhs vectors."""
     peak, _ = measured_peaks()
     out = {}
     Vh = ctx.Vh
@@ -148,6 +150,22 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200):
             out[f"{name}_{fmt}"] = {"ms": round(ms, 5), "launches": launches, "GB/s": round(gbs, 1), "GFLOP/s": round(flops / (ms * 1e-3) / 1e9, 1),
                                     "frac_measured": round(gbs / peak, 4), "frac_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4)}
         del full, dst
+        if nrhs > 1:
+            ctx.set_mrhs_workspace(nrhs)
+            vin = ctx.empty_internal_mrhs(nrhs, prec, full=False).normal_()
+            vout = torch.empty_like(vin)
+            ms = time_launches(lambda: ctx.schur_apply_mrhs(vin, out=vout), max(n_warm // 4, 1), max(n_timed // 4, 1))
+            w = 4 if prec == torch.float32 else 8
+            G = {"f32x12": 12, "f32x18": 18, "f64x18": 18}[fmt]
+            # per site and vector: links and clover of both kernels shared by nrhs vectors + 5 spinor passes
+            nbytes = ((2 * 8 * G + 2 * 72) * w / nrhs + 5 * 24 * w) * Vh * nrhs
+            flops = (FLOPS["dslash_clover_inv"] + FLOPS["dslash_clover_xpay"]) * Vh * nrhs
+            single = out[f"schur_{fmt}"]["ms"]
+            out[f"schur_mrhs{nrhs}_{fmt}"] = {"ms": round(ms, 5), "launches": 2, "ms_per_rhs": round(ms / nrhs, 5), "speedup_vs_single": round(single / (ms / nrhs), 3),
+                                              "GB/s": round(nbytes / (ms * 1e-3) / 1e9, 1), "GFLOP/s": round(flops / (ms * 1e-3) / 1e9, 1)}
+            del vin, vout
+            ctx.release_mrhs_workspace()
+            torch.cuda.empty_cache()
     return out
 
 
@@ -185,6 +203,10 @@ def reference_arm(args, cfg, workload):
     import oracle
 
     dims, kappa, csw = cfg["dims"], cfg["kappa"], cfg["csw"]
+    note = ""
+    if inputs.volume(dims) > CPU_SAMPLE_MAX_SITES:   # see main(): the oracle's fields for the big lattices exceed host memory
+        note = f"; run on (32, 32, 32, 64) extents of the same link recipe because the oracle's fields for {tuple(dims)} exceed host memory"
+        dims = (32, 32, 32, 64)
     dev = "cuda" if torch.cuda.is_available() else "cpu"
     U = inputs.make_links(args.config, dims=dims, device=dev).cpu()
     Un = U.numpy()
@@ -205,7 +227,7 @@ def reference_arm(args, cfg, workload):
         x = step(x)
     dt = time.time() - t0
     val = args.steps * 2 * 3696.0 * Vh / dt / 1e9
-    sample = f"each step = one (S, S^dagger) oracle application pair on the full {dims} lattice (operator work of one CGLS iteration)"
+    sample = f"each step = one (S, S^dagger) oracle application pair on the full {dims} lattice (operator work of one CGLS iteration)" + note
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": round(val, 3), "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(dt / args.steps * 1e3, 2), "higher_is_better": True, "scaling": "weak",
@@ -231,6 +253,7 @@ def main():
                     help="profiling aid: skip the solves, run only the operator table (few launches: --op-warm/--op-timed) and print it")
     ap.add_argument("--lattice", default="", help="test aid: run the config's recipe on other extents, e.g. 16,16,16,32")
     ap.add_argument("--no-batched", action="store_true", help="config 3: skip the batched (multi-rhs) solve of the 12 sources")
+    ap.add_argument("--nrhs", type=int, default=0, help="with --operators-only: also time the multi-rhs Schur operator over this many vectors")
     ap.add_argument("--op-warm", type=int, default=20)
     ap.add_argument("--op-timed", type=int, default=200)
     args = ap.parse_args()
@@ -283,7 +306,15 @@ def main():
     ctx.gauge_upload(U)
     torch.cuda.synchronize()
     setup_s = time.time() - t0
-    U_cpu = U.cpu() if (rank == 0 and world == 1 and not args.no_cpu_baseline) else None
+    want_cpu = rank == 0 and world == 1 and not args.no_cpu_baseline
+    cpu_dims = tuple(dims)
+    if want_cpu and inputs.volume(dims) > CPU_SAMPLE_MAX_SITES:
+        # the oracle's dense 12x12 clover field alone is 2.3 KB per site: on the big lattices the bounded CPU sample
+        # runs the same recipe (links, kappa, csw) on 32^3x64 extents; the oracle's cost per site does not depend on V
+        cpu_dims = (32, 32, 32, 64)
+        U_cpu = inputs.make_links(args.config, dims=cpu_dims, device=dev).cpu()
+    else:
+        U_cpu = U.cpu() if want_cpu else None
     del U
     torch.cuda.empty_cache()
 
@@ -294,7 +325,7 @@ def main():
 
     if args.operators_only:   # not a bench line: a short launch sequence for ncu captures of each operator kernel
         print(json.dumps({"operators_only": True, "lattice": list(dims),
-                          "operators": operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed)}))
+                          "operators": operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed, nrhs=args.nrhs)}))
         return
 
     def one_step():
@@ -406,7 +437,9 @@ def main():
             roof["traffic_source"] = NCU_TRAFFIC[tuple(dims)]["source"]
     cpu = None
     if U_cpu is not None:
-        cpu = cpu_baseline_sample(cfg, U_cpu)
+        cpu = cpu_baseline_sample(dict(cfg, dims=cpu_dims), U_cpu)
+        if cpu_dims != tuple(dims):
+            cpu["sample"] += f"; run on {cpu_dims} extents of the same link recipe because the oracle's fields for {tuple(dims)} exceed host memory"
 
     line = {
         "metric": METRIC, "value": round(value, 1), "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -157,7 +157,8 @@ cola_status cola_cg_solve_host(cola_ctx *c, const cola_solve_params *sp, const v
  * "nrhs vectors" = nrhs internal buffers of the stated size stored back to back.
  *
  * Workspace: a second caller-owned DEVICE buffer holding, per right-hand side, the Schur temporaries and the vectors
- * of the batched solver (5.5 fp64 half-lattice vectors).  Borrowed until cola_destroy / the next call. */
+ * of the batched solver (5.5 fp64 half-lattice vectors).  Borrowed until cola_destroy / the next call;
+ * cola_set_mrhs_workspace(c, NULL, 0, 0) gives it back. */
 size_t cola_mrhs_workspace_bytes(const cola_ctx *c, int nrhs);
 cola_status cola_set_mrhs_workspace(cola_ctx *c, void *dev_ptr, size_t bytes, int nrhs);
 /* out_p[n] = D_{p,1-p} in[n]: nrhs half-lattice internal DEVICE vectors each, no overlap. */

@@ -320,10 +320,15 @@ class Cola:
     def set_mrhs_workspace(self, nrhs: int, tensor: torch.Tensor | None = None):
         """Lend the per-right-hand-side workspace (allocated here with torch if not given)."""
         if tensor is None:
+            self.release_mrhs_workspace()
             tensor = torch.empty(self.mrhs_workspace_bytes(nrhs), dtype=torch.uint8, device=self.device)
         self._ck(_lib.cola_set_mrhs_workspace(self._h, ctypes.c_void_p(tensor.data_ptr()), tensor.numel() * tensor.element_size(), int(nrhs)))
         self._mws, self._mws_nrhs = tensor, int(nrhs)
         return tensor
+
+    def release_mrhs_workspace(self):
+        self._ck(_lib.cola_set_mrhs_workspace(self._h, None, 0, 0))
+        self._mws, self._mws_nrhs = None, 0
 
     def _need_mrhs(self, nrhs):
         if self._mws is None or self._mws_nrhs < nrhs:

@@ -1074,6 +1074,7 @@ cola_status cola_set_mrhs_workspace(cola_ctx *c, void *dev_ptr, size_t bytes, in
 {
     if (!c) return COLA_EINVAL;
     c->m_nrhs = 0;
+    if (!dev_ptr && nrhs == 0) return COLA_OK;   // release
     if (nrhs < 1 || nrhs > MRHS_MAX) return fail(c, COLA_EINVAL, "cola_set_mrhs_workspace: nrhs must be 1..16");
     if (!dev_ptr || ((uintptr_t)dev_ptr & 255)) return fail(c, COLA_EINVAL, "cola_set_mrhs_workspace: pointer must be non-NULL and 256-byte aligned");
     const CarveM k = carve_m(c, nrhs);
