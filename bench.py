@@ -37,9 +37,10 @@ from paper_2302_00850_b200 import inputs  # noqa: E402
 
 # algorithmic bytes per output site, fp32 with 12-real links; fp64 x18 in the second column
 BYTES = {
-    "dslash": {"f32x12": 576, "f32x18": 768, "f64x18": 1536},          # 8 links + 1 spinor in + 1 out
-    "dslash_clover_inv": {"f32x12": 864, "f32x18": 1056, "f64x18": 2112},   # + 72 reals clover
-    "dslash_clover_xpay": {"f32x12": 960, "f32x18": 1152, "f64x18": 2304},  # + 72 clover + 24 (x)
+    # f32h16 = COLA_F32_H16: fp32 spinors, links as 12 x int16, clover as 72 x fp16
+    "dslash": {"f32x12": 576, "f32x18": 768, "f64x18": 1536, "f32h16": 384},          # 8 links + 1 spinor in + 1 out
+    "dslash_clover_inv": {"f32x12": 864, "f32x18": 1056, "f64x18": 2112, "f32h16": 528},   # + 72 reals clover
+    "dslash_clover_xpay": {"f32x12": 960, "f32x18": 1152, "f64x18": 2304, "f32h16": 624},  # + 72 clover + 24 (x)
 }
 FLOPS = {"dslash": 1320, "dslash_clover_inv": 1824, "dslash_clover_xpay": 1872}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of dslash_kernel<F32x12, XPAY=2> from the committed
@@ -129,14 +130,15 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
     peak, _ = measured_peaks()
     out = {}
     Vh = ctx.Vh
-    for prec, fmt in ((torch.float32, fmt32), (torch.float64, "f64x18")):
+    for prec, fmt in ((torch.float32, fmt32), (torch.float64, "f64x18"), (torch.float32, "f32h16")):
         full = ctx.empty_internal(prec, full=True).normal_()
         dst = ctx.empty_internal(prec, full=True)
+        h = fmt == "f32h16"
         rows = {
-            "dslash_even": ("dslash", 1, lambda: ctx.dslash_apply(0, full[1], out=dst[0])),
-            "dslash_odd": ("dslash", 1, lambda: ctx.dslash_apply(1, full[0], out=dst[1])),
-            "fermion_matrix": ("dslash_clover_xpay", 2, lambda: ctx.fermion_matrix_apply(full, out=dst)),
-            "schur": (None, 2, lambda: ctx.schur_apply(full[0], out=dst[0])),
+            "dslash_even": ("dslash", 1, lambda: ctx.dslash_apply(0, full[1], out=dst[0], h16=h)),
+            "dslash_odd": ("dslash", 1, lambda: ctx.dslash_apply(1, full[0], out=dst[1], h16=h)),
+            "fermion_matrix": ("dslash_clover_xpay", 2, lambda: ctx.fermion_matrix_apply(full, out=dst, h16=h)),
+            "schur": (None, 2, lambda: ctx.schur_apply(full[0], out=dst[0], h16=h)),
         }
         for name, (kind, launches, fn) in rows.items():
             ms = time_launches(fn, n_warm, n_timed)
@@ -150,7 +152,7 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
             out[f"{name}_{fmt}"] = {"ms": round(ms, 5), "launches": launches, "GB/s": round(gbs, 1), "GFLOP/s": round(flops / (ms * 1e-3) / 1e9, 1),
                                     "frac_measured": round(gbs / peak, 4), "frac_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4)}
         del full, dst
-        if nrhs > 1:
+        if nrhs > 1 and not h:
             ctx.set_mrhs_workspace(nrhs)
             vin = ctx.empty_internal_mrhs(nrhs, prec, full=False).normal_()
             vout = torch.empty_like(vin)
@@ -252,6 +254,7 @@ def main():
     ap.add_argument("--operators-only", action="store_true",
                     help="profiling aid: skip the solves, run only the operator table (few launches: --op-warm/--op-timed) and print it")
     ap.add_argument("--lattice", default="", help="test aid: run the config's recipe on other extents, e.g. 16,16,16,32")
+    ap.add_argument("--no-h16", action="store_true", help="skip the extra solve with 16-bit links/clover in the inner iteration")
     ap.add_argument("--no-batched", action="store_true", help="config 3: skip the batched (multi-rhs) solve of the 12 sources")
     ap.add_argument("--nrhs", type=int, default=0, help="with --operators-only: also time the multi-rhs Schur operator over this many vectors")
     ap.add_argument("--op-warm", type=int, default=20)
@@ -387,6 +390,35 @@ def main():
     ms_e, flops_e_all = aggregate_over_ranks(e0.elapsed_time(e1), flops_e, device=dev)
     nbytes = b_host.numel() * b_host.element_size() * n_src
 
+    # ---- the same step with the inner operator reading 16-bit links and clover (mixed = 2)
+    solve_h16 = None
+    if rank == 0 and not args.no_h16:
+        def h16_step():
+            fl, infs = 0.0, []
+            for n in range(n_src):
+                bn = b if n_src == 1 else source(n)
+                xn, inf = ctx.cg_solve(bn, tol=1e-10, even_odd=True, mixed=2)
+                fl += inf["op_flops"]
+                infs.append(inf)
+                del xn
+            return fl, infs
+
+        for _ in range(min(args.warmup, 2)):
+            h16_step()
+        torch.cuda.synchronize()
+        e0.record()
+        fl_h = 0.0
+        for _ in range(args.steps):
+            f1, infs_h = h16_step()
+            fl_h += f1
+        e1.record()
+        torch.cuda.synchronize()
+        ms_h = e0.elapsed_time(e1) / args.steps
+        solve_h16 = {"ms_per_step": round(ms_h, 3), "GFLOP/s": round(fl_h / args.steps / (ms_h * 1e-3) / 1e9, 1),
+                     "speedup_vs_fp32_inner": round(ms_local / args.steps / ms_h, 3), "iters": [i["iters"] for i in infs_h],
+                     "reliable_updates": [i["reliable_updates"] for i in infs_h],
+                     "max_true_residual": max(i["true_residual"] for i in infs_h), "converged": all(i["converged"] for i in infs_h)}
+
     # ---- the same sources as ONE batched solve (links and clover read once per pass for all)
     batched = None
     if n_src > 1 and rank == 0 and not args.no_batched:
@@ -457,6 +489,7 @@ def main():
         line["solve"]["iters_per_source"] = [i["iters"] for i in infos]
         line["solve"]["max_true_residual"] = max(i["true_residual"] for i in infos)
         line["batched"] = batched
+    line["solve_h16"] = solve_h16
     print(json.dumps(line))
     if world > 1:
         torch.distributed.destroy_process_group()

@@ -55,7 +55,13 @@ typedef enum {
     COLA_ENOMEM = 5      /* workspace too small */
 } cola_status;
 
-typedef enum { COLA_F64 = 0, COLA_F32 = 1 } cola_prec;
+/* COLA_F32_H16 ("additional computation in order to reduce traffic", P:45 mixed precision):
+ * fp32 spinors and fp32 arithmetic, but links read from 16-bit fixed point (12 reals, third row rebuilt) and the
+ * clover fields from fp16, which cuts the bytes per Schur application from 1824 to 1152 per site.  It is an
+ * approximate ("sloppy") operator, |K16 x - K x| / |K x| ~ 1e-4, meant for the inner iteration of the mixed-precision
+ * solver (cola_solve_params.mixed = 2), whose reliable updates use the exact fp64 operator.  Spinor buffers and
+ * cola_spinor_* calls take COLA_F32 for it. */
+typedef enum { COLA_F64 = 0, COLA_F32 = 1, COLA_F32_H16 = 2 } cola_prec;
 typedef enum { COLA_EVEN = 0, COLA_ODD = 1 } cola_parity;
 
 typedef struct {
@@ -126,7 +132,8 @@ typedef struct {
                           being iterated (M x = b, or S x_e = bhat_e whose residual equals the full one) */
     int max_iter;      /* CGLS passes (one K and one K^+ each) */
     int even_odd;      /* 0: CGNR on M (BJ:c0); 1: CGNR on the Schur complement + reconstruction */
-    int mixed;         /* 0: all fp64; 1: fp32 inner iteration with fp64 reliable updates */
+    int mixed;         /* 0: all fp64; 1: fp32 inner iteration with fp64 reliable updates;
+                          2: as 1, with the inner operator reading 16-bit links and clover (COLA_F32_H16) */
     double delta;      /* reliable-update threshold (mixed only); <= 0 selects the default 0.1 */
 } cola_solve_params;
 

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("COLA_LIBRARY_PATH") or os.path.join(_HERE, "libcola.so")
 
 COLA_OK, COLA_EINVAL, COLA_ECUDA, COLA_ENOTREADY, COLA_ENOCONV, COLA_ENOMEM = range(6)
-COLA_F64, COLA_F32 = 0, 1
+COLA_F64, COLA_F32, COLA_F32_H16 = 0, 1, 2
 COLA_EVEN, COLA_ODD = 0, 1
 STATUS_NAMES = {0: "COLA_OK", 1: "COLA_EINVAL", 2: "COLA_ECUDA", 3: "COLA_ENOTREADY", 4: "COLA_ENOCONV", 5: "COLA_ENOMEM"}
 
@@ -242,28 +242,37 @@ class Cola:
         self._ck(_lib.cola_spinor_convert(self._h, dp, ctypes.c_void_p(src.data_ptr()), ctypes.c_void_p(out.data_ptr()), 2 if full else 1))
         return out
 
-    # ---- H3-H8
-    def dslash_apply(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
-        pr = _PREC[inp.dtype]
+    # ---- H3-H8.  h16=True (fp32 tensors only): COLA_F32_H16, the operator that reads 16-bit links and clover
+    @staticmethod
+    def _op_prec(t: torch.Tensor, h16: bool) -> int:
+        pr = _PREC[t.dtype]
+        if h16:
+            if pr != COLA_F32:
+                raise ValueError("h16 operators take fp32 spinors")
+            return COLA_F32_H16
+        return pr
+
+    def dslash_apply(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
+        pr = self._op_prec(inp, h16)
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.Vh * 24
         if out is None:
-            out = self.empty_internal(pr, full=False)
+            out = self.empty_internal(inp.dtype, full=False)
         self._ck(_lib.cola_dslash_apply(self._h, pr, int(out_parity), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def fermion_matrix_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
-        pr = _PREC[inp.dtype]
+    def fermion_matrix_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
+        pr = self._op_prec(inp, h16)
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.V * 24
         if out is None:
-            out = self.empty_internal(pr, full=True)
+            out = self.empty_internal(inp.dtype, full=True)
         self._ck(_lib.cola_fermion_matrix_apply(self._h, pr, int(bool(dagger)), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def schur_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
-        pr = _PREC[inp.dtype]
+    def schur_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
+        pr = self._op_prec(inp, h16)
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.Vh * 24
         if out is None:
-            out = self.empty_internal(pr, full=False)
+            out = self.empty_internal(inp.dtype, full=False)
         self._ck(_lib.cola_schur_apply(self._h, pr, int(bool(dagger)), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
@@ -271,7 +280,7 @@ class Cola:
     @staticmethod
     def _solve_params(tol, max_iter, even_odd, mixed, delta):
         sp = ColaSolveParams()
-        sp.tol, sp.max_iter, sp.even_odd, sp.mixed, sp.delta = float(tol), int(max_iter), int(bool(even_odd)), int(bool(mixed)), float(delta)
+        sp.tol, sp.max_iter, sp.even_odd, sp.mixed, sp.delta = float(tol), int(max_iter), int(bool(even_odd)), int(mixed), float(delta)
         return sp
 
     @staticmethod
@@ -339,8 +348,8 @@ class Cola:
         one = self.empty_internal(prec, full=full)
         return torch.empty((int(nrhs),) + tuple(one.shape), dtype=one.dtype, device=self.device)
 
-    def dslash_apply_mrhs(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
-        pr, nrhs = _PREC[inp.dtype], inp.shape[0]
+    def dslash_apply_mrhs(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
+        pr, nrhs = self._op_prec(inp, h16), inp.shape[0]
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.Vh * 24
         self._need_mrhs(nrhs)
         if out is None:
@@ -348,8 +357,8 @@ class Cola:
         self._ck(_lib.cola_dslash_apply_mrhs(self._h, pr, int(out_parity), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def fermion_matrix_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
-        pr, nrhs = _PREC[inp.dtype], inp.shape[0]
+    def fermion_matrix_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
+        pr, nrhs = self._op_prec(inp, h16), inp.shape[0]
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.V * 24
         self._need_mrhs(nrhs)
         if out is None:
@@ -357,8 +366,8 @@ class Cola:
         self._ck(_lib.cola_fermion_matrix_apply_mrhs(self._h, pr, int(bool(dagger)), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def schur_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None) -> torch.Tensor:
-        pr, nrhs = _PREC[inp.dtype], inp.shape[0]
+    def schur_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
+        pr, nrhs = self._op_prec(inp, h16), inp.shape[0]
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.Vh * 24
         self._need_mrhs(nrhs)
         if out is None:
@@ -366,7 +375,7 @@ class Cola:
         self._ck(_lib.cola_schur_apply_mrhs(self._h, pr, int(bool(dagger)), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def cg_solve_mrhs(self, b: torch.Tensor, tol=1e-10, max_iter=20000, delta=0.1, x: torch.Tensor | None = None):
+    def cg_solve_mrhs(self, b: torch.Tensor, tol=1e-10, max_iter=20000, delta=0.1, x: torch.Tensor | None = None, mixed=1):
         """b: nrhs canonical complex128 sources, shape (nrhs, t, z, y, x, 4, 3), on the device.
         Returns (x, [info dict per system])."""
         assert b.is_cuda and b.dtype == torch.complex128 and b.dim() == 7 and b[0].numel() == self.V * 12
@@ -375,7 +384,7 @@ class Cola:
         self._need_mrhs(nrhs)
         if x is None:
             x = torch.empty_like(b)
-        sp = self._solve_params(tol, max_iter, True, True, delta)
+        sp = self._solve_params(tol, max_iter, True, mixed, delta)
         infos = (ColaSolveInfo * nrhs)()
         st = _lib.cola_cg_solve_mrhs(self._h, ctypes.byref(sp), nrhs, ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), infos)
         self._ck(st, ok=(COLA_OK, COLA_ENOCONV))

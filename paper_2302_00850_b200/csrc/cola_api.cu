@@ -21,6 +21,8 @@ struct cola_ctx {
     char *gauge64, *gauge32;        // [parity][mu][chunk][Vh]
     char *clovA64, *clovA32;        // [parity][chunk][Vh]
     char *clovI64, *clovI32;        // odd parity only
+    char *gauge16, *clovA16, *clovI16;   // 16-bit copies for COLA_F32_H16 (same index structure)
+    int sloppy16;                   // the running solve's inner operator reads the 16-bit fields
     char *tmp64, *tmp32;            // odd half-lattice temporaries of the Schur operator
     ReduceWs red;                   // deterministic-reduction buffers
     size_t red_blocks;              // max grid size of a reducing launch
@@ -69,11 +71,11 @@ static cola_status fail(cola_ctx *c, cola_status st, const char *fmt, const char
     } while (0)
 
 static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
-static size_t half_bytes(const cola_ctx *c, cola_prec prec) { return c->Vh * 24 * (prec == COLA_F64 ? 8 : 4); }
+static size_t half_bytes(const cola_ctx *c, cola_prec prec) { return c->Vh * 24 * (prec == COLA_F64 ? 8 : 4); }   // COLA_F32_H16: fp32 spinors
 static const size_t SCRATCH_HALF64 = 12;   // solver scratch in units of one fp64 half-lattice spinor
 
 struct Carve {
-    size_t gauge64, gauge32, clovA64, clovA32, clovI64, clovI32, tmp64, tmp32, partials, scratch, total;
+    size_t gauge64, gauge32, clovA64, clovA32, clovI64, clovI32, gauge16, clovA16, clovI16, tmp64, tmp32, partials, scratch, total;
 };
 
 static Carve carve(const cola_ctx *c)
@@ -88,6 +90,9 @@ static Carve carve(const cola_ctx *c)
     k.clovA32 = take(2 * 288 * Vh);
     k.clovI64 = take(576 * Vh);
     k.clovI32 = take(288 * Vh);
+    k.gauge16 = take(8 * link_bytes(LINK_I16_12) * Vh);
+    k.clovA16 = take(2 * CLOVER_H16_BYTES * Vh);
+    k.clovI16 = take(CLOVER_H16_BYTES * Vh);
     k.tmp64 = take(192 * Vh);
     k.tmp32 = take(96 * Vh);
     {
@@ -199,6 +204,7 @@ cola_status cola_set_workspace(cola_ctx *c, void *dev_ptr, size_t bytes)
     c->gauge64 = c->ws + k.gauge64; c->gauge32 = c->ws + k.gauge32;
     c->clovA64 = c->ws + k.clovA64; c->clovA32 = c->ws + k.clovA32;
     c->clovI64 = c->ws + k.clovI64; c->clovI32 = c->ws + k.clovI32;
+    c->gauge16 = c->ws + k.gauge16; c->clovA16 = c->ws + k.clovA16; c->clovI16 = c->ws + k.clovI16;
     c->tmp64 = c->ws + k.tmp64; c->tmp32 = c->ws + k.tmp32;
     {
         size_t nb = dslash_grid_blocks(c->Vh);
@@ -228,22 +234,27 @@ static cola_status need_ready(cola_ctx *c, const char *who)
     return COLA_OK;
 }
 
-static int fmt_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? (int)LINK_F64_18 : c->fmt32; }
+static int fmt_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? (int)LINK_F64_18 : (prec == COLA_F32_H16 ? (int)LINK_I16_12 : c->fmt32); }
 static char *gauge_of(const cola_ctx *c, cola_prec prec, int parity)
 {
-    return prec == COLA_F64 ? c->gauge64 + (size_t)parity * 4 * 144 * c->Vh : c->gauge32 + (size_t)parity * 4 * link_bytes(c->fmt32) * c->Vh;
+    if (prec == COLA_F64) return c->gauge64 + (size_t)parity * 4 * 144 * c->Vh;
+    if (prec == COLA_F32_H16) return c->gauge16 + (size_t)parity * 4 * link_bytes(LINK_I16_12) * c->Vh;
+    return c->gauge32 + (size_t)parity * 4 * link_bytes(c->fmt32) * c->Vh;
 }
 static char *clovA_of(const cola_ctx *c, cola_prec prec, int parity)
 {
-    return prec == COLA_F64 ? c->clovA64 + (size_t)parity * 576 * c->Vh : c->clovA32 + (size_t)parity * 288 * c->Vh;
+    if (prec == COLA_F64) return c->clovA64 + (size_t)parity * 576 * c->Vh;
+    if (prec == COLA_F32_H16) return c->clovA16 + (size_t)parity * CLOVER_H16_BYTES * c->Vh;
+    return c->clovA32 + (size_t)parity * 288 * c->Vh;
 }
-static char *clovI_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? c->clovI64 : c->clovI32; }
+static char *clovI_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? c->clovI64 : (prec == COLA_F32_H16 ? c->clovI16 : c->clovI32); }
 static char *tmp_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? c->tmp64 : c->tmp32; }
 
 // out_p = [post] ( [A] y + coef * D_{p,1-p} in ), optional |out|^2 -> norm_out
 static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, const void *in, void *out, const void *y, int clov_on_y,
                           double coef, int post_inv, double *norm_out, int norm_accumulate, const int *skip = nullptr)
 {
+    if ((int)prec < 0 || (int)prec > (int)COLA_F32_H16) return fail(c, COLA_EINVAL, "unknown cola_prec");
     DslashArgs a;
     memset(&a, 0, sizeof(a));
     a.g = c->g;
@@ -316,8 +327,8 @@ static cola_status gauge_finish(cola_ctx *c)
     memcpy(&c->max_unitarity_dev, &bits, sizeof(double));
     if (c->p.compress12 && !(c->max_unitarity_dev <= 1e-10))
         return fail(c, COLA_EINVAL, "cola_gauge_upload: links are not unitary to 1e-10; 12-real compression would be wrong");
-    CK(launch_clover_build(c->g, c->gauge64, c->p.kappa * c->p.csw, c->p.trace_sub, c->clovA64, c->clovA32, c->stream));
-    CK(launch_clover_invert(c->g, c->clovA64 + 576 * c->Vh, c->clovI64, c->clovI32, c->stream));
+    CK(launch_clover_build(c->g, c->gauge64, c->p.kappa * c->p.csw, c->p.trace_sub, c->clovA64, c->clovA32, c->clovA16, c->stream));
+    CK(launch_clover_invert(c->g, c->clovA64 + 576 * c->Vh, c->clovI64, c->clovI32, c->clovI16, c->stream));
     c->launches += 2;
     CK(cudaStreamSynchronize(c->stream));
     c->ready = 1;
@@ -333,7 +344,7 @@ static cola_status gauge_upload_impl(cola_ctx *c, const double *links, int on_ho
     c->ready = 0;
     CK(cudaMemsetAsync(c->max_dev_bits, 0, sizeof(unsigned long long), c->stream));
     if (!on_host) {
-        CK(launch_gauge_reorder(c->g, links, 0, (long)c->V, c->gauge64, c->gauge32, c->fmt32, c->max_dev_bits, c->stream));
+        CK(launch_gauge_reorder(c->g, links, 0, (long)c->V, c->gauge64, c->gauge32, c->fmt32, c->gauge16, c->max_dev_bits, c->stream));
         c->launches++;
         return gauge_finish(c);
     }
@@ -343,7 +354,7 @@ static cola_status gauge_upload_impl(cola_ctx *c, const double *links, int on_ho
     for (size_t lo = 0; lo < c->V; lo += chunk_sites) {
         const size_t n = (c->V - lo < chunk_sites) ? c->V - lo : chunk_sites;
         CK(cudaMemcpyAsync(c->scratch, links + lo * 72, n * per_site, cudaMemcpyHostToDevice, c->stream));
-        CK(launch_gauge_reorder(c->g, (const double *)c->scratch, (long)lo, (long)n, c->gauge64, c->gauge32, c->fmt32, c->max_dev_bits, c->stream));
+        CK(launch_gauge_reorder(c->g, (const double *)c->scratch, (long)lo, (long)n, c->gauge64, c->gauge32, c->fmt32, c->gauge16, c->max_dev_bits, c->stream));
         c->launches++;
     }
     return gauge_finish(c);
@@ -361,7 +372,9 @@ struct System {            // K x = rhs on n_sites sites; K = S (even_odd) or M
 
 cola_status apply_K(cola_ctx *c, const System &sy, cola_prec prec, int dagger, const void *in, void *out, double *norm_out, const int *skip = nullptr)
 {
-    return sy.even_odd ? schur(c, prec, dagger, in, out, norm_out, skip) : fmatrix(c, prec, dagger, in, out, norm_out, skip);
+    // the inner fp32 iteration of a mixed = 2 solve reads the 16-bit links and clover (same fp32 vectors)
+    const cola_prec op = (prec == COLA_F32 && c->sloppy16) ? COLA_F32_H16 : prec;
+    return sy.even_odd ? schur(c, op, dagger, in, out, norm_out, skip) : fmatrix(c, op, dagger, in, out, norm_out, skip);
 }
 
 // (re)arm the device-side decision state: rmax2, target2, delta2, flag = 0, iters
@@ -445,6 +458,8 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve: tol must be > 0 and max_iter >= 1");
     CK(cudaSetDevice(c->p.device));
     memset(info, 0, sizeof(*info));
+    if (sp->mixed < 0 || sp->mixed > 2) return fail(c, COLA_EINVAL, "cola_cg_solve: mixed must be 0, 1 or 2");
+    c->sloppy16 = sp->mixed == 2;
     const double delta = sp->delta > 0 ? sp->delta : 0.1;
     const double kappa = c->p.kappa;
     const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32);
@@ -658,6 +673,7 @@ cola_status dslash_m(cola_ctx *c, cola_prec prec, int parity, int dagger, const 
                      size_t out_stride, const void *y, size_t y_stride, int clov_on_y, double coef, int post_inv, double *norm_out, int norm_accumulate,
                      const int *skip)
 {
+    if ((int)prec < 0 || (int)prec > (int)COLA_F32_H16) return fail(c, COLA_EINVAL, "unknown cola_prec");
     MrhsArgs m;
     memset(&m, 0, sizeof(m));
     DslashArgs &a = m.d;
@@ -733,7 +749,7 @@ cola_status first_half_m(cola_ctx *c, int k, const MrhsList &A, int na)
     CtlM *cm = c->ctlm;
     const size_t h32 = half_bytes(c, COLA_F32);
     const int nb = blas_mrhs_blocks(c->Vh, COLA_F32);
-    ST(schur_m(c, COLA_F32, 0, A, na, c->m_p32, h32, c->m_tmp32, c->m_q32, h32, cm->qq, &cm->flag));
+    ST(schur_m(c, c->sloppy16 ? COLA_F32_H16 : COLA_F32, 0, A, na, c->m_p32, h32, c->m_tmp32, c->m_q32, h32, cm->qq, &cm->flag));
     CK(launch_r_update_mrhs(COLA_F32, c->m_r32, c->m_q32, h32, cm, k & 1, A, na, &cm->flag, c->Vh, c->m_partials, c->stream));
     CK(launch_mrhs_reduce(c->m_partials, nb, na, A.v, cm->rr, 0, &cm->flag, c->stream));
     CK(launch_decide_mrhs(cm, A, na, k + 1, &cm->flag, c->d_statusm + (k & 1), c->stream));
@@ -746,7 +762,7 @@ cola_status second_half_m(cola_ctx *c, int k, int do_x, const MrhsList &A, int n
 {
     CtlM *cm = c->ctlm;
     const size_t h32 = half_bytes(c, COLA_F32);
-    ST(schur_m(c, COLA_F32, 1, A, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[(k & 1) ^ 1], &cm->flag));
+    ST(schur_m(c, c->sloppy16 ? COLA_F32_H16 : COLA_F32, 1, A, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[(k & 1) ^ 1], &cm->flag));
     CK(launch_xp_update_mrhs(COLA_F32, c->m_x32, c->m_p32, c->m_q32, h32, cm, k & 1, A, na, do_x, 1, &cm->flag, c->Vh, c->stream));
     c->launches++;
     return COLA_OK;
@@ -766,7 +782,9 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
     ST(need_mrhs(c, "cola_cg_solve_mrhs", nrhs));
     if (!sp || !b_canon_dev || !x_canon_dev || !infos) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: NULL argument");
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: tol must be > 0 and max_iter >= 1");
-    if (!sp->even_odd || !sp->mixed) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd solver is batched (even_odd = 1, mixed = 1)");
+    if (!sp->even_odd || sp->mixed < 1 || sp->mixed > 2)
+        return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd solver is batched (even_odd = 1, mixed = 1 or 2)");
+    c->sloppy16 = sp->mixed == 2;
     CK(cudaSetDevice(c->p.device));
     const double delta = sp->delta > 0 ? sp->delta : 0.1, kappa = c->p.kappa;
     const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32), f64 = 2 * h64;
@@ -820,7 +838,7 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
         st.delta2 = delta * delta;
         CK(cudaMemcpyAsync(cm, &st, sizeof(st), cudaMemcpyHostToDevice, c->stream));
         MrhsList L = list_of(A, na);
-        ST(schur_m(c, COLA_F32, 1, L, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[0], nullptr));    // s0 = S^+ r0, gamma_0
+        ST(schur_m(c, c->sloppy16 ? COLA_F32_H16 : COLA_F32, 1, L, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[0], nullptr));    // s0 = S^+ r0, gamma_0
         CK(cudaMemcpyAsync(c->m_p32, c->m_q32, (size_t)nrhs * h32, cudaMemcpyDeviceToDevice, c->stream));
         for (int j = 0; j < na; j++) flops[A[j]] += flops_K;
         c->h_statusm[0].iters = c->h_statusm[1].iters = 0;

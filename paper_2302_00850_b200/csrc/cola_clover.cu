@@ -144,9 +144,23 @@ __device__ __forceinline__ void pack_block(const double (&br)[36], const double 
         }
 }
 
-__device__ __forceinline__ void store_block(char *c64, char *c32, size_t Vh, int blk, size_t i, const double (&p)[36])
+__device__ __forceinline__ unsigned pack_h16(double a, double b)
+{
+    const __half2 h = __floats2half2_rn((float)a, (float)b);
+    return *reinterpret_cast<const unsigned *>(&h);
+}
+
+__device__ __forceinline__ void store_block(char *c64, char *c32, char *c16, size_t Vh, int blk, size_t i, const double (&p)[36])
 {
     store_reals<double, 36>(reinterpret_cast<double2 *>(c64) + (size_t)blk * 18 * Vh, Vh, i, p);
+    if (c16) {   // fp16 copy: per block 4 chunks of 8 halfs + 1 chunk of 4 halfs (clover_apply<.., H16> in cola_device.cuh)
+        char *base = c16 + (size_t)blk * 72 * Vh;
+#pragma unroll
+        for (int k = 0; k < 4; k++)
+            reinterpret_cast<uint4 *>(base + (size_t)k * 16 * Vh)[i] =
+                make_uint4(pack_h16(p[8 * k], p[8 * k + 1]), pack_h16(p[8 * k + 2], p[8 * k + 3]), pack_h16(p[8 * k + 4], p[8 * k + 5]), pack_h16(p[8 * k + 6], p[8 * k + 7]));
+        reinterpret_cast<uint2 *>(base + (size_t)64 * Vh)[i] = make_uint2(pack_h16(p[32], p[33]), pack_h16(p[34], p[35]));
+    }
     if (c32) {
         float f[36];
 #pragma unroll
@@ -156,7 +170,7 @@ __device__ __forceinline__ void store_block(char *c64, char *c32, size_t Vh, int
 }
 
 // one thread per site: tid < 2*Vh, parity = tid / Vh
-__global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *gauge64, double k, int trace_sub, char *A64, char *A32)
+__global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *gauge64, double k, int trace_sub, char *A64, char *A32, char *A16)
 {
     const long tid = (long)blockIdx.x * CB + threadIdx.x;
     if (tid >= 2L * g.Vh) return;
@@ -182,6 +196,7 @@ __global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *ga
     const size_t Vh = g.Vh;
     char *a64 = A64 + (size_t)parity * 72 * 8 * Vh;
     char *a32 = A32 ? A32 + (size_t)parity * 72 * 4 * Vh : nullptr;
+    char *a16 = A16 ? A16 + (size_t)parity * CLOVER_H16_BYTES * Vh : nullptr;
 #pragma unroll
     for (int blk = 0; blk < 2; blk++) {
         const double sg = blk == 0 ? 1.0 : -1.0;
@@ -207,12 +222,12 @@ __global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *ga
             }
         double p[36];
         pack_block(br, bi, p);
-        store_block(a64, a32, Vh, blk, i, p);
+        store_block(a64, a32, a16, Vh, blk, i, p);
     }
 }
 
 // one thread per (site, block) of one parity: tid < 2*Vh, blk = tid / Vh
-__global__ void __launch_bounds__(CB) clover_invert_kernel(Geom g, const char *A64, char *I64, char *I32)
+__global__ void __launch_bounds__(CB) clover_invert_kernel(Geom g, const char *A64, char *I64, char *I32, char *I16)
 {
     const long tid = (long)blockIdx.x * CB + threadIdx.x;
     if (tid >= 2L * g.Vh) return;
@@ -258,7 +273,7 @@ __global__ void __launch_bounds__(CB) clover_invert_kernel(Geom g, const char *A
     }
     double q[36];
     pack_block(ar, ai, q);
-    store_block(I64, I32, Vh, blk, i, q);
+    store_block(I64, I32, I16, Vh, blk, i, q);
 }
 
 // expand packed blocks to canonical 12x12 complex per lex site; parity_mask bit p set => parity p is
@@ -301,17 +316,17 @@ __global__ void __launch_bounds__(CB) clover_unpack_kernel(Geom g, const char *c
 
 }  // namespace
 
-cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, cudaStream_t s)
+cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, void *clovA16, cudaStream_t s)
 {
     const long n = 2L * g.Vh;
-    clover_build_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)gauge64, kappa_csw, trace_sub, (char *)clovA64, (char *)clovA32);
+    clover_build_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)gauge64, kappa_csw, trace_sub, (char *)clovA64, (char *)clovA32, (char *)clovA16);
     return cudaGetLastError();
 }
 
-cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, cudaStream_t s)
+cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, void *clovI16, cudaStream_t s)
 {
     const long n = 2L * g.Vh;
-    clover_invert_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)clovA64_odd, (char *)clovI64, (char *)clovI32);
+    clover_invert_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)clovA64_odd, (char *)clovI64, (char *)clovI32, (char *)clovI16);
     return cudaGetLastError();
 }
 

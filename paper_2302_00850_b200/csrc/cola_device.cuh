@@ -2,6 +2,8 @@
 // in-register third-row reconstruction (BJ:ns), packed 6x6 Hermitian clover mat-vec,
 // deterministic warp-shuffle + block + last-block reduction.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "cola_internal.h"
 
 namespace cola {
@@ -34,6 +36,18 @@ __device__ __forceinline__ double2 ld_stream(const double2 *p)
 {
     double2 r;
     asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ uint4 ld_stream(const uint4 *p)
+{
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ uint2 ld_stream(const uint2 *p)
+{
+    uint2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
     return r;
 }
 __device__ __forceinline__ float4 ld_cached(const float4 *p) { return __ldg(p); }
@@ -94,6 +108,21 @@ template <int FMT> struct LinkT;
 template <> struct LinkT<LINK_F64_18> { typedef double T; };
 template <> struct LinkT<LINK_F32_18> { typedef float T; };
 template <> struct LinkT<LINK_F32_12> { typedef float T; };
+template <> struct LinkT<LINK_I16_12> { typedef float T; };
+
+// two 16-bit fixed-point reals (x 32767) of one 32-bit word
+__device__ __forceinline__ void unpack_i16(unsigned w, float &a, float &b)
+{
+    constexpr float inv = 1.0f / 32767.0f;
+    a = (float)(short)(w & 0xffffu) * inv;
+    b = (float)(short)(w >> 16) * inv;
+}
+__device__ __forceinline__ void unpack_h16(unsigned w, float &a, float &b)
+{
+    const float2 f = __half22float2(*reinterpret_cast<const __half2 *>(&w));
+    a = f.x;
+    b = f.y;
+}
 
 // base = start of the [chunk][Vh] block of one (parity, mu)
 // STREAM: read-once data, no L1 allocation (single right-hand side); !STREAM: the same link is read by the
@@ -103,6 +132,18 @@ __device__ __forceinline__ void load_link(const char *base, size_t Vh, size_t i,
 {
     if constexpr (FMT == LINK_F64_18) {
         load_reals<double, 18, STREAM>(base, Vh, i, u);
+    } else if constexpr (FMT == LINK_I16_12) {
+        const uint4 *pa = reinterpret_cast<const uint4 *>(base) + i;
+        const uint2 *pb = reinterpret_cast<const uint2 *>(base + 16 * Vh) + i;
+        const uint4 a = STREAM ? ld_stream(pa) : __ldg(pa);
+        const uint2 b = STREAM ? ld_stream(pb) : __ldg(pb);
+        unpack_i16(a.x, u[0], u[1]);
+        unpack_i16(a.y, u[2], u[3]);
+        unpack_i16(a.z, u[4], u[5]);
+        unpack_i16(a.w, u[6], u[7]);
+        unpack_i16(b.x, u[8], u[9]);
+        unpack_i16(b.y, u[10], u[11]);
+        reconstruct_row3(u);
     } else if constexpr (FMT == LINK_F32_12) {
         float r[12];
         load_reals<float, 12, STREAM>(base, Vh, i, r);
@@ -149,7 +190,8 @@ __device__ __forceinline__ void clover_block_mul(const T *c, const T *v, T *w)
 }
 
 // w = C(site i) v on the full 24-real spinor; clov = [72/N chunks][Vh]
-template <typename T, bool STREAM = true>
+// H16: the field is stored in fp16, per block 4 chunks of 8 halfs + 1 chunk of 4 halfs (72 bytes), [block][chunk][Vh]
+template <typename T, bool STREAM = true, bool H16 = false>
 __device__ __forceinline__ void clover_apply(const void *clov, size_t Vh, size_t i, const T (&v)[24], T (&w)[24])
 {
     typedef typename VT<T>::V V;
@@ -157,7 +199,24 @@ __device__ __forceinline__ void clover_apply(const void *clov, size_t Vh, size_t
 #pragma unroll
     for (int b = 0; b < 2; b++) {
         T c[36];
-        load_reals<T, 36, STREAM>(reinterpret_cast<const V *>(clov) + (size_t)b * (36 / N) * Vh, Vh, i, c);
+        if constexpr (H16) {
+            const char *base = reinterpret_cast<const char *>(clov) + (size_t)b * 72 * Vh;
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                const uint4 *p = reinterpret_cast<const uint4 *>(base + (size_t)k * 16 * Vh) + i;
+                const uint4 q = STREAM ? ld_stream(p) : __ldg(p);
+                unpack_h16(q.x, c[8 * k], c[8 * k + 1]);
+                unpack_h16(q.y, c[8 * k + 2], c[8 * k + 3]);
+                unpack_h16(q.z, c[8 * k + 4], c[8 * k + 5]);
+                unpack_h16(q.w, c[8 * k + 6], c[8 * k + 7]);
+            }
+            const uint2 *p2 = reinterpret_cast<const uint2 *>(base + (size_t)64 * Vh) + i;
+            const uint2 q2 = STREAM ? ld_stream(p2) : __ldg(p2);
+            unpack_h16(q2.x, c[32], c[33]);
+            unpack_h16(q2.y, c[34], c[35]);
+        } else {
+            load_reals<T, 36, STREAM>(reinterpret_cast<const V *>(clov) + (size_t)b * (36 / N) * Vh, Vh, i, c);
+        }
         clover_block_mul(c, &v[12 * b], &w[12 * b]);
     }
 }

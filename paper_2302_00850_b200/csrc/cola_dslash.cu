@@ -198,7 +198,7 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
             const T cf = (T)a.coef;
             if (XPAY == 2) {
                 T cy[24];
-                clover_apply<T, STREAM>(a.clov_y, Vh, i, yv, cy);
+                clover_apply<T, STREAM, FMT == LINK_I16_12>(a.clov_y, Vh, i, yv, cy);
 #pragma unroll
                 for (int k = 0; k < 24; k++) acc[k] = cy[k] + cf * acc[k];
             } else {
@@ -208,7 +208,7 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
         }
         if (POST != 0) {
             T w[24];
-            clover_apply<T, STREAM>(a.clov_post, Vh, i, acc, w);
+            clover_apply<T, STREAM, FMT == LINK_I16_12>(a.clov_post, Vh, i, acc, w);
 #pragma unroll
             for (int k = 0; k < 24; k++) acc[k] = w[k];
         }
@@ -401,6 +401,7 @@ cudaError_t launch_dslash_mrhs(int fmt, MrhsArgs &m, cudaStream_t s)
         case LINK_F64_18: return launch_mrhs_fmt<LINK_F64_18>(m, s);
         case LINK_F32_18: return launch_mrhs_fmt<LINK_F32_18>(m, s);
         case LINK_F32_12: return launch_mrhs_fmt<LINK_F32_12>(m, s);
+        case LINK_I16_12: return launch_mrhs_fmt<LINK_I16_12>(m, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -422,6 +423,7 @@ cudaError_t launch_dslash(int fmt, const DslashArgs &a, cudaStream_t s)
         case LINK_F64_18: return launch_fmt<LINK_F64_18>(a, s);
         case LINK_F32_18: return launch_fmt<LINK_F32_18>(a, s);
         case LINK_F32_12: return launch_fmt<LINK_F32_12>(a, s);
+        case LINK_I16_12: return launch_fmt<LINK_I16_12>(a, s);
     }
     return cudaErrorInvalidValue;
 }

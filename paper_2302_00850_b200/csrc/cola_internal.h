@@ -40,8 +40,11 @@ struct Geom {
 };
 
 // Bytes of one link per site in each storage format.
-enum LinkFmt { LINK_F64_18 = 0, LINK_F32_18 = 1, LINK_F32_12 = 2 };
-__host__ __device__ inline size_t link_bytes(int fmt) { return fmt == LINK_F64_18 ? 144 : (fmt == LINK_F32_18 ? 72 : 48); }
+// LINK_I16_12: rows 1 and 2 as 16-bit fixed point (x 32767), 24 bytes per link = one 16-byte and
+// one 8-byte chunk; it comes with the fp16 clover field (CLOVER_H16_BYTES per site) and fp32 spinors and arithmetic.
+enum LinkFmt { LINK_F64_18 = 0, LINK_F32_18 = 1, LINK_F32_12 = 2, LINK_I16_12 = 3 };
+__host__ __device__ inline size_t link_bytes(int fmt) { return fmt == LINK_F64_18 ? 144 : (fmt == LINK_F32_18 ? 72 : (fmt == LINK_F32_12 ? 48 : 24)); }
+constexpr size_t CLOVER_H16_BYTES = 144;   // 2 blocks x (4 x 16 B + 1 x 8 B) = 72 halfs
 
 // Device-resident scalars of the CG recurrence (all reductions land here; alpha and beta are
 // formed inside the consuming kernels, so the host only ever reads `rr`).
@@ -168,12 +171,12 @@ cudaError_t launch_clover_apply(cola_prec prec, const Geom &g, const void *clov,
 
 // layout / setup kernels (cola_layout.cu, cola_clover.cu)
 cudaError_t launch_gauge_reorder(const Geom &g, const double *canon_dev, long site_lo, long n_sites, void *gauge64, void *gauge32,
-                                 int fmt32, unsigned long long *max_dev_bits, cudaStream_t s);
+                                 int fmt32, void *gauge16, unsigned long long *max_dev_bits, cudaStream_t s);
 cudaError_t launch_spinor_pack(cola_prec prec, const Geom &g, const void *canon, void *internal, cudaStream_t s);
 cudaError_t launch_spinor_unpack(cola_prec prec, const Geom &g, const void *internal, void *canon, cudaStream_t s);
 cudaError_t launch_spinor_convert(cola_prec dst_prec, const void *src, void *dst, size_t n_sites, cudaStream_t s);
-cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, cudaStream_t s);
-cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, cudaStream_t s);
+cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, void *clovA16, cudaStream_t s);
+cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, void *clovI16, cudaStream_t s);
 cudaError_t launch_clover_unpack(const Geom &g, const void *clov64, int parity_mask, void *canon, cudaStream_t s);
 
 // fused BLAS-1 (cola_blas.cu).  n = number of sites of the vectors (Vh or V).

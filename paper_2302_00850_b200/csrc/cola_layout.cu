@@ -22,7 +22,7 @@ __device__ __forceinline__ void lex_to_cb(const Geom &g, long lex, int &parity, 
 
 // one thread per (lex site, mu) of the staged canonical chunk
 __global__ void __launch_bounds__(LB) gauge_reorder_kernel(Geom g, const double *canon, long site_lo, long n_sites, char *gauge64,
-                                                           char *gauge32, int fmt32, unsigned long long *max_dev_bits)
+                                                           char *gauge32, int fmt32, char *gauge16, unsigned long long *max_dev_bits)
 {
     const long tid = (long)blockIdx.x * LB + threadIdx.x;
     double dev = 0.0;
@@ -49,6 +49,18 @@ __global__ void __launch_bounds__(LB) gauge_reorder_kernel(Geom g, const double 
             for (int k = 0; k < 16; k++) f[k] = (float)u[k];
             store_reals<float, 16>(b32, Vh, cb, f);
             reinterpret_cast<float2 *>(b32 + 64 * Vh)[cb] = make_float2((float)u[16], (float)u[17]);
+        }
+        if (gauge16) {   // rows 1, 2 as 16-bit fixed point: round(u * 32767), |u| <= 1 for a unitary matrix (clamped otherwise)
+            char *b16 = gauge16 + (size_t)(parity * 4 + mu) * link_bytes(LINK_I16_12) * Vh;
+            unsigned w[6];
+#pragma unroll
+            for (int k = 0; k < 6; k++) {
+                const int lo = __double2int_rn(fmin(fmax(u[2 * k], -1.0), 1.0) * 32767.0);
+                const int hi = __double2int_rn(fmin(fmax(u[2 * k + 1], -1.0), 1.0) * 32767.0);
+                w[k] = ((unsigned)lo & 0xffffu) | ((unsigned)hi << 16);
+            }
+            reinterpret_cast<uint4 *>(b16)[cb] = make_uint4(w[0], w[1], w[2], w[3]);
+            reinterpret_cast<uint2 *>(b16 + 16 * Vh)[cb] = make_uint2(w[4], w[5]);
         }
         // max |U U^+ - 1| (entry-wise)
 #pragma unroll
@@ -114,11 +126,11 @@ __global__ void __launch_bounds__(LB) convert_kernel(const void *src, void *dst,
 }  // namespace
 
 cudaError_t launch_gauge_reorder(const Geom &g, const double *canon_dev, long site_lo, long n_sites, void *gauge64, void *gauge32,
-                                 int fmt32, unsigned long long *max_dev_bits, cudaStream_t s)
+                                 int fmt32, void *gauge16, unsigned long long *max_dev_bits, cudaStream_t s)
 {
     const long n = 4 * n_sites;
     gauge_reorder_kernel<<<(unsigned)((n + LB - 1) / LB), LB, 0, s>>>(g, canon_dev, site_lo, n_sites, (char *)gauge64, (char *)gauge32,
-                                                                     fmt32, max_dev_bits);
+                                                                     fmt32, (char *)gauge16, max_dev_bits);
     return cudaGetLastError();
 }
 
