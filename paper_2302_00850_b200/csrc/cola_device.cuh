@@ -124,42 +124,66 @@ __device__ __forceinline__ void unpack_h16(unsigned w, float &a, float &b)
     b = f.y;
 }
 
+// A link as it sits in memory (raw) and its expansion to the 18 reals of the 3x3 matrix.  Split in two so that the
+// load of the NEXT hop's link can be issued while the current hop is still computing (software pipelining): the raw
+// words are all that has to stay live.
+template <int FMT> struct RawLink;
+template <> struct RawLink<LINK_F64_18> { double r[18]; };
+template <> struct RawLink<LINK_F32_18> { float r[18]; };
+template <> struct RawLink<LINK_F32_12> { float r[12]; };
+template <> struct RawLink<LINK_I16_12> { unsigned w[6]; };
+
 // base = start of the [chunk][Vh] block of one (parity, mu)
 // STREAM: read-once data, no L1 allocation (single right-hand side); !STREAM: the same link is read by the
 // threads of several right-hand sides of one block, so it is kept in L1.
 template <int FMT, bool STREAM = true>
-__device__ __forceinline__ void load_link(const char *base, size_t Vh, size_t i, typename LinkT<FMT>::T (&u)[18])
+__device__ __forceinline__ void load_raw_link(const char *base, size_t Vh, size_t i, RawLink<FMT> &raw)
 {
     if constexpr (FMT == LINK_F64_18) {
-        load_reals<double, 18, STREAM>(base, Vh, i, u);
+        load_reals<double, 18, STREAM>(base, Vh, i, raw.r);
     } else if constexpr (FMT == LINK_I16_12) {
         const uint4 *pa = reinterpret_cast<const uint4 *>(base) + i;
         const uint2 *pb = reinterpret_cast<const uint2 *>(base + 16 * Vh) + i;
         const uint4 a = STREAM ? ld_stream(pa) : __ldg(pa);
         const uint2 b = STREAM ? ld_stream(pb) : __ldg(pb);
-        unpack_i16(a.x, u[0], u[1]);
-        unpack_i16(a.y, u[2], u[3]);
-        unpack_i16(a.z, u[4], u[5]);
-        unpack_i16(a.w, u[6], u[7]);
-        unpack_i16(b.x, u[8], u[9]);
-        unpack_i16(b.y, u[10], u[11]);
-        reconstruct_row3(u);
+        raw.w[0] = a.x; raw.w[1] = a.y; raw.w[2] = a.z; raw.w[3] = a.w; raw.w[4] = b.x; raw.w[5] = b.y;
     } else if constexpr (FMT == LINK_F32_12) {
-        float r[12];
-        load_reals<float, 12, STREAM>(base, Vh, i, r);
-#pragma unroll
-        for (int k = 0; k < 12; k++) u[k] = r[k];
-        reconstruct_row3(u);
+        load_reals<float, 12, STREAM>(base, Vh, i, raw.r);
     } else {
         float r[16];
         load_reals<float, 16, STREAM>(base, Vh, i, r);
 #pragma unroll
-        for (int k = 0; k < 16; k++) u[k] = r[k];
+        for (int k = 0; k < 16; k++) raw.r[k] = r[k];
         const float2 *tp = reinterpret_cast<const float2 *>(base + 64 * Vh) + i;
         float2 t = STREAM ? ld_stream(tp) : __ldg(tp);
-        u[16] = t.x;
-        u[17] = t.y;
+        raw.r[16] = t.x;
+        raw.r[17] = t.y;
     }
+}
+
+template <int FMT>
+__device__ __forceinline__ void expand_link(const RawLink<FMT> &raw, typename LinkT<FMT>::T (&u)[18])
+{
+    if constexpr (FMT == LINK_F64_18 || FMT == LINK_F32_18) {
+#pragma unroll
+        for (int k = 0; k < 18; k++) u[k] = raw.r[k];
+    } else if constexpr (FMT == LINK_I16_12) {
+#pragma unroll
+        for (int k = 0; k < 6; k++) unpack_i16(raw.w[k], u[2 * k], u[2 * k + 1]);
+        reconstruct_row3(u);
+    } else {
+#pragma unroll
+        for (int k = 0; k < 12; k++) u[k] = raw.r[k];
+        reconstruct_row3(u);
+    }
+}
+
+template <int FMT, bool STREAM = true>
+__device__ __forceinline__ void load_link(const char *base, size_t Vh, size_t i, typename LinkT<FMT>::T (&u)[18])
+{
+    RawLink<FMT> raw;
+    load_raw_link<FMT, STREAM>(base, Vh, i, raw);
+    expand_link<FMT>(raw, u);
 }
 
 // ---- packed clover: per site 2 chiral blocks x (6 real diagonal + 15 complex strictly-lower entries,

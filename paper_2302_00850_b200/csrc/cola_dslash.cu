@@ -16,18 +16,22 @@ namespace cola {
 
 namespace {
 
-// Tuning knobs (compile-time).  Defaults = best of the round-1 sweep on B200: 64 threads
-// per block; fp32 kernels capped at 80 registers (12 blocks = 24 warps per SM), fp64 kernels at 168 registers
-// (6 blocks = 12 warps per SM).  The kernels are bound by bytes in flight: fewer registers than this spill, more
-// registers cost occupancy, and both lose bandwidth.
+// Tuning knobs (compile-time).  Defaults = best of the round-1 sweeps on B200: 64 threads per
+// block; fp32 kernels software-pipelined over the hops (COLA_PIPE) with 128 registers (8 blocks = 16 warps per SM);
+// fp64 kernels unpipelined at 168 registers (6 blocks = 12 warps per SM).  Without pipelining the best fp32 point was
+// 80 registers (12 blocks): the kernels are bound by bytes in flight, which either more warps or loads issued one hop
+// ahead provide; one hop ahead at 16 warps beats 24 warps without by 4-8 %.
 #ifndef COLA_DSLASH_BLOCK
 #define COLA_DSLASH_BLOCK 64
 #endif
 #ifndef COLA_DSLASH_MINB_F32
-#define COLA_DSLASH_MINB_F32 12
+#define COLA_DSLASH_MINB_F32 8
 #endif
 #ifndef COLA_DSLASH_MINB_F64
 #define COLA_DSLASH_MINB_F64 6
+#endif
+#ifndef COLA_PIPE
+#define COLA_PIPE 1
 #endif
 constexpr int DSLASH_BLOCK = COLA_DSLASH_BLOCK;
 template <int FMT> struct MinBlocks { static constexpr int value = (FMT == LINK_F64_18) ? COLA_DSLASH_MINB_F64 : COLA_DSLASH_MINB_F32; };
@@ -140,6 +144,25 @@ __device__ __forceinline__ void hop(const void *in, const char *gauge_mu, size_t
     reconstruct_accumulate<MU>(g, eta, s, acc);
 }
 
+// Hop H = 2*MU + BACK of the pipelined sequence: consumes (psi, raw) of hop H, then refills them with hop H+1's
+// neighbour spinor `nb_next` and link `li_next` of `gauge_next` (nullptr: last hop).
+template <int FMT, int H, bool STREAM, typename T>
+__device__ __forceinline__ void hop_pipe(const void *in, const char *gauge_next, size_t Vh, int nb_next, int li_next, T (&psi)[24], RawLink<FMT> &raw,
+                                         T eta, T s, T (&acc)[24])
+{
+    constexpr int MU = H >> 1;
+    constexpr bool BACK = (H & 1) != 0;
+    T h[12], g[12], u[18];
+    project<MU>(psi, s, h);
+    expand_link<FMT>(raw, u);
+    if (H < 7) {
+        load_reals<T, 24, false>(in, Vh, nb_next, psi);
+        load_raw_link<FMT, STREAM>(gauge_next, Vh, li_next, raw);
+    }
+    su3_mul<BACK>(u, h, g);
+    reconstruct_accumulate<MU>(g, eta, s, acc);
+}
+
 // One output site i of parity a.parity:  v = D in;  v = [A] y + coef v (XPAY);  v = Cpost v (POST);  out = v.
 // Returns |v|^2 if want_norm.  XPAY: 0 none, 1 v = y + coef v, 2 v = A y + coef v.   POST: 0 none, 1 v = Cpost v.
 // STREAM: links and clover are read once (no L1 allocation); !STREAM: they are shared by the right-hand sides of a block.
@@ -183,6 +206,26 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
 #pragma unroll
         for (int k = 0; k < 24; k++) acc[k] = 0;
 
+#if COLA_PIPE
+        if constexpr (FMT != LINK_F64_18) {
+            // software-pipelined hops: the loads of hop h+1 (neighbour spinor and raw link) are issued right after the
+            // projection of hop h, whose spinor registers are dead by then, so they are in flight during the SU(3)
+            // multiply and the accumulation of hop h
+            T psi[24];
+            RawLink<FMT> raw;
+            load_reals<T, 24, false>(in, Vh, xf, psi);
+            load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, raw);
+            hop_pipe<FMT, 0, STREAM>(in, gq + 0 * lb, Vh, xb, xb, psi, raw, ex_f, sf, acc);
+            hop_pipe<FMT, 1, STREAM>(in, gp + 1 * lb, Vh, yf, i, psi, raw, ex_b, sb, acc);
+            hop_pipe<FMT, 2, STREAM>(in, gq + 1 * lb, Vh, yb, yb, psi, raw, ey_f, sf, acc);
+            hop_pipe<FMT, 3, STREAM>(in, gp + 2 * lb, Vh, zf, i, psi, raw, ey_b, sb, acc);
+            hop_pipe<FMT, 4, STREAM>(in, gq + 2 * lb, Vh, zb, zb, psi, raw, ez_f, sf, acc);
+            hop_pipe<FMT, 5, STREAM>(in, gp + 3 * lb, Vh, tf, i, psi, raw, ez_b, sb, acc);
+            hop_pipe<FMT, 6, STREAM>(in, gq + 3 * lb, Vh, tb, tb, psi, raw, et_f, sf, acc);
+            hop_pipe<FMT, 7, STREAM>(in, nullptr, Vh, 0, 0, psi, raw, et_b, sb, acc);
+        } else
+#endif
+        {
         hop<FMT, 0, false, STREAM>(in, gp + 0 * lb, Vh, xf, i, ex_f, sf, acc);
         hop<FMT, 0, true, STREAM>(in, gq + 0 * lb, Vh, xb, xb, ex_b, sb, acc);
         hop<FMT, 1, false, STREAM>(in, gp + 1 * lb, Vh, yf, i, ey_f, sf, acc);
@@ -191,6 +234,7 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
         hop<FMT, 2, true, STREAM>(in, gq + 2 * lb, Vh, zb, zb, ez_b, sb, acc);
         hop<FMT, 3, false, STREAM>(in, gp + 3 * lb, Vh, tf, i, et_f, sf, acc);
         hop<FMT, 3, true, STREAM>(in, gq + 3 * lb, Vh, tb, tb, et_b, sb, acc);
+        }
 
         if (XPAY != 0) {
             T yv[24];
@@ -236,13 +280,16 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
 
 // ---- multi-right-hand-side variant (MrhsArgs in cola_internal.h)
 #ifndef COLA_MRHS_PER_BLOCK_F32
-#define COLA_MRHS_PER_BLOCK_F32 4
+#define COLA_MRHS_PER_BLOCK_F32 2
 #endif
 #ifndef COLA_MRHS_PER_BLOCK_F64
 #define COLA_MRHS_PER_BLOCK_F64 2
 #endif
-#ifndef COLA_MRHS_MINB
-#define COLA_MRHS_MINB 3
+#ifndef COLA_MRHS_MINB_F32
+#define COLA_MRHS_MINB_F32 4
+#endif
+#ifndef COLA_MRHS_MINB_F64
+#define COLA_MRHS_MINB_F64 3
 #endif
 #ifndef COLA_MRHS_SITES
 #define COLA_MRHS_SITES 64
@@ -251,10 +298,13 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
 #define COLA_MRHS_TILE_X 16
 #endif
 constexpr int MSITES = COLA_MRHS_SITES;
-template <int FMT> struct MrhsCfg { static constexpr int NRB = (FMT == LINK_F64_18) ? COLA_MRHS_PER_BLOCK_F64 : COLA_MRHS_PER_BLOCK_F32; };
+template <int FMT> struct MrhsCfg {
+    static constexpr int NRB = (FMT == LINK_F64_18) ? COLA_MRHS_PER_BLOCK_F64 : COLA_MRHS_PER_BLOCK_F32;
+    static constexpr int MINB = (FMT == LINK_F64_18) ? COLA_MRHS_MINB_F64 : COLA_MRHS_MINB_F32;
+};
 
 template <int FMT, int XPAY, int POST>
-__global__ void __launch_bounds__(MSITES * MrhsCfg<FMT>::NRB, COLA_MRHS_MINB) dslash_mrhs_kernel(const __grid_constant__ MrhsArgs m)
+__global__ void __launch_bounds__(MSITES * MrhsCfg<FMT>::NRB, MrhsCfg<FMT>::MINB) dslash_mrhs_kernel(const __grid_constant__ MrhsArgs m)
 {
     constexpr int NRB = MrhsCfg<FMT>::NRB;
     if (m.d.skip && *m.d.skip) return;
