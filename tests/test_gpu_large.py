@@ -149,3 +149,54 @@ def test_mixed_precision_solve(big):
         x64, info64 = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=False)
         assert info64["converged"] and abs(info64["iters"] - g["iters"]) <= max(1, math.ceil(0.02 * g["iters"]))
         assert rel(x64.cpu().numpy(), xn) < 5e-9
+
+
+def test_16bit_operator_and_solver_at_full_size(big):
+    """COLA_F32_H16 in bench.py's launch configuration: sampled-site operator parity within the
+    storage-error tolerance of tests/test_gpu_h16.py, and the mixed = 2 solve to the same bar as mixed = 1."""
+    c, dims, cfg, k = big.ctx, big.dims, big.cfg, big.k
+    psi = inputs.source_gaussian(dims, 4342 + k, device="cuda")
+    psin = psi.cpu().numpy()
+    internal = c.spinor_pack(psi.to(torch.complex64))
+    args = (dims, inputs.BC, big.Un, cfg["kappa"], cfg["csw"])
+    got = at_sites(c.spinor_unpack(c.fermion_matrix_apply(internal, h16=True)), big.sites)
+    e = rel(got, oracle.apply_sites(*args, "M", psin, big.sites))
+    assert 1e-6 < e < 5e-4, e
+    even = big.sites[big.par == 0]
+    out = torch.zeros_like(internal)
+    c.schur_apply(internal[0], dagger=True, out=out[0], h16=True)
+    assert rel(at_sites(c.spinor_unpack(out), even), oracle.apply_sites(*args, "Sdag", psin, even)) < 5e-4
+    if k == 4:
+        return      # the 64^3x128 solve is covered by test_mixed_precision_solve; keep this test short
+    b = inputs.source_point(dims, 1, 2, device="cuda") if cfg["source"] == "point" else inputs.source_gaussian(dims, inputs.config_seed_source(k), device="cuda")
+    x, info = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=2)
+    assert info["converged"] and info["true_residual"] <= 1.05e-10
+    x1, info1 = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=1)
+    assert abs(info["iters"] - info1["iters"]) <= max(1, math.ceil(0.02 * info1["iters"])), (info["iters"], info1["iters"])
+    assert rel(x.cpu().numpy(), x1.cpu().numpy()) < 5e-9
+    if k == 2:
+        g = json.load(open(GOLD))["2"]["eo"]
+        assert abs(info["iters"] - g["iters"]) <= max(1, math.ceil(0.02 * g["iters"]))
+        xs = x.cpu().numpy().reshape(-1, 12)[np.array(g["sites"])]
+        want = np.array(g["x_re"]) + 1j * np.array(g["x_im"])
+        assert np.linalg.norm(xs - want) / np.linalg.norm(want) < 5e-8
+
+
+def test_multi_rhs_operators_at_full_size(big):
+    """Multi-rhs launches at full size: 3 vectors (a ragged last rhs group), sampled-site parity
+    against the oracle for one of them and bit-identity with the single-rhs kernels for all."""
+    c, dims, cfg, k = big.ctx, big.dims, big.cfg, big.k
+    if k == 4:
+        pytest.skip("at 64^3x128 the single-rhs workspace (125 GB) leaves no room for a multi-rhs workspace on one 180 GB GPU")
+    psis = [inputs.source_gaussian(dims, 4442 + k + n, device="cuda") for n in range(3)]
+    full = torch.stack([c.spinor_pack(p.to(torch.complex64)) for p in psis])
+    out = c.fermion_matrix_apply_mrhs(full)
+    args = (dims, inputs.BC, big.Un, cfg["kappa"], cfg["csw"])
+    got = at_sites(c.spinor_unpack(out[2].contiguous()), big.sites)
+    assert rel(got, oracle.apply_sites(*args, "M", psis[2].cpu().numpy(), big.sites)) < TOL[torch.float32]
+    outs = c.schur_apply_mrhs(full[:, 0].contiguous(), dagger=True)
+    for n in range(3):
+        assert torch.equal(out[n], c.fermion_matrix_apply(full[n].contiguous()))
+        assert torch.equal(outs[n], c.schur_apply(full[n, 0].contiguous(), dagger=True))
+    c.release_mrhs_workspace()
+    torch.cuda.empty_cache()
