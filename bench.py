@@ -428,21 +428,23 @@ def main():
             bs = torch.stack([source(n) for n in range(n_src)])
             xs = torch.empty_like(bs)
             ctx.set_mrhs_workspace(n_src)
-            for _ in range(min(args.warmup, 1)):
-                ctx.cg_solve_mrhs(bs, tol=1e-10, x=xs)
-            torch.cuda.synchronize()
-            e0.record()
-            fl_b = 0.0
-            for _ in range(args.steps):
-                _, infos_b = ctx.cg_solve_mrhs(bs, tol=1e-10, x=xs)
-                fl_b += sum(i["op_flops"] for i in infos_b)
-            e1.record()
-            torch.cuda.synchronize()
-            ms_b = e0.elapsed_time(e1) / args.steps
-            batched = {"ms_per_step": round(ms_b, 3), "GFLOP/s": round(fl_b / args.steps / (ms_b * 1e-3) / 1e9, 1),
-                       "speedup_vs_sequential": round(ms / args.steps / ms_b, 3), "nrhs": n_src,
-                       "iters": [i["iters"] for i in infos_b], "reliable_updates": [i["reliable_updates"] for i in infos_b],
-                       "max_true_residual": max(i["true_residual"] for i in infos_b)}
+            batched = {"nrhs": n_src}
+            for key, mode in (("fp32_inner", 1), ("h16_inner", 2)):
+                for _ in range(min(args.warmup, 1)):
+                    ctx.cg_solve_mrhs(bs, tol=1e-10, x=xs, mixed=mode)
+                torch.cuda.synchronize()
+                e0.record()
+                fl_b = 0.0
+                for _ in range(args.steps):
+                    _, infos_b = ctx.cg_solve_mrhs(bs, tol=1e-10, x=xs, mixed=mode)
+                    fl_b += sum(i["op_flops"] for i in infos_b)
+                e1.record()
+                torch.cuda.synchronize()
+                ms_b = e0.elapsed_time(e1) / args.steps
+                batched[key] = {"ms_per_step": round(ms_b, 3), "GFLOP/s": round(fl_b / args.steps / (ms_b * 1e-3) / 1e9, 1),
+                                "speedup_vs_sequential": round(ms / args.steps / ms_b, 3),
+                                "iters": [i["iters"] for i in infos_b], "reliable_updates": [i["reliable_updates"] for i in infos_b],
+                                "max_true_residual": max(i["true_residual"] for i in infos_b)}
             del bs, xs
         except (RuntimeError, binding.ColaError) as ex:   # e.g. out of memory for 12 systems at once
             batched = {"unavailable": str(ex)[:200]}
