@@ -19,8 +19,8 @@ namespace {
 // Tuning knobs (compile-time).  Defaults = best of the round-1 sweeps on B200: 64 threads per
 // block; fp32 kernels software-pipelined over the hops (COLA_PIPE) with 128 registers (8 blocks = 16 warps per SM);
 // fp64 kernels unpipelined at 168 registers (6 blocks = 12 warps per SM).  Without pipelining the best fp32 point was
-// 80 registers (12 blocks): the kernels are bound by bytes in flight, which either more warps or loads issued one hop
-// ahead provide; one hop ahead at 16 warps beats 24 warps without by 4-8 %.
+// 80 registers (12 blocks): the kernels are bound by bytes in flight, which either more warps or loads issued ahead of
+// use provide; two hops ahead at 16 warps beats 24 warps without by 5-9 % (one hop ahead: 4-8 %).
 #ifndef COLA_DSLASH_BLOCK
 #define COLA_DSLASH_BLOCK 64
 #endif
@@ -31,7 +31,7 @@ namespace {
 #define COLA_DSLASH_MINB_F64 6
 #endif
 #ifndef COLA_PIPE
-#define COLA_PIPE 1
+#define COLA_PIPE 2   // 0: hop by hop; 1: loads one hop ahead; 2: two hops ahead (two spinor/link buffers), +1-2 % over 1
 #endif
 constexpr int DSLASH_BLOCK = COLA_DSLASH_BLOCK;
 template <int FMT> struct MinBlocks { static constexpr int value = (FMT == LINK_F64_18) ? COLA_DSLASH_MINB_F64 : COLA_DSLASH_MINB_F32; };
@@ -146,7 +146,7 @@ __device__ __forceinline__ void hop(const void *in, const char *gauge_mu, size_t
 
 // Hop H = 2*MU + BACK of the pipelined sequence: consumes (psi, raw) of hop H, then refills them with hop H+1's
 // neighbour spinor `nb_next` and link `li_next` of `gauge_next` (nullptr: last hop).
-template <int FMT, int H, bool STREAM, typename T>
+template <int FMT, int H, bool STREAM, int LAST_REFILL = 7, typename T>
 __device__ __forceinline__ void hop_pipe(const void *in, const char *gauge_next, size_t Vh, int nb_next, int li_next, T (&psi)[24], RawLink<FMT> &raw,
                                          T eta, T s, T (&acc)[24])
 {
@@ -155,7 +155,7 @@ __device__ __forceinline__ void hop_pipe(const void *in, const char *gauge_next,
     T h[12], g[12], u[18];
     project<MU>(psi, s, h);
     expand_link<FMT>(raw, u);
-    if (H < 7) {
+    if (H < LAST_REFILL) {
         load_reals<T, 24, false>(in, Vh, nb_next, psi);
         load_raw_link<FMT, STREAM>(gauge_next, Vh, li_next, raw);
     }
@@ -211,6 +211,23 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
             // software-pipelined hops: the loads of hop h+1 (neighbour spinor and raw link) are issued right after the
             // projection of hop h, whose spinor registers are dead by then, so they are in flight during the SU(3)
             // multiply and the accumulation of hop h
+#if COLA_PIPE == 2
+            // two hops ahead: buffers A (even hops) and B (odd hops); hop h refills its buffer with hop h+2
+            T psiA[24], psiB[24];
+            RawLink<FMT> rawA, rawB;
+            load_reals<T, 24, false>(in, Vh, xf, psiA);
+            load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, rawA);
+            load_reals<T, 24, false>(in, Vh, xb, psiB);
+            load_raw_link<FMT, STREAM>(gq + 0 * lb, Vh, xb, rawB);
+            hop_pipe<FMT, 0, STREAM, 6>(in, gp + 1 * lb, Vh, yf, i, psiA, rawA, ex_f, sf, acc);
+            hop_pipe<FMT, 1, STREAM, 6>(in, gq + 1 * lb, Vh, yb, yb, psiB, rawB, ex_b, sb, acc);
+            hop_pipe<FMT, 2, STREAM, 6>(in, gp + 2 * lb, Vh, zf, i, psiA, rawA, ey_f, sf, acc);
+            hop_pipe<FMT, 3, STREAM, 6>(in, gq + 2 * lb, Vh, zb, zb, psiB, rawB, ey_b, sb, acc);
+            hop_pipe<FMT, 4, STREAM, 6>(in, gp + 3 * lb, Vh, tf, i, psiA, rawA, ez_f, sf, acc);
+            hop_pipe<FMT, 5, STREAM, 6>(in, gq + 3 * lb, Vh, tb, tb, psiB, rawB, ez_b, sb, acc);
+            hop_pipe<FMT, 6, STREAM, 6>(in, nullptr, Vh, 0, 0, psiA, rawA, et_f, sf, acc);
+            hop_pipe<FMT, 7, STREAM, 6>(in, nullptr, Vh, 0, 0, psiB, rawB, et_b, sb, acc);
+#else
             T psi[24];
             RawLink<FMT> raw;
             load_reals<T, 24, false>(in, Vh, xf, psi);
@@ -223,6 +240,7 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
             hop_pipe<FMT, 5, STREAM>(in, gp + 3 * lb, Vh, tf, i, psi, raw, ez_b, sb, acc);
             hop_pipe<FMT, 6, STREAM>(in, gq + 3 * lb, Vh, tb, tb, psi, raw, et_f, sf, acc);
             hop_pipe<FMT, 7, STREAM>(in, nullptr, Vh, 0, 0, psi, raw, et_b, sb, acc);
+#endif
         } else
 #endif
         {
