@@ -83,6 +83,11 @@ cola_status cola_destroy(cola_ctx *c);
 /* Message of the last failure on c (valid until the next call on c); "" if none.  c may be NULL
  * (returns the message of the last failed cola_create in this thread). */
 const char *cola_last_error(const cola_ctx *c);
+/* Tuning: bytes of L2 the kernels' sweep order may count on for the reuse of neighbour spinors (default 40 MB; 0
+ * restores it).  A neighbour spinor is used from three consecutive time slices; when three slices of reused spinors
+ * (all right-hand sides of a launch) exceed this budget the thread blocks sweep the lattice in bands of z-planes
+ * instead of slice by slice, which keeps the reuse inside L2.  Results do not depend on it. */
+cola_status cola_set_l2_budget(cola_ctx *c, size_t bytes);
 /* Change the stream subsequent calls launch on. */
 cola_status cola_set_stream(cola_ctx *c, void *stream);
 

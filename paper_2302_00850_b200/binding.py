@@ -27,7 +27,7 @@ EXPORTS = [
     "cola_cg_solve", "cola_dslash_apply_host", "cola_fermion_matrix_apply_host", "cola_cg_solve_host",
     "cola_launch_count",
     "cola_mrhs_workspace_bytes", "cola_set_mrhs_workspace", "cola_dslash_apply_mrhs", "cola_fermion_matrix_apply_mrhs",
-    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs",
+    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget",
 ]
 
 
@@ -66,6 +66,7 @@ def _load():
     lib.cola_last_error.argtypes = [vp]
     lib.cola_last_error.restype = ctypes.c_char_p
     lib.cola_set_stream.argtypes = [vp, vp]
+    lib.cola_set_l2_budget.argtypes = [vp, ctypes.c_size_t]
     lib.cola_spinor_bytes.argtypes = [vp, ci, ci]
     lib.cola_spinor_bytes.restype = ctypes.c_size_t
     lib.cola_workspace_bytes.argtypes = [vp]
@@ -160,6 +161,10 @@ class Cola:
             self.close()
         except Exception:
             pass
+
+    def set_l2_budget(self, nbytes: int = 0):
+        """Bytes of L2 the sweep order counts on for neighbour reuse (0: default 40 MB); tuning only, results unchanged."""
+        self._ck(_lib.cola_set_l2_budget(self._h, int(nbytes)))
 
     def set_stream(self, stream):
         self._ck(_lib.cola_set_stream(self._h, ctypes.c_void_p(stream)))

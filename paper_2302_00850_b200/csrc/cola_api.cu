@@ -23,6 +23,7 @@ struct cola_ctx {
     char *clovI64, *clovI32;        // odd parity only
     char *gauge16, *clovA16, *clovI16;   // 16-bit copies for COLA_F32_H16 (same index structure)
     int sloppy16;                   // the running solve's inner operator reads the 16-bit fields
+    size_t l2_budget;               // bytes of L2 the sweep order counts on for neighbour reuse (cola_set_l2_budget)
     char *tmp64, *tmp32;            // odd half-lattice temporaries of the Schur operator
     ReduceWs red;                   // deterministic-reduction buffers
     size_t red_blocks;              // max grid size of a reducing launch
@@ -135,6 +136,7 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     c->g.Vh = (int)c->Vh;
     for (int k = 0; k < 4; k++) c->g.bc[k] = p->bc[k];
     c->fmt32 = p->compress12 ? LINK_F32_12 : LINK_F32_18;
+    c->l2_budget = (size_t)40 << 20;
     c->stream = (cudaStream_t)p->stream;
     char *blk = nullptr;
     cudaError_t e = cudaMalloc(&blk, 4096);
@@ -176,6 +178,13 @@ cola_status cola_destroy(cola_ctx *c)
 }
 
 const char *cola_last_error(const cola_ctx *c) { return c ? c->err : g_create_err; }
+
+cola_status cola_set_l2_budget(cola_ctx *c, size_t bytes)
+{
+    if (!c) return COLA_EINVAL;
+    c->l2_budget = bytes ? bytes : ((size_t)40 << 20);
+    return COLA_OK;
+}
 
 cola_status cola_set_stream(cola_ctx *c, void *stream)
 {
@@ -269,6 +278,7 @@ static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, c
     a.sgn = dagger ? +1.0 : -1.0;
     a.parity = parity;
     a.skip = skip;
+    a.sweep = make_sweep(c->g, choose_zband(c->g.Xh * c->g.Y, c->g.Z, prec == COLA_F64 ? 192 : 96, c->l2_budget, 1));
     if (norm_out) {
         a.red = c->red;
         a.counter = &c->ctl->counter[0];
@@ -689,6 +699,7 @@ cola_status dslash_m(cola_ctx *c, cola_prec prec, int parity, int dagger, const 
     a.sgn = dagger ? +1.0 : -1.0;
     a.parity = parity;
     a.skip = skip;
+    a.sweep.zb = choose_zband(c->g.Xh * c->g.Y, c->g.Z, (size_t)(prec == COLA_F64 ? 192 : 96) * (size_t)nrhs, c->l2_budget, mrhs_tile_z(c->g));
     m.nrhs = nrhs;
     m.in_stride = in_stride;
     m.out_stride = out_stride;

@@ -10,6 +10,8 @@
 //
 // Chiral basis: gamma_mu = [[0, A_mu], [A_mu^+, 0]], A_k = -i sigma_k, A_t = 1:
 //   (1 + s gamma_mu) psi = [ h ; s A_mu^+ h ],   h = psi_upper + s A_mu psi_lower,   s = +-1.
+#include <string.h>
+
 #include "cola_device.cuh"
 
 namespace cola {
@@ -289,7 +291,14 @@ template <int FMT, int XPAY, int POST>
 __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
 {
     if (a.skip && *a.skip) return;
-    const int i = blockIdx.x * DSLASH_BLOCK + threadIdx.x;
+    unsigned run = blockIdx.x;   // which run of DSLASH_BLOCK consecutive sites this block covers
+    if (a.sweep.on) {            // z-banded sweep (Sweep in cola_internal.h): block order = [unit in plane, z in band, t, band]
+        const unsigned q1 = a.sweep.d_up.div(run), u = run - q1 * a.sweep.d_up.d;
+        const unsigned q2 = a.sweep.d_zb.div(q1), zi = q1 - q2 * a.sweep.d_zb.d;
+        const unsigned band = a.sweep.d_t.div(q2), t = q2 - band * a.sweep.d_t.d;
+        run = ((t * (unsigned)a.g.Z + band * a.sweep.d_zb.d + zi) * a.sweep.d_up.d) + u;
+    }
+    const int i = (int)run * DSLASH_BLOCK + (int)threadIdx.x;
     const bool want_norm = a.red.partials != nullptr;
     double nrm = 0.0;
     if (i < a.g.Vh) nrm = dslash_site<FMT, XPAY, POST, true>(a, i, a.in, a.y, a.out, want_norm);
@@ -331,13 +340,23 @@ __global__ void __launch_bounds__(MSITES * MrhsCfg<FMT>::NRB, MrhsCfg<FMT>::MINB
     const unsigned sb = blockIdx.x / (unsigned)m.ngroups, grp = blockIdx.x - sb * (unsigned)m.ngroups;
     const int k = (int)grp * NRB + (int)threadIdx.y;
     // site of this thread: tile origin (block-uniform) + position inside the tile
-    const unsigned b1 = tl.nb[0].div(sb), b2 = tl.nb[1].div(b1), b3 = tl.nb[2].div(b2);
+    const unsigned b1 = tl.nb[0].div(sb), b2 = tl.nb[1].div(b1);
+    unsigned bz, bt;
+    if (m.tsweep.on) {   // z-banded sweep over tiles: [x tile, y tile, z tile in band, t tile, band]
+        const unsigned q3 = m.tsweep.d_zb.div(b2), zi = b2 - q3 * m.tsweep.d_zb.d;
+        const unsigned band = m.tsweep.d_t.div(q3);
+        bt = q3 - band * m.tsweep.d_t.d;
+        bz = band * m.tsweep.d_zb.d + zi;
+    } else {
+        bt = tl.nb[2].div(b2);
+        bz = b2 - bt * tl.nb[2].d;
+    }
     const unsigned l = threadIdx.x;
     const int s0 = tl.sh[0], s1 = tl.sh[1], s2 = tl.sh[2];
     const int xh = (int)((sb - b1 * tl.nb[0].d) << s0) + (int)(l & ((1u << s0) - 1u));
     const int y = (int)((b1 - b2 * tl.nb[1].d) << s1) + (int)((l >> s0) & ((1u << s1) - 1u));
-    const int z = (int)((b2 - b3 * tl.nb[2].d) << s2) + (int)((l >> (s0 + s1)) & ((1u << s2) - 1u));
-    const int t = (int)(b3 << tl.sh[3]) + (int)(l >> (s0 + s1 + s2));
+    const int z = (int)(bz << s2) + (int)((l >> (s0 + s1)) & ((1u << s2) - 1u));
+    const int t = (int)(bt << tl.sh[3]) + (int)(l >> (s0 + s1 + s2));
     const int i = xh + g.Xh * (y + g.Y * (z + g.Z * t));
     const bool want_norm = m.partials != nullptr;
     const bool live = k < m.nrhs && (int)l < tl.vol;
@@ -409,6 +428,17 @@ cudaError_t launch_mrhs_fmt(MrhsArgs &m, cudaStream_t s)
     m.tile = make_tile(m.d.g, MSITES, COLA_MRHS_TILE_X);
     m.nsb = m.tile.ntiles;
     m.ngroups = (m.nrhs + NRB - 1) / NRB;
+    memset(&m.tsweep, 0, sizeof(m.tsweep));
+    {
+        const int tz = 1 << m.tile.sh[2], nbz = m.d.g.Z >> m.tile.sh[2], nbt = m.d.g.T >> m.tile.sh[3];
+        const int zbt = m.d.sweep.zb / tz;   // band in tiles
+        if (m.d.sweep.zb > 0 && zbt >= 1 && zbt < nbz && nbz % zbt == 0) {
+            m.tsweep.on = 1;
+            m.tsweep.zb = zbt;
+            m.tsweep.d_zb = make_fastdiv((unsigned)zbt);
+            m.tsweep.d_t = make_fastdiv((unsigned)nbt);
+        }
+    }
     const dim3 grid((unsigned)m.nsb * (unsigned)m.ngroups), block(MSITES, NRB);
     if (xpay == 0 && post == 0) dslash_mrhs_kernel<FMT, 0, 0><<<grid, block, 0, s>>>(m);
     else if (xpay == 0 && post == 1) dslash_mrhs_kernel<FMT, 0, 1><<<grid, block, 0, s>>>(m);
@@ -460,6 +490,32 @@ Tile make_tile(const Geom &g, int max_sites, int max_x)
     return t;
 }
 
+int choose_zband(int sites_per_plane, int nz, size_t bytes_per_site, size_t l2_budget, int mult)
+{
+    const double plane3 = 3.0 * (double)sites_per_plane * (double)bytes_per_site;
+    if (plane3 * nz <= (double)l2_budget) return 0;
+    int best = 0;
+    for (int zb = mult; zb < nz; zb += mult)
+        if (nz % zb == 0 && plane3 * zb <= (double)l2_budget) best = zb;
+    if (best == 0 && mult < nz && nz % mult == 0) best = mult;
+    return best;
+}
+
+Sweep make_sweep(const Geom &g, int zb)
+{
+    Sweep w;
+    memset(&w, 0, sizeof(w));
+    const int plane = g.Xh * g.Y;
+    if (zb <= 0 || zb >= g.Z || g.Z % zb != 0 || plane % DSLASH_BLOCK != 0) return w;
+    w.on = 1;
+    w.zb = zb;
+    w.d_up = make_fastdiv((unsigned)(plane / DSLASH_BLOCK));
+    w.d_zb = make_fastdiv((unsigned)zb);
+    w.d_t = make_fastdiv((unsigned)g.T);
+    return w;
+}
+
+int mrhs_tile_z(const Geom &g) { return 1 << make_tile(g, MSITES, COLA_MRHS_TILE_X).sh[2]; }
 int mrhs_site_blocks(const Geom &g) { return make_tile(g, MSITES, COLA_MRHS_TILE_X).ntiles; }
 
 cudaError_t launch_dslash_mrhs(int fmt, MrhsArgs &m, cudaStream_t s)

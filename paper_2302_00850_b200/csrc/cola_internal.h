@@ -111,8 +111,25 @@ struct HostStatus {
 //   v   = Cy*y + coef*v        if y      (Cy = A_p if clov_y else 1)     (H6/H7/H8 epilogue)
 //   v   = Cpost*v              if clov_post                              (H6: A^-1)
 //   out = v;  *norm_out = sum |v|^2 if partials                          (H9)
+// Sweep order of the thread blocks over the lattice.  A neighbour spinor is used three times one time slice apart
+// (hops from t-1, from its own slice, from t+1); L2 serves the second and third use only if the reused spinors of three
+// slices fit beside the streaming data.  When they do not (fp64 at 64^3x128, many right-hand sides), the blocks sweep
+// the lattice in bands of `zb` z-planes: all time slices of one band before the next band, so the reuse distance
+// shrinks to one band-slice at the price of re-reading the two z-planes next to each band.  `on == 0`: linear order.
+struct Sweep {
+    int on;
+    int zb;            // z-planes (single-rhs) or z-tiles (multi-rhs) per band
+    FastDiv d_up;      // block units per z-plane (single-rhs: Xh*Y/64) or tiles along x*y ... see the kernels
+    FastDiv d_zb;
+    FastDiv d_t;       // time extent (in tiles for the multi-rhs kernels)
+};
+// zb = 0 (off) if three slices of `bytes_per_site` reused bytes fit `l2_budget`, else the largest divisor of nz
+// (a multiple of `mult`) whose three band-slices fit, at least `mult`
+int choose_zband(int sites_per_plane, int nz, size_t bytes_per_site, size_t l2_budget, int mult);
+
 struct DslashArgs {
     Geom g;
+    Sweep sweep;            // single-rhs kernels; needs (Xh*Y) % 64 == 0
     const void *in;         // parity 1-p, internal half spinor
     void *out;              // parity p
     const void *gauge_p;    // links of parity p:   [mu][chunk][Vh]
@@ -149,8 +166,9 @@ struct Tile {
 Tile make_tile(const Geom &g, int max_sites, int max_x);
 
 struct MrhsArgs {
-    DslashArgs d;
-    Tile tile;           // d.red / d.counter / d.norm_out unused (per-rhs norms go through `partials`)
+    DslashArgs d;           // d.sweep.zb = z-PLANES per band wanted (0: linear); the launcher converts it to tiles
+    Tile tile;
+    Sweep tsweep;           // the same in units of tiles (filled by the launcher)           // d.red / d.counter / d.norm_out unused (per-rhs norms go through `partials`)
     int nrhs;               // right-hand sides of this launch, 1..MRHS_MAX
     int ngroups;            // rhs groups per site block (filled by the launcher)
     int nsb;                // site blocks (filled by the launcher)
@@ -161,11 +179,13 @@ struct MrhsArgs {
 
 // launchers (cola_dslash.cu)
 cudaError_t launch_dslash_mrhs(int fmt, MrhsArgs &m, cudaStream_t s);
+int mrhs_tile_z(const Geom &g);        // z extent of the multi-rhs tile (bands are whole tiles)
 int mrhs_site_blocks(const Geom &g);   // site blocks (tiles) of a multi-rhs launch = partial sums per vector
 // out[list[k]] (+)= sum_sb partials[list[k]*nsb + sb], fixed order
 cudaError_t launch_mrhs_reduce(const double *partials, int nsb, int nrhs, const int *list, double *out, int accumulate, const int *skip, cudaStream_t s);
 size_t dslash_grid_blocks(size_t Vh);   // blocks a dslash launch uses = partial sums it may write
 cudaError_t launch_dslash(int fmt, const DslashArgs &a, cudaStream_t s);
+Sweep make_sweep(const Geom &g, int zb);   // single-rhs sweep descriptor for bands of zb z-planes (zb = 0 or unsuitable geometry: off)
 // clover-only apply: out = C in on one parity (cola_dslash.cu)
 cudaError_t launch_clover_apply(cola_prec prec, const Geom &g, const void *clov, const void *in, void *out, cudaStream_t s);
 

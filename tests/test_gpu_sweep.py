@@ -1,0 +1,71 @@
+"""The z-banded sweep order of the thread blocks (cola_set_l2_budget) only changes WHICH block
+computes which sites: every operator result must be bit-identical to the linear sweep, for every band width, in the
+single-rhs kernels (bands of z-planes over runs of 64 sites) and the multi-rhs kernels (bands of z-tiles), and it must
+still agree with the oracle.  Small lattices never trigger it by themselves, so the L2 budget is lowered to force it."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2302_00850_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+BC = (1, 1, 1, -1)
+
+
+def rel(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+# (Xh*Y) % 64 == 0 is what the single-rhs banded sweep needs: 16x8 -> 64, 16x16 -> 128; Z = 8 gives bands of 1, 2, 4
+@pytest.mark.parametrize("dims", [(16, 8, 8, 4), (16, 16, 8, 2), (32, 4, 8, 6)])
+def test_banded_sweep_is_bit_identical_and_matches_oracle(dims):
+    from paper_2302_00850_b200 import binding
+
+    U = inputs.links_smooth(dims, 0.3, 23)
+    c = binding.Cola(dims, 0.1245, 1.0, bc=BC)
+    c.gauge_upload(U)
+    psi = inputs.source_gaussian(dims, 24)
+    v64 = c.spinor_pack(psi.cuda())
+    v32 = c.spinor_pack(psi.to(torch.complex64).cuda())
+    many = torch.stack([v32, c.spinor_pack(inputs.source_gaussian(dims, 25).to(torch.complex64).cuda()), v32.flip(2).contiguous()])
+
+    def everything():
+        return [c.fermion_matrix_apply(v64), c.fermion_matrix_apply(v32, dagger=True), c.schur_apply(v32[0].contiguous()),
+                c.schur_apply(v64[0].contiguous(), dagger=True), c.dslash_apply(1, v32[0].contiguous()),
+                c.fermion_matrix_apply(v32, h16=True), c.fermion_matrix_apply_mrhs(many), c.schur_apply_mrhs(many[:, 0].contiguous())]
+
+    ref = everything()
+    plane3 = 3 * (dims[0] // 2) * dims[1] * 96
+    for budget in (1, 2 * plane3, 4 * plane3, 2 * 2 * plane3):      # bands of 1, 2, 4 planes (fp32), 1, 1, 2, 2 (fp64)
+        c.set_l2_budget(budget)
+        for a, b in zip(everything(), ref):
+            assert torch.equal(a, b), budget
+    # and the banded result is right, not just reproducible
+    c.set_l2_budget(2 * plane3)
+    Un = U.numpy()
+    A = oracle.clover(dims, Un, 0.1245, 1.0)
+    want = oracle.M(dims, BC, Un, A, 0.1245, psi.numpy())
+    assert rel(c.spinor_unpack(c.fermion_matrix_apply(v64)).cpu().numpy(), want) < 1e-12
+    x, info = c.cg_solve(psi.cuda(), mixed=1)
+    assert info["converged"] and info["true_residual"] <= 1.05e-10
+    c.set_l2_budget(0)
+    x0, info0 = c.cg_solve(psi.cuda(), mixed=1)
+    assert info0["iters"] == info["iters"] and torch.equal(x, x0)
+    c.close()
+
+
+def test_unsuitable_geometry_falls_back_to_the_linear_sweep():
+    from paper_2302_00850_b200 import binding
+
+    dims = (12, 10, 6, 4)            # Xh*Y = 60: not a multiple of the 64-site runs
+    c = binding.Cola(dims, 0.1245, 1.0, bc=BC)
+    c.gauge_upload(inputs.links_smooth(dims, 0.3, 26))
+    v = c.spinor_pack(inputs.source_gaussian(dims, 27).to(torch.complex64).cuda())
+    ref = c.fermion_matrix_apply(v)
+    c.set_l2_budget(1)
+    assert torch.equal(c.fermion_matrix_apply(v), ref)
+    assert torch.equal(c.fermion_matrix_apply_mrhs(torch.stack([v, v]))[1], ref)
+    c.close()
