@@ -45,7 +45,7 @@ BYTES = {
 FLOPS = {"dslash": 1320, "dslash_clover_inv": 1824, "dslash_clover_xpay": 1872}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of dslash_kernel<F32x12, XPAY=2> from the committed
 # ncu --set full capture (a number read from a profile, never a timing taken under the profiler)
-NCU_TRAFFIC = {(32, 32, 32, 64): {"bytes_per_launch": 979020000, "source": "profiles/r1c_operators_full.txt (909.2 MB read + 69.82 MB write)"}}
+NCU_TRAFFIC = {(32, 32, 32, 64): {"bytes_per_launch": 979430000, "source": "profiles/r1d_operators_full.txt (909.2 MB read + 70.24 MB write)"}}
 CPU_SAMPLE_MAX_SITES = 1 << 22   # largest lattice the oracle's full fields are built for inside bench.py
 NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star's denominator, reported beside the measured one
 
