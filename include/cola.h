@@ -187,6 +187,11 @@ cola_status cola_schur_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int n
  * multi-rhs workspace for nrhs systems. */
 cola_status cola_cg_solve_mrhs(cola_ctx *c, const cola_solve_params *sp, int nrhs, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *infos);
 
+/* Host-only self-test (no GPU, no context): the magic-number division the kernels use for site indices against the
+ * hardware division, thread-block tile shapes and sweep-order permutations against their invariants.  msg (HOST, may be
+ * NULL) receives "ok" or the first failure.  COLA_OK or COLA_EINVAL. */
+cola_status cola_selftest_host(char *msg, size_t msg_len);
+
 /* Benchmark aid: number of kernels this context has launched since creation. */
 unsigned long long cola_launch_count(const cola_ctx *c);
 

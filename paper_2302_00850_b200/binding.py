@@ -27,7 +27,7 @@ EXPORTS = [
     "cola_cg_solve", "cola_dslash_apply_host", "cola_fermion_matrix_apply_host", "cola_cg_solve_host",
     "cola_launch_count",
     "cola_mrhs_workspace_bytes", "cola_set_mrhs_workspace", "cola_dslash_apply_mrhs", "cola_fermion_matrix_apply_mrhs",
-    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget",
+    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host",
 ]
 
 
@@ -67,6 +67,7 @@ def _load():
     lib.cola_last_error.restype = ctypes.c_char_p
     lib.cola_set_stream.argtypes = [vp, vp]
     lib.cola_set_l2_budget.argtypes = [vp, ctypes.c_size_t]
+    lib.cola_selftest_host.argtypes = [ctypes.c_char_p, ctypes.c_size_t]
     lib.cola_spinor_bytes.argtypes = [vp, ci, ci]
     lib.cola_spinor_bytes.restype = ctypes.c_size_t
     lib.cola_workspace_bytes.argtypes = [vp]
@@ -103,6 +104,15 @@ def _load():
 
 
 _lib = _load()
+
+
+def selftest_host() -> str:
+    """cola_selftest_host: host-side index machinery (no GPU).  Returns "ok" or raises with the first failure."""
+    buf = ctypes.create_string_buffer(256)
+    st = _lib.cola_selftest_host(buf, 256)
+    if st != COLA_OK:
+        raise RuntimeError(buf.value.decode())
+    return buf.value.decode()
 
 
 class ColaError(RuntimeError):

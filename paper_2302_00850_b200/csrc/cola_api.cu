@@ -1160,6 +1160,74 @@ cola_status cola_cg_solve_mrhs(cola_ctx *c, const cola_solve_params *sp, int nrh
     return solve_mrhs_impl(c, sp, nrhs, b_canon_dev, x_canon_dev, infos);
 }
 
+// Host-side self-test of the index machinery the kernels rely on (no GPU needed): magic-number division against the
+// hardware division, tile shapes and sweep descriptors against their invariants.
+cola_status cola_selftest_host(char *msg, size_t msg_len)
+{
+    auto say = [&](const char *what, long a, long b) {
+        if (msg && msg_len) snprintf(msg, msg_len, "%s (%ld, %ld)", what, a, b);
+        return COLA_EINVAL;
+    };
+    // floor(n/d) for every divisor up to 4096 (and a few large ones) over a spread of n < 2^31 incl. the edges
+    unsigned long long lcg = 88172645463325252ull;
+    for (unsigned d = 1; d <= 4200; d++) {
+        const FastDiv f = make_fastdiv(d);
+        auto q = [&](unsigned n) { return f.d == 1u ? n : (unsigned)(((unsigned long long)n * f.m) >> 32) >> f.sh; };
+        const unsigned edge[] = {0u, 1u, d - 1u, d, d + 1u, 2u * d - 1u, 2u * d, 0x7fffffffu, 0x7ffffffeu, 0x7fffffffu / d * d, 0x7fffffffu / d * d - 1u};
+        for (unsigned n : edge)
+            if (n <= 0x7fffffffu && q(n) != n / d) return say("fastdiv edge", (long)n, (long)d);
+        for (int k = 0; k < 2000; k++) {
+            lcg = lcg * 6364136223846793005ull + 1442695040888963407ull;
+            const unsigned n = (unsigned)(lcg >> 33);
+            if (q(n) != n / d) return say("fastdiv", (long)n, (long)d);
+        }
+    }
+    for (unsigned d : {65536u, 1000003u, 16777216u, 0x40000000u, 0x7fffffffu}) {
+        const FastDiv f = make_fastdiv(d);
+        for (unsigned n : {0u, d - 1u, d, d + 1u, 0x7fffffffu})
+            if ((f.d == 1u ? n : (unsigned)(((unsigned long long)n * f.m) >> 32) >> f.sh) != n / d) return say("fastdiv large", (long)n, (long)d);
+    }
+    // tiles and sweeps on a spread of lattices
+    const int L[][4] = {{2, 2, 2, 2}, {4, 4, 4, 4}, {4, 2, 6, 2}, {12, 10, 6, 4}, {16, 16, 16, 32}, {32, 32, 32, 64}, {48, 48, 48, 96}, {64, 64, 64, 128}, {6, 4, 2, 8}, {128, 2, 2, 2}};
+    for (const auto &d : L) {
+        Geom g;
+        memset(&g, 0, sizeof(g));
+        g.X = d[0]; g.Y = d[1]; g.Z = d[2]; g.T = d[3]; g.Xh = d[0] / 2;
+        g.Vh = g.Xh * g.Y * g.Z * g.T;
+        for (int ms : {32, 64, 128, 256}) {
+            const Tile t = make_tile(g, ms, 16);
+            const int ext[4] = {g.Xh, g.Y, g.Z, g.T};
+            int vol = 1;
+            for (int k = 0; k < 4; k++) {
+                if (ext[k] % (1 << t.sh[k])) return say("tile extent does not divide the lattice", d[k], 1 << t.sh[k]);
+                vol <<= t.sh[k];
+            }
+            if (vol != t.vol || vol > ms || t.ntiles * vol != g.Vh) return say("tile volume", vol, ms);
+        }
+        for (size_t budget : {(size_t)1, (size_t)100000, (size_t)40 << 20}) {
+            for (int mult : {1, 2}) {
+                const int zb = choose_zband(g.Xh * g.Y, g.Z, 96, budget, mult);
+                if (zb < 0 || zb >= g.Z + (zb == 0) || (zb && (g.Z % zb || zb % mult))) return say("zband", zb, g.Z);
+                const Sweep w = make_sweep(g, zb);
+                if (w.on && ((g.Xh * g.Y) % 64 || g.Z % w.zb)) return say("sweep on unsuitable geometry", zb, g.Z);
+                if (w.on) {   // the block permutation is a bijection on [0, Vh/64)
+                    const unsigned nb = (unsigned)(g.Vh / 64), up = w.d_up.d;
+                    unsigned long long sum = 0, want = (unsigned long long)nb * (nb - 1) / 2;
+                    for (unsigned b = 0; b < nb; b++) {
+                        const unsigned q1 = b / up, u = b % up, q2 = q1 / (unsigned)w.zb, zi = q1 % (unsigned)w.zb, band = q2 / (unsigned)g.T, t = q2 % (unsigned)g.T;
+                        const unsigned run = ((t * (unsigned)g.Z + band * (unsigned)w.zb + zi) * up) + u;
+                        if (run >= nb) return say("sweep run out of range", (long)run, (long)nb);
+                        sum += run;
+                    }
+                    if (sum != want) return say("sweep is not a permutation", (long)sum, (long)want);
+                }
+            }
+        }
+    }
+    if (msg && msg_len) snprintf(msg, msg_len, "ok");
+    return COLA_OK;
+}
+
 unsigned long long cola_launch_count(const cola_ctx *c) { return c ? c->launches : 0; }
 
 }  // extern "C"

@@ -44,6 +44,9 @@ def test_binding_lists_the_same_names(lib):
         method = name[len("cola_"):]
         if method in ("create", "destroy", "last_error"):
             continue
+        if method == "selftest_host":
+            assert hasattr(binding, method)
+            continue
         assert hasattr(binding.Cola, method), f"binding lacks Cola.{method}"
 
 
@@ -79,3 +82,10 @@ def test_oracle_and_cuda_path_share_no_code():
                     if s.startswith(("import ", "from ", "#include")):
                         for b in banned:
                             assert b not in s, f"{d}/{f}: '{s}'"
+
+
+def test_host_index_machinery_selftest(lib):
+    """Magic-number division vs hardware division for every divisor <= 4200, tile shapes, sweep permutations (no GPU)."""
+    from paper_2302_00850_b200 import binding
+
+    assert binding.selftest_host() == "ok"
