@@ -156,6 +156,12 @@ typedef struct {
  * Returns COLA_OK, or COLA_ENOCONV with info filled and x = last iterate. */
 cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info);
 
+/* Same solve, also recording the residual history of the recurrence: resid_hist_host[k] = |r_{k+1}| / |b| after CGLS
+ * pass k (k < min(info->iters, hist_len)); HOST array of hist_len doubles.  In the mixed modes this is the fp32
+ * recurrence's residual (the value the reliable-update test sees), before a reliable update replaces it. */
+cola_status cola_cg_solve_history(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info,
+                                  double *resid_hist_host, int hist_len);
+
 /* End-to-end variants: HOST canonical buffers; the host<->device copies are part of the call. */
 cola_status cola_dslash_apply_host(cola_ctx *c, cola_prec prec, cola_parity out_parity, const void *in_canon_host, void *out_canon_host);
 cola_status cola_fermion_matrix_apply_host(cola_ctx *c, cola_prec prec, int dagger, const void *in_canon_host, void *out_canon_host);

@@ -27,7 +27,7 @@ EXPORTS = [
     "cola_cg_solve", "cola_dslash_apply_host", "cola_fermion_matrix_apply_host", "cola_cg_solve_host",
     "cola_launch_count",
     "cola_mrhs_workspace_bytes", "cola_set_mrhs_workspace", "cola_dslash_apply_mrhs", "cola_fermion_matrix_apply_mrhs",
-    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host",
+    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host", "cola_cg_solve_history",
 ]
 
 
@@ -68,6 +68,7 @@ def _load():
     lib.cola_set_stream.argtypes = [vp, vp]
     lib.cola_set_l2_budget.argtypes = [vp, ctypes.c_size_t]
     lib.cola_selftest_host.argtypes = [ctypes.c_char_p, ctypes.c_size_t]
+    lib.cola_cg_solve_history.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo), ctypes.POINTER(cd), ci]
     lib.cola_spinor_bytes.argtypes = [vp, ci, ci]
     lib.cola_spinor_bytes.restype = ctypes.c_size_t
     lib.cola_workspace_bytes.argtypes = [vp]
@@ -316,6 +317,21 @@ class Cola:
         st = fn(self._h, ctypes.byref(sp), ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), ctypes.byref(info))
         self._ck(st, ok=(COLA_OK, COLA_ENOCONV))
         return x, self._info_dict(info, st)
+
+    def cg_solve_history(self, b: torch.Tensor, tol=1e-10, max_iter=20000, even_odd=True, mixed=False, delta=0.1, hist_len=4096):
+        """cg_solve on a device source that also returns the residual history |r_{k+1}|/|b| of the recurrence."""
+        assert b.is_cuda and b.dtype == torch.complex128 and b.numel() == self.V * 12
+        b = b.contiguous()
+        x = torch.empty_like(b)
+        sp = self._solve_params(tol, max_iter, even_odd, mixed, delta)
+        info = ColaSolveInfo()
+        hist = (ctypes.c_double * hist_len)()
+        st = _lib.cola_cg_solve_history(self._h, ctypes.byref(sp), ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), ctypes.byref(info),
+                                        hist, hist_len)
+        self._ck(st, ok=(COLA_OK, COLA_ENOCONV))
+        d = self._info_dict(info, st)
+        d["history"] = [hist[k] for k in range(min(info.iters, hist_len))]
+        return x, d
 
     def cg_solve_host(self, b: torch.Tensor, **kw):
         assert not b.is_cuda

@@ -23,6 +23,8 @@ struct cola_ctx {
     char *clovI64, *clovI32;        // odd parity only
     char *gauge16, *clovA16, *clovI16;   // 16-bit copies for COLA_F32_H16 (same index structure)
     int sloppy16;                   // the running solve's inner operator reads the 16-bit fields
+    double *hist;                   // HOST array of the running solve's residual history or nullptr (cola_cg_solve_history)
+    int hist_len;
     size_t l2_budget;               // bytes of L2 the sweep order counts on for neighbour reuse (cola_set_l2_budget)
     char *tmp64, *tmp32;            // odd half-lattice temporaries of the Schur operator
     ReduceWs red;                   // deterministic-reduction buffers
@@ -556,6 +558,7 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
                 const HostStatus *st = &hs;
                 rr = st->rr;
                 iters = k + 1;
+                if (c->hist && k < c->hist_len) c->hist[k] = sqrt(rr) / bnorm;   // |r_{k+1}| / |b| of the recurrence
                 flops += flops_K;
                 if (!st->flag) {
                     flops += flops_K;
@@ -1031,6 +1034,19 @@ cola_status cola_schur_apply(cola_ctx *c, cola_prec prec, int dagger, const void
 cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info)
 {
     return solve_impl(c, sp, b_canon_dev, x_canon_dev, info);
+}
+
+cola_status cola_cg_solve_history(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info,
+                                  double *resid_hist_host, int hist_len)
+{
+    if (!c) return COLA_EINVAL;
+    if (!resid_hist_host || hist_len < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_history: NULL or empty history buffer");
+    c->hist = resid_hist_host;
+    c->hist_len = hist_len;
+    const cola_status st = solve_impl(c, sp, b_canon_dev, x_canon_dev, info);
+    c->hist = nullptr;
+    c->hist_len = 0;
+    return st;
 }
 
 // ---- end-to-end variants with HOST buffers.  Staging lives in the tail of the solver scratch
