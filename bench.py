@@ -365,6 +365,15 @@ def main():
     ms, flops_all = aggregate_over_ranks(ms_local, flops, device=dev)
     value = flops_all / (ms * 1e-3) / 1e9
 
+    # ---- one more step with CUDA-event pairs around every launch of the dominant kernel (in-solve duration for `roofline`)
+    in_solve = None
+    if rank == 0:
+        ctx.profile_kernel(True)
+        one_step()
+        k_ms, k_n, k_skipped = ctx.profile_result()
+        ctx.profile_kernel(False)
+        in_solve = {"avg_launch_ms": round(k_ms, 5), "launches": k_n, "skipped_speculative_launches": k_skipped}
+
     # ---- end to end: host buffers through cola_cg_solve_host
     b_host = source(0).cpu().pin_memory()
     x_host = torch.empty_like(b_host).pin_memory()
@@ -469,6 +478,12 @@ def main():
         if tuple(dims) in NCU_TRAFFIC:
             roof["traffic"] = NCU_TRAFFIC[tuple(dims)]["bytes_per_launch"]
             roof["traffic_source"] = NCU_TRAFFIC[tuple(dims)]["source"]
+        if in_solve and in_solve["launches"]:
+            # the same kernel inside a solve step (event pair around each launch, speculative no-op launches excluded)
+            gbs = per_launch_bytes / (in_solve["avg_launch_ms"] * 1e-3) / 1e9
+            in_solve.update({"achieved": round(gbs, 1), "frac": round(gbs / peak, 4), "frac_of_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4),
+                             "note": "same peak (MEASURED_PEAKS.json has one HBM figure); measured in an extra step after the timed ones"})
+            roof["in_solve"] = in_solve
     cpu = None
     if U_cpu is not None:
         cpu = cpu_baseline_sample(dict(cfg, dims=cpu_dims), U_cpu)

@@ -193,6 +193,14 @@ cola_status cola_schur_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int n
  * multi-rhs workspace for nrhs systems. */
 cola_status cola_cg_solve_mrhs(cola_ctx *c, const cola_solve_params *sp, int nrhs, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *infos);
 
+/* Measurement aid: with enable != 0 every later launch of the fused dslash + clover + xpay kernel in fp32 / 16-bit
+ * (Schur kernel 2 / M: the dominant kernel of a mixed-precision solve) is bracketed by a pair of CUDA events on the
+ * context's stream, up to 4096 launches; cola_profile_result synchronises, returns the average duration in ms of the
+ * launches that did work, their count and the number of speculative launches that returned at once, and clears the
+ * window.  The event pairs cost about a microsecond per launch; leave it off for timed runs. */
+cola_status cola_profile_kernel(cola_ctx *c, int enable);
+cola_status cola_profile_result(cola_ctx *c, double *avg_ms, int *count, int *skipped);
+
 /* Host-only self-test (no GPU, no context): the magic-number division the kernels use for site indices against the
  * hardware division, thread-block tile shapes and sweep-order permutations against their invariants.  msg (HOST, may be
  * NULL) receives "ok" or the first failure.  COLA_OK or COLA_EINVAL. */

@@ -27,7 +27,7 @@ EXPORTS = [
     "cola_cg_solve", "cola_dslash_apply_host", "cola_fermion_matrix_apply_host", "cola_cg_solve_host",
     "cola_launch_count",
     "cola_mrhs_workspace_bytes", "cola_set_mrhs_workspace", "cola_dslash_apply_mrhs", "cola_fermion_matrix_apply_mrhs",
-    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host", "cola_cg_solve_history",
+    "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host", "cola_cg_solve_history", "cola_profile_kernel", "cola_profile_result",
 ]
 
 
@@ -68,6 +68,8 @@ def _load():
     lib.cola_set_stream.argtypes = [vp, vp]
     lib.cola_set_l2_budget.argtypes = [vp, ctypes.c_size_t]
     lib.cola_selftest_host.argtypes = [ctypes.c_char_p, ctypes.c_size_t]
+    lib.cola_profile_kernel.argtypes = [vp, ci]
+    lib.cola_profile_result.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(ci)]
     lib.cola_cg_solve_history.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo), ctypes.POINTER(cd), ci]
     lib.cola_spinor_bytes.argtypes = [vp, ci, ci]
     lib.cola_spinor_bytes.restype = ctypes.c_size_t
@@ -172,6 +174,16 @@ class Cola:
             self.close()
         except Exception:
             pass
+
+    def profile_kernel(self, enable: bool = True):
+        """Bracket later launches of the fused dslash+clover+xpay kernel (fp32 / 16-bit) with CUDA event pairs."""
+        self._ck(_lib.cola_profile_kernel(self._h, int(bool(enable))))
+
+    def profile_result(self):
+        """(average ms of the launches that did work, their count, speculative launches that returned at once)."""
+        ms, n, sk = ctypes.c_double(), ctypes.c_int(), ctypes.c_int()
+        self._ck(_lib.cola_profile_result(self._h, ctypes.byref(ms), ctypes.byref(n), ctypes.byref(sk)))
+        return ms.value, n.value, sk.value
 
     def set_l2_budget(self, nbytes: int = 0):
         """Bytes of L2 the sweep order counts on for neighbour reuse (0: default 40 MB); tuning only, results unchanged."""
