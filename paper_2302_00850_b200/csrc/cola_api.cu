@@ -211,17 +211,25 @@ cola_status cola_profile_result(cola_ctx *c, double *avg_ms, int *count, int *sk
     if (!c->prof_ev || c->prof_n == 0) return COLA_OK;
     CK(cudaSetDevice(c->p.device));
     CK(cudaStreamSynchronize(c->stream));
-    float *ms = new float[c->prof_n];
-    float mx = 0.f;
+    float *ms = new float[2 * c->prof_n];
     for (int k = 0; k < c->prof_n; k++) {
         cudaError_t e = cudaEventElapsedTime(&ms[k], c->prof_ev[2 * k], c->prof_ev[2 * k + 1]);
         if (e != cudaSuccess) { delete[] ms; return fail(c, COLA_ECUDA, "cola_profile_result: %s", cudaGetErrorString(e)); }
-        if (ms[k] > mx) mx = ms[k];
+        ms[c->prof_n + k] = ms[k];
     }
-    // speculatively queued launches that found the flag raised return at once: they are not applications of the operator
+    // speculatively queued launches that found the flag raised return at once: they are not applications of the
+    // operator.  Working launches are the large majority, so "well below the median" identifies the no-ops.
+    float *sorted = ms + c->prof_n;
+    for (int i = 1; i < c->prof_n; i++) {   // insertion sort: at most 4096 entries, once per window
+        const float v = sorted[i];
+        int j = i - 1;
+        for (; j >= 0 && sorted[j] > v; j--) sorted[j + 1] = sorted[j];
+        sorted[j + 1] = v;
+    }
+    const float median = sorted[c->prof_n / 2];
     double sum = 0.0;
     for (int k = 0; k < c->prof_n; k++) {
-        if (ms[k] < 0.25f * mx) (*skipped)++;
+        if (ms[k] < 0.25f * median) (*skipped)++;
         else { sum += ms[k]; (*count)++; }
     }
     delete[] ms;

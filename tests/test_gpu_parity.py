@@ -342,3 +342,29 @@ def test_device_links_upload_equals_host_upload(cola_mod):
     ya = a.fermion_matrix_apply(a.spinor_pack(psi))
     yd = d.fermion_matrix_apply(d.spinor_pack(psi))
     assert torch.equal(ya, yd)
+
+
+def test_profile_kernel_counts_the_dominant_kernel_only(cola_mod):
+    dims = (8, 8, 8, 16)
+    c = cola_mod.Cola(dims, 0.1245, 1.0)
+    c.gauge_upload(inputs.links_smooth(dims, 0.3, 9))
+    v32 = c.spinor_pack(inputs.source_gaussian(dims, 3).to(torch.complex64).cuda())
+    v64 = c.spinor_pack(inputs.source_gaussian(dims, 3).cuda())
+    assert c.profile_result() == (0.0, 0, 0)
+    c.profile_kernel(True)
+    for _ in range(5):
+        c.schur_apply(v32[0].contiguous())          # one fused dslash+clover+xpay launch each (kernel 2)
+    c.fermion_matrix_apply(v32)                      # two
+    c.schur_apply(v64[0].contiguous())               # fp64: not the inner-precision kernel, not counted
+    c.dslash_apply(0, v32[1].contiguous())           # plain dslash: not counted
+    ms, n, skipped = c.profile_result()
+    assert n == 7 and skipped == 0 and 0 < ms < 5
+    # a mixed solve: 2 per iteration + the start-up application, speculative no-ops reported apart
+    x, info = c.cg_solve(inputs.source_gaussian(dims, 4).cuda(), mixed=1)
+    ms, n, skipped = c.profile_result()
+    # (on a lattice this small a working launch is not much longer than a no-op, so only the total is exact)
+    assert 2 * info["iters"] + 1 <= n + skipped <= 2 * info["iters"] + 1 + 2 * info["reliable_updates"] and n > info["iters"]
+    c.profile_kernel(False)
+    c.schur_apply(v32[0].contiguous())
+    assert c.profile_result() == (0.0, 0, 0)
+    c.close()
