@@ -34,6 +34,8 @@ __global__ void __launch_bounds__(BB) norm2_kernel(const typename VT<T>::V *v, s
 template <typename T>
 __global__ void __launch_bounds__(BB) r_update_kernel(typename VT<T>::V *r, const typename VT<T>::V *q, Ctl *ctl, int cur, int iter, const int *skip, HostStatus *mirror, size_t n, ReduceWs red)
 {
+    pdl_trigger();
+    pdl_wait();
     if (skip && *skip) return;
     const T ma = (T)(-(ctl->gam[cur] / ctl->qq));
     double acc = 0.0;
@@ -64,6 +66,8 @@ __global__ void __launch_bounds__(BB) r_update_kernel(typename VT<T>::V *r, cons
 template <typename T, bool DO_X, bool DO_P>
 __global__ void __launch_bounds__(BB) xp_update_kernel(typename VT<T>::V *x, typename VT<T>::V *p, const typename VT<T>::V *s, const Ctl *ctl, int cur, const int *skip, size_t n)
 {
+    pdl_trigger();
+    pdl_wait();
     if (skip && *skip) return;
     const T alpha = (T)(ctl->gam[cur] / ctl->qq);
     const T beta = (T)(ctl->gam[cur ^ 1] / ctl->gam[cur]);
@@ -263,10 +267,10 @@ cudaError_t launch_r_update(cola_prec prec, void *r, const void *q, Ctl *ctl, in
 {
     if (prec == COLA_F64) {
         const size_t n = 12 * n_sites;
-        r_update_kernel<double><<<blas_grid(n), BB, 0, s>>>((double2 *)r, (const double2 *)q, ctl, cur, iter, skip, mirror, n, red);
+        return launch_pdl(r_update_kernel<double>, dim3(blas_grid(n)), dim3(BB), s, (double2 *)r, (const double2 *)q, ctl, cur, iter, skip, mirror, n, red);
     } else {
         const size_t n = 6 * n_sites;
-        r_update_kernel<float><<<blas_grid(n), BB, 0, s>>>((float4 *)r, (const float4 *)q, ctl, cur, iter, skip, mirror, n, red);
+        return launch_pdl(r_update_kernel<float>, dim3(blas_grid(n)), dim3(BB), s, (float4 *)r, (const float4 *)q, ctl, cur, iter, skip, mirror, n, red);
     }
     return cudaGetLastError();
 }
@@ -276,9 +280,9 @@ static void xp_dispatch(void *x, void *p, const void *sv, const Ctl *ctl, int cu
 {
     typedef typename VT<T>::V V;
     const unsigned grid = blas_grid(n);
-    if (do_x && do_p) xp_update_kernel<T, true, true><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
-    else if (do_x) xp_update_kernel<T, true, false><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
-    else if (do_p) xp_update_kernel<T, false, true><<<grid, BB, 0, s>>>((V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
+    if (do_x && do_p) launch_pdl(xp_update_kernel<T, true, true>, dim3(grid), dim3(BB), s, (V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
+    else if (do_x) launch_pdl(xp_update_kernel<T, true, false>, dim3(grid), dim3(BB), s, (V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
+    else if (do_p) launch_pdl(xp_update_kernel<T, false, true>, dim3(grid), dim3(BB), s, (V *)x, (V *)p, (const V *)sv, ctl, cur, skip, n);
 }
 
 cudaError_t launch_xp_update(cola_prec prec, void *x, void *p, const void *sv, const Ctl *ctl, int cur, int do_x, int do_p, const int *skip, size_t n_sites, cudaStream_t s)

@@ -8,6 +8,47 @@
 
 namespace cola {
 
+// Programmatic dependent launch (sm_90+): a kernel launched with launch_pdl may be scheduled while its predecessor in
+// the stream is still draining.  pdl_trigger() at the top of the predecessor says "my blocks have all started", so the
+// successor's blocks take the SM slots the predecessor's last wave leaves free; pdl_wait() in the successor blocks
+// until the predecessor has completed and its writes are visible.  Every kernel launched through launch_pdl calls
+// pdl_wait() before it touches memory.  Without the launch attribute both are no-ops.
+#ifndef COLA_PDL
+#define COLA_PDL 1
+#endif
+__device__ __forceinline__ void pdl_trigger()
+{
+#if COLA_PDL
+    asm volatile("griddepcontrol.launch_dependents;");
+#endif
+}
+__device__ __forceinline__ void pdl_wait()
+{
+#if COLA_PDL
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, cudaStream_t s, Args... args)
+{
+#if COLA_PDL
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+#else
+    kern<<<grid, block, 0, s>>>(args...);
+    return cudaGetLastError();
+#endif
+}
+
 template <typename T> struct VT;
 template <> struct VT<float> {
     typedef float4 V;

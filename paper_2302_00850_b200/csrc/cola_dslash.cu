@@ -290,6 +290,8 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
 template <int FMT, int XPAY, int POST>
 __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
 {
+    pdl_trigger();
+    pdl_wait();
     if (a.skip && *a.skip) return;
     unsigned run = blockIdx.x;   // which run of DSLASH_BLOCK consecutive sites this block covers
     if (a.sweep.on) {            // z-banded sweep (Sweep in cola_internal.h): block order = [unit in plane, z in band, t, band]
@@ -410,11 +412,11 @@ cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
     const int xpay = a.y ? (a.clov_y ? 2 : 1) : 0;
     const int post = a.clov_post ? 1 : 0;
     const dim3 grid((a.g.Vh + DSLASH_BLOCK - 1) / DSLASH_BLOCK), block(DSLASH_BLOCK);
-    if (xpay == 0 && post == 0) dslash_kernel<FMT, 0, 0><<<grid, block, 0, s>>>(a);
-    else if (xpay == 0 && post == 1) dslash_kernel<FMT, 0, 1><<<grid, block, 0, s>>>(a);
-    else if (xpay == 1 && post == 0) dslash_kernel<FMT, 1, 0><<<grid, block, 0, s>>>(a);
-    else if (xpay == 1 && post == 1) dslash_kernel<FMT, 1, 1><<<grid, block, 0, s>>>(a);
-    else if (xpay == 2 && post == 0) dslash_kernel<FMT, 2, 0><<<grid, block, 0, s>>>(a);
+    if (xpay == 0 && post == 0) launch_pdl(dslash_kernel<FMT, 0, 0>, grid, block, s, a);
+    else if (xpay == 0 && post == 1) launch_pdl(dslash_kernel<FMT, 0, 1>, grid, block, s, a);
+    else if (xpay == 1 && post == 0) launch_pdl(dslash_kernel<FMT, 1, 0>, grid, block, s, a);
+    else if (xpay == 1 && post == 1) launch_pdl(dslash_kernel<FMT, 1, 1>, grid, block, s, a);
+    else if (xpay == 2 && post == 0) launch_pdl(dslash_kernel<FMT, 2, 0>, grid, block, s, a);
     else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
