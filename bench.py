@@ -171,7 +171,7 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
     return out
 
 
-def cpu_baseline_sample(cfg, U_cpu, n_pairs=2):
+def cpu_baseline_sample(cfg, U_cpu, n_pairs=10):
     """The oracle as it stands on the host cores: n_pairs x (S, S^dagger) applications on the same lattice."""
     import numpy as np
 
