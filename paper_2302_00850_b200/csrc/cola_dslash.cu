@@ -168,7 +168,11 @@ __device__ __forceinline__ void hop_pipe(const void *in, const char *gauge_next,
 // One output site i of parity a.parity:  v = D in;  v = [A] y + coef v (XPAY);  v = Cpost v (POST);  out = v.
 // Returns |v|^2 if want_norm.  XPAY: 0 none, 1 v = y + coef v, 2 v = A y + coef v.   POST: 0 none, 1 v = Cpost v.
 // STREAM: links and clover are read once (no L1 allocation); !STREAM: they are shared by the right-hand sides of a block.
-template <int FMT, int XPAY, int POST, bool STREAM>
+// PDLW (16-bit kernels only): the kernel was launched as a programmatic dependent and has not waited for its predecessor
+// yet: the index arithmetic and the raw links of the first two hops run before pdl_wait(); a raised skip flag
+// (grid-uniform) is reported by returning -1.  (+2 % for the SM-bound 16-bit kernels; the fp32 kernels lose 1.7 % with
+// the reordered first loads and wait at the top of the kernel instead.)
+template <int FMT, int XPAY, int POST, bool STREAM, bool PDLW = false>
 __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, const void *in, const void *yin, void *out, const bool want_norm)
 {
     typedef typename LinkT<FMT>::T T;
@@ -217,10 +221,19 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
             // two hops ahead: buffers A (even hops) and B (odd hops); hop h refills its buffer with hop h+2
             T psiA[24], psiB[24];
             RawLink<FMT> rawA, rawB;
-            load_reals<T, 24, false>(in, Vh, xf, psiA);
-            load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, rawA);
-            load_reals<T, 24, false>(in, Vh, xb, psiB);
-            load_raw_link<FMT, STREAM>(gq + 0 * lb, Vh, xb, rawB);
+            if (PDLW) {
+                load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, rawA);
+                load_raw_link<FMT, STREAM>(gq + 0 * lb, Vh, xb, rawB);
+                pdl_wait();
+                if (a.skip && *a.skip) return -1.0;
+                load_reals<T, 24, false>(in, Vh, xf, psiA);
+                load_reals<T, 24, false>(in, Vh, xb, psiB);
+            } else {
+                load_reals<T, 24, false>(in, Vh, xf, psiA);
+                load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, rawA);
+                load_reals<T, 24, false>(in, Vh, xb, psiB);
+                load_raw_link<FMT, STREAM>(gq + 0 * lb, Vh, xb, rawB);
+            }
             hop_pipe<FMT, 0, STREAM, 6>(in, gp + 1 * lb, Vh, yf, i, psiA, rawA, ex_f, sf, acc);
             hop_pipe<FMT, 1, STREAM, 6>(in, gq + 1 * lb, Vh, yb, yb, psiB, rawB, ex_b, sb, acc);
             hop_pipe<FMT, 2, STREAM, 6>(in, gp + 2 * lb, Vh, zf, i, psiA, rawA, ey_f, sf, acc);
@@ -290,9 +303,12 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
 template <int FMT, int XPAY, int POST>
 __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
 {
+    constexpr bool LATE_WAIT = (FMT == LINK_I16_12) && (COLA_PIPE == 2);   // see dslash_site<.., PDLW>
     pdl_trigger();
-    pdl_wait();
-    if (a.skip && *a.skip) return;
+    if (!LATE_WAIT) {
+        pdl_wait();
+        if (a.skip && *a.skip) return;
+    }
     unsigned run = blockIdx.x;   // which run of DSLASH_BLOCK consecutive sites this block covers
     if (a.sweep.on) {            // z-banded sweep (Sweep in cola_internal.h): block order = [unit in plane, z in band, t, band]
         const unsigned q1 = a.sweep.d_up.div(run), u = run - q1 * a.sweep.d_up.d;
@@ -303,7 +319,13 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
     const int i = (int)run * DSLASH_BLOCK + (int)threadIdx.x;
     const bool want_norm = a.red.partials != nullptr;
     double nrm = 0.0;
-    if (i < a.g.Vh) nrm = dslash_site<FMT, XPAY, POST, true>(a, i, a.in, a.y, a.out, want_norm);
+    if (i < a.g.Vh) {
+        nrm = dslash_site<FMT, XPAY, POST, true, LATE_WAIT>(a, i, a.in, a.y, a.out, want_norm);
+    } else if (LATE_WAIT) {
+        pdl_wait();
+        nrm = (a.skip && *a.skip) ? -1.0 : 0.0;
+    }
+    if (LATE_WAIT && nrm < 0.0) return;   // skip flag raised: the same for every thread of the grid
     if (want_norm) grid_sum_finalize(nrm, a.red, a.counter, a.norm_out, a.norm_accumulate != 0);
 }
 
