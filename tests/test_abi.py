@@ -65,6 +65,13 @@ def test_create_rejects_bad_lattices_without_touching_the_gpu(lib):
         assert st == binding.COLA_EINVAL
         assert not h.value
         assert b"cola_create" in lib.cola_last_error(None)
+    # largest lattice: site indices are 32-bit, so a half volume above 2e9 is refused (1024^3 x 8 = 4.3e9 per parity)
+    p = binding.ColaParams()
+    p.dims[:] = (1024, 1024, 1024, 8)
+    p.bc[:] = (1, 1, 1, -1)
+    h = ctypes.c_void_p()
+    assert lib.cola_create(ctypes.byref(h), ctypes.byref(p)) == binding.COLA_EINVAL and not h.value
+    assert b"32-bit" in lib.cola_last_error(None)
     assert lib.cola_create(None, None) == binding.COLA_EINVAL
     assert lib.cola_destroy(None) == binding.COLA_OK
 

@@ -184,6 +184,8 @@ def test_mrhs_error_codes(binding):
     with pytest.raises(b.ColaError) as e:
         c.set_mrhs_workspace(17)
     assert e.value.status == b.COLA_EINVAL
+    assert c.mrhs_workspace_bytes(0) == 0 and c.mrhs_workspace_bytes(17) == 0
+    assert b._lib.cola_schur_apply_mrhs(c._h, b.COLA_F32, 0, 0, v.data_ptr(), out.data_ptr()) in (b.COLA_EINVAL, b.COLA_ENOTREADY)   # empty batch
     c.set_mrhs_workspace(2)
     st = b._lib.cola_schur_apply_mrhs(c._h, b.COLA_F32, 0, 3, v.data_ptr(), out.data_ptr())
     assert st == b.COLA_ENOTREADY                  # workspace too small for 3 systems
