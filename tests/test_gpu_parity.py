@@ -368,3 +368,35 @@ def test_profile_kernel_counts_the_dominant_kernel_only(cola_mod):
     c.schur_apply(v32[0].contiguous())
     assert c.profile_result() == (0.0, 0, 0)
     c.close()
+
+
+def test_everything_runs_on_the_callers_stream(cola_mod):
+    """The context launches on the stream it was given (torch's current stream at creation, or cola_set_stream): a solve
+    on a side stream, with the inputs produced on that stream right before, gives the default-stream result bit for bit."""
+    dims = (8, 8, 8, 16)
+    U = inputs.links_smooth(dims, 0.3, 9)
+    b_host = inputs.source_gaussian(dims, 5)
+    c0 = cola_mod.Cola(dims, 0.1245, 1.0)
+    c0.gauge_upload(U)
+    x0, info0 = c0.cg_solve(b_host.cuda(), mixed=1)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        c1 = cola_mod.Cola(dims, 0.1245, 1.0)          # picks up `side`
+        c1.gauge_upload(U)
+        b = b_host.cuda(non_blocking=True) * 1.0        # produced on `side` just before the solve
+        x1, info1 = c1.cg_solve(b, mixed=1)
+        v = c1.spinor_pack(b.to(torch.complex64))
+        y1 = c1.schur_apply(v[0].contiguous())
+    side.synchronize()
+    assert info1["iters"] == info0["iters"] and torch.equal(x1, x0)
+    y0 = c0.schur_apply(c0.spinor_pack(b_host.to(torch.complex64).cuda())[0].contiguous())
+    torch.cuda.synchronize()
+    assert torch.equal(y0, y1)
+    # cola_set_stream moves an existing context
+    c0.set_stream(side.cuda_stream)
+    with torch.cuda.stream(side):
+        x2, info2 = c0.cg_solve(b_host.cuda(), mixed=1)
+    side.synchronize()
+    assert torch.equal(x2, x0)
+    c0.close()
+    c1.close()
