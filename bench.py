@@ -13,7 +13,13 @@ metric  = Dirac-operator GFLOP/s sustained over the solve, counted flops (1320/s
           clover, 48/site xpay) / device time, whole job over all ranks (BASELINE.json "metric").
 e2e     = the same through cola_cg_solve_host: b in pinned HOST memory, x returned to pinned HOST memory.
 roofline= the dominant kernel (fused dslash + clover + xpay, fp32 with 12-real links) timed alone with CUDA
-          events: algorithmic bytes per launch / average launch time, against MEASURED_PEAKS.json hbm_gbs.
+          events: algorithmic bytes per launch / average launch time, against MEASURED_PEAKS.json hbm_gbs;
+          roofline.in_solve = the same kernel inside a solve (CUDA-event pair around each of its launches in one extra
+          step; cola_profile_kernel).
+extras  : solve_h16 = the same step with 16-bit links + fp16 clover in the inner iteration (mixed = 2, SURVEY 8(f)
+          NEXT-2); batched (config 3) = its 12 sources as one multi-rhs solve (NEXT-1); operators = every operator
+          x {fp32 x12, fp64 x18, 16-bit}.  --operators-only [--nrhs N] [--lattice X,Y,Z,T] is the short launch sequence
+          the ncu captures and the volume sweep in profiles/ come from.
 N > 1   : replicas only (the path has no inter-GPU exchange): every rank solves its own
           source on its own GPU; value = all ranks' flops / max-over-ranks time ("weak").
 """
