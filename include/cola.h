@@ -188,8 +188,9 @@ cola_status cola_schur_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int n
 /* Batched solve of M x_n = b_n, n < nrhs, by mixed-precision even-odd CGNR (sp->even_odd and sp->mixed must be 1):
  * the systems advance in lock step, each with its own alpha, beta, stopping test and reliable-update schedule
  * (SURVEY O7/O8 per system); a system that has converged drops out of the batch.  b_canon_dev / x_canon_dev: nrhs
- * canonical complex128 DEVICE arrays back to back; infos: HOST array of nrhs entries (seconds = time of the whole
- * batch).  COLA_ENOCONV if any system hit max_iter (its info has the last residual).  COLA_ENOTREADY without a
+ * canonical complex128 DEVICE arrays back to back (b and x must not overlap; during the call x also holds the
+ * solver's internal iterates, its final content is the canonical solution); infos: HOST array of nrhs entries
+ * (seconds = time of the whole batch).  COLA_ENOCONV if any system hit max_iter (its info has the last residual).  COLA_ENOTREADY without a
  * multi-rhs workspace for nrhs systems. */
 cola_status cola_cg_solve_mrhs(cola_ctx *c, const cola_solve_params *sp, int nrhs, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *infos);
 
