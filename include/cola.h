@@ -153,7 +153,8 @@ typedef struct {
 } cola_solve_info;
 
 /* H9-H12: solve M x = b.  b_canon_dev / x_canon_dev: canonical complex128 DEVICE arrays, V sites.
- * Returns COLA_OK, or COLA_ENOCONV with info filled and x = last iterate. */
+ * Returns COLA_OK, or COLA_ENOCONV with info filled and x = last iterate; COLA_EINVAL if the source (or, through the
+ * residual, the gauge field) contains NaN or Inf. */
 cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info);
 
 /* Same solve, also recording the residual history of the recurrence: resid_hist_host[k] = |r_{k+1}| / |b| after CGLS

@@ -571,6 +571,7 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
     double bb = 0.0;
     ST(norm2(c, COLA_F64, B, c->V, &ctl->aux[2]));
     ST(read_scalar(c, &ctl->aux[2], &bb));
+    if (!(bb == bb) || bb > 1e300) return fail(c, COLA_EINVAL, "cola_cg_solve: the source contains NaN or Inf");
     CK(cudaMemsetAsync(X, 0, 2 * h64, c->stream));
     const double bnorm = sqrt(bb);
     int status_conv = 0;
@@ -622,6 +623,10 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
                 rr = st->rr;
                 iters = k + 1;
                 if (c->hist && k < c->hist_len) c->hist[k] = sqrt(rr) / bnorm;   // |r_{k+1}| / |b| of the recurrence
+                if (!(rr == rr)) {   // NaN/Inf in the source or the links: no test below would ever fire
+                    CK(cudaStreamSynchronize(c->stream));
+                    return fail(c, COLA_EINVAL, "cola_cg_solve: the residual is not a number (NaN or Inf in the source or the gauge field)");
+                }
                 flops += flops_K;
                 if (!st->flag) {
                     flops += flops_K;
@@ -885,6 +890,7 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
         c->launches++;
         ST(norm2(c, COLA_F64, Bt, c->V, &ctl->aux[2]));
         ST(read_scalar(c, &ctl->aux[2], &bb[n]));
+        if (!(bb[n] == bb[n]) || bb[n] > 1e300) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: a source contains NaN or Inf");
         bnorm[n] = sqrt(bb[n]);
         CK(cudaMemsetAsync(X, 0, f64, c->stream));
         CK(cudaMemsetAsync(c->m_x32 + (size_t)n * h32, 0, h32, c->stream));

@@ -329,6 +329,17 @@ def test_error_codes(cola_mod):
     with pytest.raises(b.ColaError) as e:
         c.cg_solve(src, tol=-1.0)
     assert e.value.status == b.COLA_EINVAL
+    bad_src = src.clone()
+    bad_src[1, 2, 3, 0, 1, 1] = float("nan")
+    for kw in (dict(mixed=0), dict(mixed=1)):
+        with pytest.raises(b.ColaError) as e:
+            c.cg_solve(bad_src, **kw)
+        assert e.value.status == b.COLA_EINVAL and "NaN" in str(e.value)
+    with pytest.raises(b.ColaError) as e:
+        c.cg_solve_mrhs(torch.stack([src, bad_src]))
+    assert e.value.status == b.COLA_EINVAL
+    xx, info = c.cg_solve(src)                       # the context is still usable afterwards
+    assert info["converged"]
 
 
 def test_device_links_upload_equals_host_upload(cola_mod):
