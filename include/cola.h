@@ -88,6 +88,23 @@ const char *cola_last_error(const cola_ctx *c);
  * (all right-hand sides of a launch) exceed this budget the thread blocks sweep the lattice in bands of z-planes
  * instead of slice by slice, which keeps the reuse inside L2.  Results do not depend on it. */
 cola_status cola_set_l2_budget(cola_ctx *c, size_t bytes);
+/* Optional parts of the workspace (the fields are ~7.3 KB per even site with everything on: 125 GB at 64^3x128).
+ * Call before cola_workspace_bytes / cola_set_workspace (it un-lends the workspace and invalidates the gauge field).
+ * Default: COLA_FEAT_ALL.
+ *   COLA_FEAT_FULL_M  fp32 (and fp16) copies of A on the ODD parity and the larger solver scratch: needed by
+ *                     cola_fermion_matrix_apply* in COLA_F32 / COLA_F32_H16 and by solves with even_odd = 0.  The fp64
+ *                     operator on the full lattice is always available (the true residual |b - M x| needs it).
+ *   COLA_FEAT_H16     16-bit links + fp16 clover: COLA_F32_H16 operators and mixed = 2.
+ * A call that needs a missing feature returns COLA_EINVAL. */
+typedef enum { COLA_FEAT_FULL_M = 1, COLA_FEAT_H16 = 2, COLA_FEAT_ALL = 3 } cola_feature;
+cola_status cola_set_features(cola_ctx *c, unsigned features);
+/* Tuning: which kernel family the single-right-hand-side fp32 / 16-bit operators use.  0: every thread loads its 8
+ * neighbour spinors from global memory through L1; 1: a thread block owns a 4-D tile of sites and stages the tile's
+ * input spinors and its six faces in shared memory with cp.async, so that neighbours are read with LDS (BJ:ns
+ * "shared-memory ... staging of neighbour half-spinors").  Operator results are bit-identical in
+ * both modes (fused norms differ in summation order).  fp64 operators and lattices the tiles do not fit (X > 512) use
+ * mode 0 regardless.  Default: DESIGN.md section 6 says which and why. */
+cola_status cola_set_staging(cola_ctx *c, int mode);
 /* Change the stream subsequent calls launch on. */
 cola_status cola_set_stream(cola_ctx *c, void *stream);
 
@@ -104,12 +121,19 @@ cola_status cola_set_workspace(cola_ctx *c, void *dev_ptr, size_t bytes);
  * (fp64 18 reals; fp32 18 or 12 reals), build the clover field A from the four-leaf field
  * strength, invert its 6x6 blocks on the odd parity, make fp32 copies.  Links stay pure SU(3)
  * (no boundary sign folded in).  host_links: HOST pointer, 4*V*18 doubles.
- * With compress12, links with max|U U^+ - 1| > 1e-10 are rejected with COLA_EINVAL. */
+ * With compress12, links with max|U U^+ - 1| > 1e-10 are rejected with COLA_EINVAL.  Without compress12 such links
+ * are accepted for the fp64 and fp32 x18 operators, but their 16-bit copy (always 12 reals, third row rebuilt) would be
+ * wrong: COLA_F32_H16 operators and mixed = 2 solves then return COLA_EINVAL.
+ * COLA_EINVAL also if a 6x6 block of A on the odd parity is not positive definite (a Gauss-Jordan pivot <= 0;
+ * SURVEY O6 expects eigenvalues in about [0.74, 1.26] for the configs): the Schur complement needs A_oo^-1. */
 cola_status cola_gauge_upload(cola_ctx *c, const double *host_links);
 /* Same, from a DEVICE pointer (e.g. links generated on the GPU for the 64^3x128 case). */
 cola_status cola_gauge_upload_dev(cola_ctx *c, const double *dev_links);
 /* Diagnostics of the last upload: max |U U^+ - 1| over all links. */
 cola_status cola_gauge_info(const cola_ctx *c, double *max_unitarity_dev);
+/* Diagnostics of the last upload (SURVEY O6 "report the smallest pivot it meets"): the smallest pivot of the unpivoted
+ * Gauss-Jordan inversions of the 6x6 blocks of A_oo.  Valid (and <= 0) also after an upload that failed for it. */
+cola_status cola_clover_info(const cola_ctx *c, double *min_pivot);
 
 /* Tests of H1/H2: expand the packed fp64 clover field to canonical 12x12 blocks.
  * which = 0: A on all sites.  which = 1: A^-1 on odd sites, zero blocks on even sites.
@@ -120,7 +144,8 @@ cola_status cola_clover_unpack(cola_ctx *c, int which, void *canon_dev);
  * DEVICE buffer of the same precision. */
 cola_status cola_spinor_pack(cola_ctx *c, cola_prec prec, const void *canon_dev, void *internal_dev);
 cola_status cola_spinor_unpack(cola_ctx *c, cola_prec prec, const void *internal_dev, void *canon_dev);
-/* Internal fp64 <-> internal fp32 (round to nearest even), n_half = 1 (half lattice) or 2 (full). */
+/* Internal fp64 <-> internal fp32 (round to nearest even), n_half = 1 (half lattice) or 2 (full).
+ * cola_spinor_pack / unpack / convert take COLA_F64 or COLA_F32 only (COLA_EINVAL otherwise). */
 cola_status cola_spinor_convert(cola_ctx *c, cola_prec dst_prec, const void *src_dev, void *dst_dev, int n_half);
 
 /* H3-H5, parity dslash: out_p = D_{p,1-p} in_{1-p}.  in, out: internal half-lattice DEVICE buffers
@@ -159,9 +184,12 @@ cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *
 
 /* Same solve, also recording the residual history of the recurrence: resid_hist_host[k] = |r_{k+1}| / |b| after CGLS
  * pass k (k < min(info->iters, hist_len)); HOST array of hist_len doubles.  In the mixed modes this is the fp32
- * recurrence's residual (the value the reliable-update test sees), before a reliable update replaces it. */
+ * recurrence's residual (the value the reliable-update test sees), before a reliable update replaces it.
+ * update_iters_host (HOST, may be NULL): receives the 1-based pass numbers after which the reliable updates fired
+ * (the first min(info->reliable_updates, update_len) of them) -- SURVEY O8's schedule, compared in the tests with the
+ * rule applied to the oracle's fp64 history. */
 cola_status cola_cg_solve_history(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info,
-                                  double *resid_hist_host, int hist_len);
+                                  double *resid_hist_host, int hist_len, int *update_iters_host, int update_len);
 
 /* End-to-end variants: HOST canonical buffers; the host<->device copies are part of the call. */
 cola_status cola_dslash_apply_host(cola_ctx *c, cola_prec prec, cola_parity out_parity, const void *in_canon_host, void *out_canon_host);
@@ -175,10 +203,12 @@ cola_status cola_cg_solve_host(cola_ctx *c, const cola_solve_params *sp, const v
  * Per vector the arithmetic, its order and hence the result are those of the single-rhs entry points.
  * "nrhs vectors" = nrhs internal buffers of the stated size stored back to back.
  *
- * Workspace: a second caller-owned DEVICE buffer holding, per right-hand side, the Schur temporaries and the vectors
- * of the batched solver (5.5 fp64 half-lattice vectors).  Borrowed until cola_destroy / the next call;
- * cola_set_mrhs_workspace(c, NULL, 0, 0) gives it back. */
-size_t cola_mrhs_workspace_bytes(const cola_ctx *c, int nrhs);
+ * Workspace: a second caller-owned DEVICE buffer holding, per right-hand side, the Schur temporaries (1.5 fp64
+ * half-lattice vectors: enough for the cola_*_apply_mrhs operators, for_solver = 0) and, with for_solver != 0, the
+ * vectors of the batched solver as well (5.5 fp64 half-lattice vectors).  cola_set_mrhs_workspace accepts either size;
+ * cola_cg_solve_mrhs returns COLA_ENOTREADY on an operators-only workspace.  Borrowed until cola_destroy / the next
+ * call; cola_set_mrhs_workspace(c, NULL, 0, 0) gives it back. */
+size_t cola_mrhs_workspace_bytes(const cola_ctx *c, int nrhs, int for_solver);
 cola_status cola_set_mrhs_workspace(cola_ctx *c, void *dev_ptr, size_t bytes, int nrhs);
 /* out_p[n] = D_{p,1-p} in[n]: nrhs half-lattice internal DEVICE vectors each, no overlap. */
 cola_status cola_dslash_apply_mrhs(cola_ctx *c, cola_prec prec, cola_parity out_parity, int nrhs, const void *in_dev, void *out_dev);

@@ -768,6 +768,10 @@ int oracle_cgnr(const int *L, const int *bc, const double *U_, const double *A_,
  * |r32| <= tol*|b|:  x64 += x32; x32 = 0; r64 = rhs - K x64 (double); r32 = float(r64);
  * r_max = |r64|; continue with the SAME p.  Terminate on the fp64 residual only.
  * Used for iteration-count comparison; reference results stay those of oracle_cgnr.
+ * Outputs that expose the schedule (no effect on the arithmetic): resid_hist[k] = |r32_{k+1}|/|b| of the
+ * recurrence as the delta test sees it (before an update replaces it), k < iterations; update_iters[j] = the
+ * iteration count `it` (1-based) at which the j-th reliable update fired, j < min(updates, max_updates).
+ * tests/test_oracle_pins.py pins the schedule against the rule applied to oracle_cgnr's fp64 history.
  * ---------------------------------------------------------------------------------------- */
 static void round_to_float(long n, cplx *v)
 {
@@ -776,7 +780,8 @@ static void round_to_float(long n, cplx *v)
 
 int oracle_cgnr_mixed(const int *L, const int *bc, const double *U_, const double *A_, const double *Ainv_,
                       double kappa, int even_odd, const double *b_, double *x_, double tol, double delta,
-                      int max_iter, int *iters_out, int *updates_out, double *true_resid_out)
+                      int max_iter, int *iters_out, int *updates_out, double *true_resid_out,
+                      double *resid_hist, int *update_iters, int max_updates)
 {
     long V = vol(L), n = 12 * V;
     op_ctx_t o = {L, bc, U_, A_, Ainv_, kappa, even_odd};
@@ -802,9 +807,11 @@ int oracle_cgnr_mixed(const int *L, const int *bc, const double *U_, const doubl
         for (long k = 0; k < n; k++) { xl[k] += alpha * p[k]; r[k] -= alpha * q[k]; }
         round_to_float(n, xl); round_to_float(n, r);
         double rn = sqrt(norm2(n, r));
+        if (resid_hist) resid_hist[it] = rn / bnorm;
         it++;
         if (rn > rmax) rmax = rn;
         if (rn < delta * rmax || rn <= tol * bnorm) {
+            if (update_iters && updates < max_updates) update_iters[updates] = it;
             for (long k = 0; k < n; k++) { x[k] += xl[k]; xl[k] = 0; }
             apply_K(&o, 0, x, q);                       /* double */
             for (long k = 0; k < n; k++) r[k] = rhs[k] - q[k];
@@ -829,6 +836,79 @@ int oracle_cgnr_mixed(const int *L, const int *bc, const double *U_, const doubl
     if (iters_out) *iters_out = it;
     if (updates_out) *updates_out = updates;
     free(rhs); free(r); free(p); free(q); free(s); free(xl);
+    return status;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * BiCGStab ("other Krylov variants (BiCGStab on S)"; "solvers for linear systems") for
+ * K x = b, K = M (even_odd = 0) or K = S with b = bhat_e (even_odd = 1), in van der Vorst's order, unpreconditioned,
+ * x0 = 0, shadow residual rhat = r0:
+ *   rho_0 = alpha = omega_0 = 1; v_0 = p_0 = 0
+ *   for i = 1, 2, ...:
+ *     rho_i = <rhat, r_{i-1}>;  beta = (rho_i / rho_{i-1}) (alpha / omega_{i-1});
+ *     p_i = r_{i-1} + beta (p_{i-1} - omega_{i-1} v_{i-1});   v_i = K p_i;   alpha = rho_i / <rhat, v_i>;
+ *     s = r_{i-1} - alpha v_i;   t = K s;   omega_i = <t, s> / <t, t>;
+ *     x_i = x_{i-1} + alpha p_i + omega_i s;   r_i = s - omega_i t;   stop if |r_i| <= tol |b_full|
+ * with <a, b> = sum conj(a) b.  One pass = two applications of K.  resid_hist[i-1] = |r_i| / |b_full|.  After the loop
+ * the full-lattice true residual |b - M x| / |b| is recomputed with O5, as in oracle_cgnr.
+ * returns 0 if converged, 1 if max_iter was hit, 2 on breakdown (rho, <rhat, v> or <t, t> exactly 0).
+ * ---------------------------------------------------------------------------------------- */
+static cplx cdot(long n, const cplx *a, const cplx *b)
+{
+    double re = 0, im = 0;
+    for (long k = 0; k < n; k++) {
+        re += creal(a[k]) * creal(b[k]) + cimag(a[k]) * cimag(b[k]);
+        im += creal(a[k]) * cimag(b[k]) - cimag(a[k]) * creal(b[k]);
+    }
+    return re + I * im;
+}
+
+int oracle_bicgstab(const int *L, const int *bc, const double *U_, const double *A_, const double *Ainv_,
+                    double kappa, int even_odd, const double *b_, double *x_, double tol, int max_iter,
+                    int *iters_out, double *resid_hist, double *true_resid_out)
+{
+    long V = vol(L), n = 12 * V;
+    op_ctx_t o = {L, bc, U_, A_, Ainv_, kappa, even_odd};
+    const cplx *b = (const cplx *)b_;
+    cplx *x = (cplx *)x_;
+    cplx *r = (cplx *)malloc(sizeof(cplx) * n), *rhat = (cplx *)malloc(sizeof(cplx) * n);
+    cplx *p = (cplx *)malloc(sizeof(cplx) * n), *v = (cplx *)malloc(sizeof(cplx) * n);
+    cplx *sv = (cplx *)malloc(sizeof(cplx) * n), *t = (cplx *)malloc(sizeof(cplx) * n);
+    double bnorm = sqrt(norm2(n, b));
+    if (even_odd) oracle_eo_prepare(L, bc, U_, Ainv_, kappa, b_, (double *)r);
+    else memcpy(r, b, sizeof(cplx) * n);
+    memcpy(rhat, r, sizeof(cplx) * n);
+    for (long k = 0; k < n; k++) { x[k] = 0; p[k] = 0; v[k] = 0; }
+    cplx rho = 1, alpha = 1, omega = 1;
+    int it = 0, status = 1;
+    if (sqrt(norm2(n, r)) <= tol * bnorm) status = 0;
+    while (status == 1 && it < max_iter) {
+        cplx rho_new = cdot(n, rhat, r);
+        if (rho_new == 0) { status = 2; break; }
+        cplx beta = (rho_new / rho) * (alpha / omega);
+        rho = rho_new;
+        for (long k = 0; k < n; k++) p[k] = r[k] + beta * (p[k] - omega * v[k]);
+        apply_K(&o, 0, p, v);
+        cplx rv = cdot(n, rhat, v);
+        if (rv == 0) { status = 2; break; }
+        alpha = rho / rv;
+        for (long k = 0; k < n; k++) sv[k] = r[k] - alpha * v[k];
+        apply_K(&o, 0, sv, t);
+        double tt = norm2(n, t);
+        if (tt == 0) { status = 2; break; }
+        omega = cdot(n, t, sv) / tt;
+        for (long k = 0; k < n; k++) { x[k] += alpha * p[k] + omega * sv[k]; r[k] = sv[k] - omega * t[k]; }
+        double rn = sqrt(norm2(n, r));
+        if (resid_hist) resid_hist[it] = rn / bnorm;
+        it++;
+        if (rn <= tol * bnorm) { status = 0; break; }
+    }
+    if (even_odd) oracle_eo_reconstruct(L, bc, U_, Ainv_, kappa, b_, x_);
+    oracle_M(L, bc, U_, A_, kappa, 0, x_, (double *)t);
+    for (long k = 0; k < n; k++) t[k] = b[k] - t[k];
+    if (true_resid_out) *true_resid_out = sqrt(norm2(n, t)) / bnorm;
+    if (iters_out) *iters_out = it;
+    free(r); free(rhat); free(p); free(v); free(sv); free(t);
     return status;
 }
 

@@ -18,7 +18,7 @@ _LIB = os.path.join(_HERE, "libcola_oracle.so")
 
 __all__ = [
     "build", "gamma", "sigma", "hop", "dslash_parity", "field_strength", "clover", "clover_inverse",
-    "block_apply", "M", "schur", "eo_prepare", "eo_reconstruct", "apply_sites", "cgnr", "cgnr_mixed",
+    "block_apply", "M", "schur", "eo_prepare", "eo_reconstruct", "apply_sites", "cgnr", "cgnr_mixed", "bicgstab",
     "dense_inverse", "num_threads", "parity_mask",
 ]
 
@@ -45,6 +45,7 @@ def _L():
         _lib.oracle_dense_inverse.restype = ctypes.c_int
         _lib.oracle_cgnr.restype = ctypes.c_int
         _lib.oracle_cgnr_mixed.restype = ctypes.c_int
+        _lib.oracle_bicgstab.restype = ctypes.c_int
         _lib.oracle_num_threads.restype = ctypes.c_int
     return _lib
 
@@ -218,9 +219,32 @@ def cgnr_mixed(dims, bc, U, A, Ainv, kappa: float, b, even_odd: bool, tol: float
     iters = ctypes.c_int(0)
     updates = ctypes.c_int(0)
     true_res = ctypes.c_double(0.0)
+    hist = np.zeros(max_iter, dtype=np.float64)
+    max_updates = 256
+    upd = np.zeros(max_updates, dtype=np.int32)
     st = _L().oracle_cgnr_mixed(_i4(dims), _i4(bc), _p(U), _p(A), _p(Ainv), ctypes.c_double(kappa),
                                 ctypes.c_int(int(even_odd)), _p(b), _p(x), ctypes.c_double(tol),
                                 ctypes.c_double(delta), ctypes.c_int(max_iter), ctypes.byref(iters),
-                                ctypes.byref(updates), ctypes.byref(true_res))
+                                ctypes.byref(updates), ctypes.byref(true_res),
+                                hist.ctypes.data_as(ctypes.c_void_p), upd.ctypes.data_as(ctypes.c_void_p),
+                                ctypes.c_int(max_updates))
     return dict(x=x, iters=iters.value, updates=updates.value, converged=(st == 0),
-                true_residual=true_res.value)
+                true_residual=true_res.value, history=hist[: iters.value].copy(),
+                update_iters=[int(v) for v in upd[: min(updates.value, max_updates)]])
+
+
+def bicgstab(dims, bc, U, A, Ainv, kappa: float, b, even_odd: bool, tol: float = 1e-10, max_iter: int = 20000):
+    """BiCGStab in van der Vorst's order on M or on the Schur system.
+    Returns dict(x, iters, converged, breakdown, true_residual, history); one iteration = two operator applications."""
+    U, A, b = _c(U), _c(A), _c(b)
+    Ainv = _c(Ainv) if Ainv is not None else A
+    x = np.zeros_like(b)
+    iters = ctypes.c_int(0)
+    true_res = ctypes.c_double(0.0)
+    hist = np.zeros(max_iter, dtype=np.float64)
+    st = _L().oracle_bicgstab(_i4(dims), _i4(bc), _p(U), _p(A), _p(Ainv), ctypes.c_double(kappa),
+                              ctypes.c_int(int(even_odd)), _p(b), _p(x), ctypes.c_double(tol),
+                              ctypes.c_int(max_iter), ctypes.byref(iters), hist.ctypes.data_as(ctypes.c_void_p),
+                              ctypes.byref(true_res))
+    return dict(x=x, iters=iters.value, converged=(st == 0), breakdown=(st == 2), true_residual=true_res.value,
+                history=hist[: iters.value].copy())

@@ -17,6 +17,7 @@ _LIB_PATH = os.environ.get("COLA_LIBRARY_PATH") or os.path.join(_HERE, "libcola.
 COLA_OK, COLA_EINVAL, COLA_ECUDA, COLA_ENOTREADY, COLA_ENOCONV, COLA_ENOMEM = range(6)
 COLA_F64, COLA_F32, COLA_F32_H16 = 0, 1, 2
 COLA_EVEN, COLA_ODD = 0, 1
+COLA_FEAT_FULL_M, COLA_FEAT_H16, COLA_FEAT_ALL = 1, 2, 3
 STATUS_NAMES = {0: "COLA_OK", 1: "COLA_EINVAL", 2: "COLA_ECUDA", 3: "COLA_ENOTREADY", 4: "COLA_ENOCONV", 5: "COLA_ENOMEM"}
 
 EXPORTS = [
@@ -28,6 +29,7 @@ EXPORTS = [
     "cola_launch_count",
     "cola_mrhs_workspace_bytes", "cola_set_mrhs_workspace", "cola_dslash_apply_mrhs", "cola_fermion_matrix_apply_mrhs",
     "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host", "cola_cg_solve_history", "cola_profile_kernel", "cola_profile_result",
+    "cola_set_features", "cola_clover_info", "cola_set_staging",
 ]
 
 
@@ -70,7 +72,11 @@ def _load():
     lib.cola_selftest_host.argtypes = [ctypes.c_char_p, ctypes.c_size_t]
     lib.cola_profile_kernel.argtypes = [vp, ci]
     lib.cola_profile_result.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(ci)]
-    lib.cola_cg_solve_history.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo), ctypes.POINTER(cd), ci]
+    lib.cola_cg_solve_history.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo), ctypes.POINTER(cd), ci,
+                                          ctypes.POINTER(ci), ci]
+    lib.cola_set_features.argtypes = [vp, ctypes.c_uint]
+    lib.cola_set_staging.argtypes = [vp, ci]
+    lib.cola_clover_info.argtypes = [vp, ctypes.POINTER(cd)]
     lib.cola_spinor_bytes.argtypes = [vp, ci, ci]
     lib.cola_spinor_bytes.restype = ctypes.c_size_t
     lib.cola_workspace_bytes.argtypes = [vp]
@@ -92,7 +98,7 @@ def _load():
     lib.cola_cg_solve_host.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo)]
     lib.cola_launch_count.argtypes = [vp]
     lib.cola_launch_count.restype = ctypes.c_ulonglong
-    lib.cola_mrhs_workspace_bytes.argtypes = [vp, ci]
+    lib.cola_mrhs_workspace_bytes.argtypes = [vp, ci, ci]
     lib.cola_mrhs_workspace_bytes.restype = ctypes.c_size_t
     lib.cola_set_mrhs_workspace.argtypes = [vp, vp, ctypes.c_size_t, ci]
     lib.cola_dslash_apply_mrhs.argtypes = [vp, ci, ci, ci, vp, vp]
@@ -133,13 +139,14 @@ _CPLX = {COLA_F64: torch.complex128, COLA_F32: torch.complex64}
 class Cola:
     """One lattice context.  Method names mirror the C entry points (cola_<name>)."""
 
-    def __init__(self, dims, kappa, csw, bc=(1, 1, 1, -1), compress12=True, trace_sub=True, device=0, stream=None):
+    def __init__(self, dims, kappa, csw, bc=(1, 1, 1, -1), compress12=True, trace_sub=True, device=0, stream=None, features=None):
         self.dims = tuple(int(d) for d in dims)
         self.device = torch.device("cuda", device)
         self._h = ctypes.c_void_p()
         self._ws = None
         self._mws = None
         self._mws_nrhs = 0
+        self._mws_solver = False
         p = ColaParams()
         p.dims[:] = self.dims
         p.kappa, p.csw = float(kappa), float(csw)
@@ -155,6 +162,8 @@ class Cola:
         self.V = lx * ly * lz * lt
         self.Vh = self.V // 2
         self.kappa, self.csw = float(kappa), float(csw)
+        if features is not None:
+            self.set_features(features)
 
     # ---- plumbing
     def _ck(self, st, ok=(COLA_OK,)):
@@ -188,6 +197,21 @@ class Cola:
     def set_l2_budget(self, nbytes: int = 0):
         """Bytes of L2 the sweep order counts on for neighbour reuse (0: default 40 MB); tuning only, results unchanged."""
         self._ck(_lib.cola_set_l2_budget(self._h, int(nbytes)))
+
+    def set_staging(self, mode: int):
+        """0: neighbour spinors through L1; 1: staged in shared memory per 4-D tile (fp32 / 16-bit single-rhs kernels)."""
+        self._ck(_lib.cola_set_staging(self._h, int(mode)))
+
+    def set_features(self, features: int):
+        """COLA_FEAT_* parts of the workspace to carve; call before set_workspace / gauge_upload."""
+        self._ck(_lib.cola_set_features(self._h, int(features)))
+        self._ws = None
+
+    def clover_info(self) -> float:
+        """Smallest Gauss-Jordan pivot of the 6x6 inverses of the last upload."""
+        v = ctypes.c_double()
+        self._ck(_lib.cola_clover_info(self._h, ctypes.byref(v)))
+        return v.value
 
     def set_stream(self, stream):
         self._ck(_lib.cola_set_stream(self._h, ctypes.c_void_p(stream)))
@@ -338,11 +362,13 @@ class Cola:
         sp = self._solve_params(tol, max_iter, even_odd, mixed, delta)
         info = ColaSolveInfo()
         hist = (ctypes.c_double * hist_len)()
+        upd = (ctypes.c_int * 256)()
         st = _lib.cola_cg_solve_history(self._h, ctypes.byref(sp), ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), ctypes.byref(info),
-                                        hist, hist_len)
+                                        hist, hist_len, upd, 256)
         self._ck(st, ok=(COLA_OK, COLA_ENOCONV))
         d = self._info_dict(info, st)
         d["history"] = [hist[k] for k in range(min(info.iters, hist_len))]
+        d["update_iters"] = [upd[k] for k in range(min(info.reliable_updates, 256))]
         return x, d
 
     def cg_solve_host(self, b: torch.Tensor, **kw):
@@ -366,25 +392,27 @@ class Cola:
         return out
 
     # ---- multi-right-hand-side operators and batched solver
-    def mrhs_workspace_bytes(self, nrhs: int) -> int:
-        return int(_lib.cola_mrhs_workspace_bytes(self._h, int(nrhs)))
+    def mrhs_workspace_bytes(self, nrhs: int, for_solver: bool = True) -> int:
+        return int(_lib.cola_mrhs_workspace_bytes(self._h, int(nrhs), int(bool(for_solver))))
 
-    def set_mrhs_workspace(self, nrhs: int, tensor: torch.Tensor | None = None):
-        """Lend the per-right-hand-side workspace (allocated here with torch if not given)."""
+    def set_mrhs_workspace(self, nrhs: int, tensor: torch.Tensor | None = None, for_solver: bool = True):
+        """Lend the per-right-hand-side workspace (allocated here with torch if not given); for_solver=False sizes it for
+        the multi-rhs operators only."""
         if tensor is None:
             self.release_mrhs_workspace()
-            tensor = torch.empty(self.mrhs_workspace_bytes(nrhs), dtype=torch.uint8, device=self.device)
+            tensor = torch.empty(self.mrhs_workspace_bytes(nrhs, for_solver), dtype=torch.uint8, device=self.device)
         self._ck(_lib.cola_set_mrhs_workspace(self._h, ctypes.c_void_p(tensor.data_ptr()), tensor.numel() * tensor.element_size(), int(nrhs)))
         self._mws, self._mws_nrhs = tensor, int(nrhs)
+        self._mws_solver = tensor.numel() * tensor.element_size() >= self.mrhs_workspace_bytes(nrhs, True)
         return tensor
 
     def release_mrhs_workspace(self):
         self._ck(_lib.cola_set_mrhs_workspace(self._h, None, 0, 0))
-        self._mws, self._mws_nrhs = None, 0
+        self._mws, self._mws_nrhs, self._mws_solver = None, 0, False
 
-    def _need_mrhs(self, nrhs):
-        if self._mws is None or self._mws_nrhs < nrhs:
-            self.set_mrhs_workspace(nrhs)
+    def _need_mrhs(self, nrhs, for_solver=False):
+        if self._mws is None or self._mws_nrhs < nrhs or (for_solver and not self._mws_solver):
+            self.set_mrhs_workspace(nrhs, for_solver=for_solver)
 
     def empty_internal_mrhs(self, nrhs, prec, full=True) -> torch.Tensor:
         """nrhs internal buffers back to back: shape (nrhs,) + the shape of empty_internal."""
@@ -424,7 +452,7 @@ class Cola:
         assert b.is_cuda and b.dtype == torch.complex128 and b.dim() == 7 and b[0].numel() == self.V * 12
         b = b.contiguous()
         nrhs = b.shape[0]
-        self._need_mrhs(nrhs)
+        self._need_mrhs(nrhs, for_solver=True)
         if x is None:
             x = torch.empty_like(b)
         sp = self._solve_params(tol, max_iter, True, mixed, delta)

@@ -1,5 +1,6 @@
 // cola_api.cu -- the C ABI of include/cola.h: context, workspace carving, gauge upload (H0-H2),
 // operator entry points (H3-H8) and the CGNR / mixed-precision solvers (H9-H12).
+#include <float.h>
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
@@ -22,13 +23,19 @@ struct cola_ctx {
     char *clovA64, *clovA32;        // [parity][chunk][Vh]
     char *clovI64, *clovI32;        // odd parity only
     char *gauge16, *clovA16, *clovI16;   // 16-bit copies for COLA_F32_H16 (same index structure)
+    unsigned features;              // COLA_FEAT_* parts of the workspace that are carved (cola_set_features)
+    int h16_valid;                  // the 16-bit link copy holds what the kernels assume (12 reals of a unitary matrix)
     int sloppy16;                   // the running solve's inner operator reads the 16-bit fields
     double *hist;                   // HOST array of the running solve's residual history or nullptr (cola_cg_solve_history)
     int hist_len;
+    int *upd_iters;                 // HOST array receiving the iterations at which reliable updates fired, or nullptr
+    int upd_len;
     // optional in-solve timing of the dominant kernel (cola_profile_kernel): event pairs around each launch of the
     // fused dslash + clover + xpay kernel of the inner precision
     int prof_on, prof_n;
     cudaEvent_t *prof_ev;           // 2 * PROF_MAX events, created on first use
+    int prof_created;               // how many of them exist
+    int staging;                    // 1: fp32 / 16-bit single-rhs kernels stage neighbour spinors in shared memory (cola_set_staging)
     size_t l2_budget;               // bytes of L2 the sweep order counts on for neighbour reuse (cola_set_l2_budget)
     char *tmp64, *tmp32;            // odd half-lattice temporaries of the Schur operator
     ReduceWs red;                   // deterministic-reduction buffers
@@ -38,11 +45,14 @@ struct cola_ctx {
     // owned
     Ctl *ctl;                       // device
     unsigned long long *max_dev_bits;   // device (inside the same allocation)
+    unsigned long long *min_pivot_key;  // device (inside the same allocation): see launch_clover_invert
+    double min_pivot;               // smallest Gauss-Jordan pivot of the 6x6 inverses of the last upload
     double *h_pinned;               // pinned host scalars
     HostStatus *h_status;           // mapped pinned host memory the device publishes the iteration status to
     HostStatus *d_status;           // device alias of h_status
     // multi-right-hand-side workspace (borrowed, cola_set_mrhs_workspace) and control state
     int m_nrhs;                     // capacity in right-hand sides (0: none)
+    int m_solver;                   // the workspace also holds the batched solver's vectors
     char *m_tmp32;                  // [m_nrhs] odd half temporaries of the fp32 Schur operator
     char *m_r64;                    // [m_nrhs] fp64 half vectors: Schur temporary of the operator API; r of the batched solver
     char *m_rhs, *m_qs;             // [m_nrhs] fp64 half vectors: prepared sources, K x of the reliable updates
@@ -78,9 +88,24 @@ static cola_status fail(cola_ctx *c, cola_status st, const char *fmt, const char
         if (s__ != COLA_OK) return s__;   \
     } while (0)
 
+static inline void cpu_relax()
+{
+#if defined(__x86_64__) || defined(__i386__)
+    __builtin_ia32_pause();
+#elif defined(__aarch64__)
+    asm volatile("yield" ::: "memory");
+#else
+    __sync_synchronize();
+#endif
+}
+
 static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 static size_t half_bytes(const cola_ctx *c, cola_prec prec) { return c->Vh * 24 * (prec == COLA_F64 ? 8 : 4); }   // COLA_F32_H16: fp32 spinors
-static const size_t SCRATCH_HALF64 = 12;   // solver scratch in units of one fp64 half-lattice spinor
+// Solver scratch in units of one fp64 half-lattice spinor.  Even-odd solves use at most 9 slots (source 2, solution 2,
+// prepared source 1, r 1, K x 1, four fp32 vectors 2), solves on M at most 12 (mixed: r 2, K x 2, four fp32 vectors 4).
+// The *_host entry points need no more: the canonical source is staged where the solution will live and the canonical
+// solution is written over the packed source once it is dead (cola_cg_solve_host).
+static size_t scratch_half64(const cola_ctx *c) { return (c->features & COLA_FEAT_FULL_M) ? 12 : 9; }
 
 struct Carve {
     size_t gauge64, gauge32, clovA64, clovA32, clovI64, clovI32, gauge16, clovA16, clovI16, tmp64, tmp32, partials, scratch, total;
@@ -92,15 +117,17 @@ static Carve carve(const cola_ctx *c)
     size_t off = 0;
     const size_t Vh = c->Vh;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    const size_t npar = (c->features & COLA_FEAT_FULL_M) ? 2 : 1;   // parities the fp32 / fp16 copies of A cover
+    const size_t h16 = (c->features & COLA_FEAT_H16) ? 1 : 0;
     k.gauge64 = take(8 * 144 * Vh);
     k.gauge32 = take(8 * link_bytes(c->fmt32) * Vh);
-    k.clovA64 = take(2 * 576 * Vh);
-    k.clovA32 = take(2 * 288 * Vh);
+    k.clovA64 = take(2 * 576 * Vh);         // fp64 A on both parities: the true residual is always |b - M x| on the full lattice
+    k.clovA32 = take(npar * 288 * Vh);
     k.clovI64 = take(576 * Vh);
     k.clovI32 = take(288 * Vh);
-    k.gauge16 = take(8 * link_bytes(LINK_I16_12) * Vh);
-    k.clovA16 = take(2 * CLOVER_H16_BYTES * Vh);
-    k.clovI16 = take(CLOVER_H16_BYTES * Vh);
+    k.gauge16 = take(h16 * 8 * link_bytes(LINK_I16_12) * Vh);
+    k.clovA16 = take(h16 * npar * CLOVER_H16_BYTES * Vh);
+    k.clovI16 = take(h16 * CLOVER_H16_BYTES * Vh);
     k.tmp64 = take(192 * Vh);
     k.tmp32 = take(96 * Vh);
     {
@@ -108,7 +135,7 @@ static Carve carve(const cola_ctx *c)
         if (nb < (size_t)blas_max_blocks()) nb = (size_t)blas_max_blocks();
         k.partials = take((nb + reduce_groups(nb)) * sizeof(double) + reduce_groups(nb) * sizeof(unsigned));
     }
-    k.scratch = take(SCRATCH_HALF64 * 192 * Vh);
+    k.scratch = take(scratch_half64(c) * 192 * Vh);
     k.total = off;
     return k;
 }
@@ -144,6 +171,7 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     for (int k = 0; k < 4; k++) c->g.bc[k] = p->bc[k];
     c->fmt32 = p->compress12 ? LINK_F32_12 : LINK_F32_18;
     c->l2_budget = (size_t)40 << 20;
+    c->features = COLA_FEAT_ALL;
     c->stream = (cudaStream_t)p->stream;
     char *blk = nullptr;
     cudaError_t e = cudaMalloc(&blk, 4096);
@@ -161,12 +189,16 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     if (e != cudaSuccess) {
         fail(nullptr, COLA_ECUDA, "cola_create: %s", cudaGetErrorString(e));
         if (blk) cudaFree(blk);
+        if (c->h_pinned) cudaFreeHost(c->h_pinned);
+        if (c->ev0) cudaEventDestroy(c->ev0);
+        if (c->ev1) cudaEventDestroy(c->ev1);
         delete c;
         return COLA_ECUDA;
     }
     c->ctl = reinterpret_cast<Ctl *>(blk);
     c->ctlm = reinterpret_cast<CtlM *>(blk + 512);
     c->max_dev_bits = reinterpret_cast<unsigned long long *>(blk + 2048);
+    c->min_pivot_key = reinterpret_cast<unsigned long long *>(blk + 2056);
     *out = c;
     return COLA_OK;
 }
@@ -181,7 +213,7 @@ cola_status cola_destroy(cola_ctx *c)
     cudaEventDestroy(c->ev0);
     cudaEventDestroy(c->ev1);
     if (c->prof_ev) {
-        for (int k = 0; k < 2 * PROF_MAX; k++) cudaEventDestroy(c->prof_ev[k]);
+        for (int k = 0; k < c->prof_created; k++) cudaEventDestroy(c->prof_ev[k]);
         delete[] c->prof_ev;
     }
     delete c;
@@ -194,9 +226,12 @@ cola_status cola_profile_kernel(cola_ctx *c, int enable)
 {
     if (!c) return COLA_EINVAL;
     CK(cudaSetDevice(c->p.device));
-    if (enable && !c->prof_ev) {
-        c->prof_ev = new cudaEvent_t[2 * PROF_MAX];
-        for (int k = 0; k < 2 * PROF_MAX; k++) CK(cudaEventCreate(&c->prof_ev[k]));
+    if (enable && c->prof_created < 2 * PROF_MAX) {
+        if (!c->prof_ev) {
+            c->prof_ev = new cudaEvent_t[2 * PROF_MAX];
+            memset(c->prof_ev, 0, sizeof(cudaEvent_t) * 2 * PROF_MAX);
+        }
+        for (; c->prof_created < 2 * PROF_MAX; c->prof_created++) CK(cudaEventCreate(&c->prof_ev[c->prof_created]));
     }
     c->prof_on = enable ? 1 : 0;
     c->prof_n = 0;
@@ -245,6 +280,25 @@ cola_status cola_set_l2_budget(cola_ctx *c, size_t bytes)
     return COLA_OK;
 }
 
+cola_status cola_set_features(cola_ctx *c, unsigned features)
+{
+    if (!c) return COLA_EINVAL;
+    if (features & ~(unsigned)COLA_FEAT_ALL) return fail(c, COLA_EINVAL, "cola_set_features: unknown feature bit");
+    c->features = features;
+    c->ws = nullptr;      // the carving changes: the workspace has to be lent again
+    c->ws_bytes = 0;
+    c->ready = 0;
+    return COLA_OK;
+}
+
+cola_status cola_set_staging(cola_ctx *c, int mode)
+{
+    if (!c) return COLA_EINVAL;
+    if (mode < 0 || mode > 1) return fail(c, COLA_EINVAL, "cola_set_staging: mode must be 0 or 1");
+    c->staging = mode;
+    return COLA_OK;
+}
+
 cola_status cola_set_stream(cola_ctx *c, void *stream)
 {
     if (!c) return COLA_EINVAL;
@@ -285,7 +339,8 @@ cola_status cola_set_workspace(cola_ctx *c, void *dev_ptr, size_t bytes)
         if (e != cudaSuccess) return fail(c, COLA_ECUDA, "cola_set_workspace: %s", cudaGetErrorString(e));
     }
     c->scratch = c->ws + k.scratch;
-    c->scratch_bytes = SCRATCH_HALF64 * 192 * c->Vh;
+    c->scratch_bytes = scratch_half64(c) * 192 * c->Vh;
+    if (!(c->features & COLA_FEAT_H16)) c->gauge16 = c->clovA16 = c->clovI16 = nullptr;
     return COLA_OK;
 }
 
@@ -318,11 +373,26 @@ static char *clovA_of(const cola_ctx *c, cola_prec prec, int parity)
 static char *clovI_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? c->clovI64 : (prec == COLA_F32_H16 ? c->clovI16 : c->clovI32); }
 static char *tmp_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? c->tmp64 : c->tmp32; }
 
+// Is the operator of precision `prec` available with the carved features / the uploaded links?  uses_A: the launch
+// reads A on `parity` (the fp32 / fp16 copies of A_oo exist only with COLA_FEAT_FULL_M).
+static cola_status check_prec(cola_ctx *c, cola_prec prec, int parity, int uses_A)
+{
+    if ((int)prec < 0 || (int)prec > (int)COLA_F32_H16) return fail(c, COLA_EINVAL, "unknown cola_prec");
+    if (prec == COLA_F32_H16) {
+        if (!(c->features & COLA_FEAT_H16)) return fail(c, COLA_EINVAL, "COLA_F32_H16 / mixed = 2 need COLA_FEAT_H16 (cola_set_features)");
+        if (!c->h16_valid)
+            return fail(c, COLA_EINVAL, "COLA_F32_H16 / mixed = 2: the uploaded links are not unitary to 1e-10, so their 16-bit copy (12 reals, third row rebuilt) is wrong");
+    }
+    if (prec != COLA_F64 && uses_A && parity == 1 && !(c->features & COLA_FEAT_FULL_M))
+        return fail(c, COLA_EINVAL, "the fp32 operator on the full lattice needs COLA_FEAT_FULL_M (cola_set_features)");
+    return COLA_OK;
+}
+
 // out_p = [post] ( [A] y + coef * D_{p,1-p} in ), optional |out|^2 -> norm_out
 static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, const void *in, void *out, const void *y, int clov_on_y,
                           double coef, int post_inv, double *norm_out, int norm_accumulate, const int *skip = nullptr)
 {
-    if ((int)prec < 0 || (int)prec > (int)COLA_F32_H16) return fail(c, COLA_EINVAL, "unknown cola_prec");
+    ST(check_prec(c, prec, parity, (y && clov_on_y) ? 1 : 0));
     DslashArgs a;
     memset(&a, 0, sizeof(a));
     a.g = c->g;
@@ -345,9 +415,11 @@ static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, c
         a.norm_accumulate = norm_accumulate;
     }
     if (post_inv && parity != 1) return fail(c, COLA_EINVAL, "internal: A^-1 is stored on the odd parity only");
-    const bool timed = c->prof_on && c->prof_ev && c->prof_n < PROF_MAX && prec != COLA_F64 && a.clov_y;   // Schur kernel 2 / M of the inner precision
+    const bool timed = c->prof_on && c->prof_created == 2 * PROF_MAX && c->prof_n < PROF_MAX && prec != COLA_F64 && a.clov_y;   // Schur kernel 2 / M of the inner precision
     if (timed) CK(cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
-    CK(launch_dslash(fmt_of(c, prec), a, c->stream));
+    cudaError_t le = c->staging ? launch_dslash_tile(fmt_of(c, prec), a, c->stream) : cudaErrorNotSupported;
+    if (le == cudaErrorNotSupported) le = launch_dslash(fmt_of(c, prec), a, c->stream);
+    CK(le);
     if (timed) {
         CK(cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream));
         c->prof_n++;
@@ -402,10 +474,19 @@ static cola_status gauge_finish(cola_ctx *c)
     memcpy(&c->max_unitarity_dev, &bits, sizeof(double));
     if (c->p.compress12 && !(c->max_unitarity_dev <= 1e-10))
         return fail(c, COLA_EINVAL, "cola_gauge_upload: links are not unitary to 1e-10; 12-real compression would be wrong");
-    CK(launch_clover_build(c->g, c->gauge64, c->p.kappa * c->p.csw, c->p.trace_sub, c->clovA64, c->clovA32, c->clovA16, c->stream));
-    CK(launch_clover_invert(c->g, c->clovA64 + 576 * c->Vh, c->clovI64, c->clovI32, c->clovI16, c->stream));
+    // the 16-bit copy stores rows 1 and 2 clamped to [-1, 1] and rebuilds row 3: only right for unitary links
+    c->h16_valid = (c->features & COLA_FEAT_H16) && c->max_unitarity_dev <= 1e-10;
+    CK(launch_clover_build(c->g, c->gauge64, c->p.kappa * c->p.csw, c->p.trace_sub, c->clovA64, c->clovA32, (c->features & COLA_FEAT_FULL_M) ? 2 : 1,
+                           c->clovA16, c->stream));
+    CK(cudaMemsetAsync(c->min_pivot_key, 0xff, sizeof(unsigned long long), c->stream));
+    CK(launch_clover_invert(c->g, c->clovA64 + 576 * c->Vh, c->clovI64, c->clovI32, c->clovI16, c->min_pivot_key, c->stream));
     c->launches += 2;
+    unsigned long long key = 0;
+    CK(cudaMemcpyAsync(&key, c->min_pivot_key, sizeof(key), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
+    c->min_pivot = pivot_from_key(key);
+    if (!(c->min_pivot > 0.0))
+        return fail(c, COLA_EINVAL, "cola_gauge_upload: a 6x6 clover block on the odd parity is not positive definite (pivot <= 0): kappa*csw too large for these links");
     c->ready = 1;
     return COLA_OK;
 }
@@ -479,7 +560,7 @@ cola_status wait_status(cola_ctx *c, int k, HostStatus *out)
             }
             if (e != cudaErrorNotReady) return fail(c, COLA_ECUDA, "cola_cg_solve: %s", cudaGetErrorString(e));
         }
-        __builtin_ia32_pause();
+        cpu_relax();
     }
     __sync_synchronize();
     out->rr = m->rr;
@@ -534,6 +615,9 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
     CK(cudaSetDevice(c->p.device));
     memset(info, 0, sizeof(*info));
     if (sp->mixed < 0 || sp->mixed > 2) return fail(c, COLA_EINVAL, "cola_cg_solve: mixed must be 0, 1 or 2");
+    if (sp->mixed == 2) ST(check_prec(c, COLA_F32_H16, 0, 0));
+    if (!sp->even_odd && !(c->features & COLA_FEAT_FULL_M))
+        return fail(c, COLA_EINVAL, "cola_cg_solve: even_odd = 0 (CGNR on M) needs COLA_FEAT_FULL_M (cola_set_features)");
     c->sloppy16 = sp->mixed == 2;
     const double delta = sp->delta > 0 ? sp->delta : 0.1;
     const double kappa = c->p.kappa;
@@ -571,7 +655,7 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
     double bb = 0.0;
     ST(norm2(c, COLA_F64, B, c->V, &ctl->aux[2]));
     ST(read_scalar(c, &ctl->aux[2], &bb));
-    if (!(bb == bb) || bb > 1e300) return fail(c, COLA_EINVAL, "cola_cg_solve: the source contains NaN or Inf");
+    if (!(bb <= DBL_MAX)) return fail(c, COLA_EINVAL, "cola_cg_solve: the source contains NaN or Inf");
     CK(cudaMemsetAsync(X, 0, 2 * h64, c->stream));
     const double bnorm = sqrt(bb);
     int status_conv = 0;
@@ -623,7 +707,7 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
                 rr = st->rr;
                 iters = k + 1;
                 if (c->hist && k < c->hist_len) c->hist[k] = sqrt(rr) / bnorm;   // |r_{k+1}| / |b| of the recurrence
-                if (!(rr == rr)) {   // NaN/Inf in the source or the links: no test below would ever fire
+                if (!(rr <= DBL_MAX)) {   // NaN/Inf in the source or the links: no test below would ever fire
                     CK(cudaStreamSynchronize(c->stream));
                     return fail(c, COLA_EINVAL, "cola_cg_solve: the residual is not a number (NaN or Inf in the source or the gauge field)");
                 }
@@ -646,7 +730,9 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
                 ST(axpby64(c, sy, r, 1.0, rhs, -1.0, qs, r32));          // r64 = rhs - K x64, r32 = float(r64)
                 ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
                 ST(read_scalar(c, &ctl->rr, &rr));
+                if (c->upd_iters && updates < c->upd_len) c->upd_iters[updates] = k + 1;
                 updates++;
+                if (!(rr <= DBL_MAX)) return fail(c, COLA_EINVAL, "cola_cg_solve: the fp64 residual is not a number (NaN or Inf in the gauge field)");
                 if (rr <= target2) { status_conv = 1; break; }
                 if (!more) break;
                 ST(set_decision_state(c, rr, target2, delta2, k + 1)); // rmax = |r64|, flag down
@@ -706,7 +792,8 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
 namespace {
 
 struct CarveM {
-    size_t tmp32, r64, rhs, qs, x32, r32, p32, q32, partials, total;
+    size_t tmp32, r64, partials, op_total;          // what the multi-rhs operators need
+    size_t rhs, qs, x32, r32, p32, q32, total;      // + the vectors of the batched solver
     int nsb;
 };
 
@@ -718,18 +805,21 @@ CarveM carve_m(const cola_ctx *c, int nrhs)
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     k.tmp32 = take(n * h32);
     k.r64 = take(n * h64);
+    {
+        size_t nsb = (size_t)mrhs_site_blocks(c->g);
+        const size_t nb32 = (size_t)blas_mrhs_blocks(c->Vh, COLA_F32), nb64 = (size_t)blas_mrhs_blocks(c->Vh, COLA_F64);
+        if (nsb < nb32) nsb = nb32;
+        if (nsb < nb64) nsb = nb64;
+        k.nsb = (int)nsb;
+        k.partials = take(n * nsb * sizeof(double));
+    }
+    k.op_total = off;
     k.rhs = take(n * h64);
     k.qs = take(n * h64);
     k.x32 = take(n * h32);
     k.r32 = take(n * h32);
     k.p32 = take(n * h32);
     k.q32 = take(n * h32);
-    size_t nsb = (size_t)mrhs_site_blocks(c->g);
-    const size_t nb32 = (size_t)blas_mrhs_blocks(c->Vh, COLA_F32), nb64 = (size_t)blas_mrhs_blocks(c->Vh, COLA_F64);
-    if (nsb < nb32) nsb = nb32;
-    if (nsb < nb64) nsb = nb64;
-    k.nsb = (int)nsb;
-    k.partials = take(n * nsb * sizeof(double));
     k.total = off;
     return k;
 }
@@ -754,7 +844,7 @@ cola_status dslash_m(cola_ctx *c, cola_prec prec, int parity, int dagger, const 
                      size_t out_stride, const void *y, size_t y_stride, int clov_on_y, double coef, int post_inv, double *norm_out, int norm_accumulate,
                      const int *skip)
 {
-    if ((int)prec < 0 || (int)prec > (int)COLA_F32_H16) return fail(c, COLA_EINVAL, "unknown cola_prec");
+    ST(check_prec(c, prec, parity, (y && clov_on_y) ? 1 : 0));
     MrhsArgs m;
     memset(&m, 0, sizeof(m));
     DslashArgs &a = m.d;
@@ -815,7 +905,7 @@ cola_status wait_status_m(cola_ctx *c, int k, HostStatusM *out)
             }
             if (e != cudaErrorNotReady) return fail(c, COLA_ECUDA, "cola_cg_solve_mrhs: %s", cudaGetErrorString(e));
         }
-        __builtin_ia32_pause();
+        cpu_relax();
     }
     __sync_synchronize();
     for (int n = 0; n < MRHS_MAX; n++) out->rr[n] = m->rr[n];
@@ -866,6 +956,8 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: tol must be > 0 and max_iter >= 1");
     if (!sp->even_odd || sp->mixed < 1 || sp->mixed > 2)
         return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd solver is batched (even_odd = 1, mixed = 1 or 2)");
+    if (sp->mixed == 2) ST(check_prec(c, COLA_F32_H16, 0, 0));
+    if (!c->m_solver) return fail(c, COLA_ENOTREADY, "cola_cg_solve_mrhs: the multi-rhs workspace was sized for operators only (cola_mrhs_workspace_bytes with for_solver = 1)");
     c->sloppy16 = sp->mixed == 2;
     CK(cudaSetDevice(c->p.device));
     const double delta = sp->delta > 0 ? sp->delta : 0.1, kappa = c->p.kappa;
@@ -890,7 +982,7 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
         c->launches++;
         ST(norm2(c, COLA_F64, Bt, c->V, &ctl->aux[2]));
         ST(read_scalar(c, &ctl->aux[2], &bb[n]));
-        if (!(bb[n] == bb[n]) || bb[n] > 1e300) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: a source contains NaN or Inf");
+        if (!(bb[n] <= DBL_MAX)) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: a source contains NaN or Inf");
         bnorm[n] = sqrt(bb[n]);
         CK(cudaMemsetAsync(X, 0, f64, c->stream));
         CK(cudaMemsetAsync(c->m_x32 + (size_t)n * h32, 0, h32, c->stream));
@@ -933,6 +1025,11 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
             HostStatusM hs;
             ST(wait_status_m(c, k, &hs));
             for (int j = 0; j < na; j++) { rr[A[j]] = hs.rr[A[j]]; iters[A[j]] = k + 1; flops[A[j]] += flops_K; }
+            for (int j = 0; j < na; j++)
+                if (!(rr[A[j]] <= DBL_MAX)) {   // NaN/Inf in a source or the links: no trigger would ever fire for that system
+                    CK(cudaStreamSynchronize(c->stream));
+                    return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: a residual is not a number (NaN or Inf in a source or the gauge field)");
+                }
             if (!hs.flag) {
                 for (int j = 0; j < na; j++) flops[A[j]] += flops_K;
                 if (!more) break;
@@ -1038,6 +1135,13 @@ cola_status cola_gauge_info(const cola_ctx *c, double *max_unitarity_dev)
     return COLA_OK;
 }
 
+cola_status cola_clover_info(const cola_ctx *c, double *min_pivot)
+{
+    if (!c || !min_pivot) return COLA_EINVAL;
+    *min_pivot = c->min_pivot;
+    return COLA_OK;
+}
+
 cola_status cola_clover_unpack(cola_ctx *c, int which, void *canon_dev)
 {
     ST(need_ready(c, "cola_clover_unpack"));
@@ -1052,6 +1156,7 @@ cola_status cola_spinor_pack(cola_ctx *c, cola_prec prec, const void *canon_dev,
 {
     if (!c) return COLA_EINVAL;
     if (!canon_dev || !internal_dev) return fail(c, COLA_EINVAL, "cola_spinor_pack: NULL pointer");
+    if (prec != COLA_F64 && prec != COLA_F32) return fail(c, COLA_EINVAL, "cola_spinor_pack: prec must be COLA_F64 or COLA_F32 (COLA_F32_H16 uses fp32 spinors)");
     CK(launch_spinor_pack(prec, c->g, canon_dev, internal_dev, c->stream));
     c->launches++;
     return COLA_OK;
@@ -1061,6 +1166,7 @@ cola_status cola_spinor_unpack(cola_ctx *c, cola_prec prec, const void *internal
 {
     if (!c) return COLA_EINVAL;
     if (!canon_dev || !internal_dev) return fail(c, COLA_EINVAL, "cola_spinor_unpack: NULL pointer");
+    if (prec != COLA_F64 && prec != COLA_F32) return fail(c, COLA_EINVAL, "cola_spinor_unpack: prec must be COLA_F64 or COLA_F32 (COLA_F32_H16 uses fp32 spinors)");
     CK(launch_spinor_unpack(prec, c->g, internal_dev, canon_dev, c->stream));
     c->launches++;
     return COLA_OK;
@@ -1070,6 +1176,7 @@ cola_status cola_spinor_convert(cola_ctx *c, cola_prec dst_prec, const void *src
 {
     if (!c) return COLA_EINVAL;
     if (!src_dev || !dst_dev || n_half < 1 || n_half > 2) return fail(c, COLA_EINVAL, "cola_spinor_convert: bad argument");
+    if (dst_prec != COLA_F64 && dst_prec != COLA_F32) return fail(c, COLA_EINVAL, "cola_spinor_convert: dst_prec must be COLA_F64 or COLA_F32");
     const cola_prec src_prec = dst_prec == COLA_F64 ? COLA_F32 : COLA_F64;
     for (int h = 0; h < n_half; h++) {
         CK(launch_spinor_convert(dst_prec, (const char *)src_dev + h * half_bytes(c, src_prec), (char *)dst_dev + h * half_bytes(c, dst_prec), c->Vh, c->stream));
@@ -1106,15 +1213,20 @@ cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *
 }
 
 cola_status cola_cg_solve_history(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info,
-                                  double *resid_hist_host, int hist_len)
+                                  double *resid_hist_host, int hist_len, int *update_iters_host, int update_len)
 {
     if (!c) return COLA_EINVAL;
     if (!resid_hist_host || hist_len < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_history: NULL or empty history buffer");
+    if (update_iters_host && update_len < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_history: empty update buffer");
     c->hist = resid_hist_host;
     c->hist_len = hist_len;
+    c->upd_iters = update_iters_host;
+    c->upd_len = update_iters_host ? update_len : 0;
     const cola_status st = solve_impl(c, sp, b_canon_dev, x_canon_dev, info);
     c->hist = nullptr;
     c->hist_len = 0;
+    c->upd_iters = nullptr;
+    c->upd_len = 0;
     return st;
 }
 
@@ -1163,25 +1275,26 @@ cola_status cola_cg_solve_host(cola_ctx *c, const cola_solve_params *sp, const v
     ST(need_ready(c, "cola_cg_solve_host"));
     if (!b_canon_host || !x_canon_host) return fail(c, COLA_EINVAL, "cola_cg_solve_host: NULL pointer");
     CK(cudaSetDevice(c->p.device));
-    // canonical staging: the last two fp64 half-slots pairs of the scratch are free in every solver mode
-    // except mixed CGNR on M, which uses all 12; stage in tmp64+tmp32 is too small, so the canonical b/x
-    // share ONE staging buffer: b is packed before x is produced.
+    // canonical staging inside the solver's own scratch (solve_impl: packed source B = slots 0-1, solution X = slots 2-3):
+    // the canonical b is staged in X's slots -- it is packed into B before X is zeroed -- and the canonical x is
+    // unpacked over B, which is dead once the true residual has been formed.  No mode needs extra room.
     const size_t fb = 2 * half_bytes(c, COLA_F64);
-    char *stage = c->scratch + c->scratch_bytes - fb;
-    if (!sp || (sp->mixed && !sp->even_odd)) return fail(c, COLA_EINVAL, "cola_cg_solve_host: mixed CGNR on M is not offered with host buffers");
-    CK(cudaMemcpyAsync(stage, b_canon_host, fb, cudaMemcpyHostToDevice, c->stream));
-    cola_status st = solve_impl(c, sp, stage, stage, info);
+    char *stage_b = c->scratch + fb, *stage_x = c->scratch;
+    if (!sp) return fail(c, COLA_EINVAL, "cola_cg_solve_host: NULL solve parameters");
+    CK(cudaMemcpyAsync(stage_b, b_canon_host, fb, cudaMemcpyHostToDevice, c->stream));
+    cola_status st = solve_impl(c, sp, stage_b, stage_x, info);
     if (st != COLA_OK && st != COLA_ENOCONV) return st;
-    CK(cudaMemcpyAsync(x_canon_host, stage, fb, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaMemcpyAsync(x_canon_host, stage_x, fb, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return st;
 }
 
 // ---- multi-right-hand-side entry points
-size_t cola_mrhs_workspace_bytes(const cola_ctx *c, int nrhs)
+size_t cola_mrhs_workspace_bytes(const cola_ctx *c, int nrhs, int for_solver)
 {
     if (!c || nrhs < 1 || nrhs > MRHS_MAX) return 0;
-    return carve_m(c, nrhs).total;
+    const CarveM k = carve_m(c, nrhs);
+    return for_solver ? k.total : k.op_total;
 }
 
 cola_status cola_set_mrhs_workspace(cola_ctx *c, void *dev_ptr, size_t bytes, int nrhs)
@@ -1192,7 +1305,8 @@ cola_status cola_set_mrhs_workspace(cola_ctx *c, void *dev_ptr, size_t bytes, in
     if (nrhs < 1 || nrhs > MRHS_MAX) return fail(c, COLA_EINVAL, "cola_set_mrhs_workspace: nrhs must be 1..16");
     if (!dev_ptr || ((uintptr_t)dev_ptr & 255)) return fail(c, COLA_EINVAL, "cola_set_mrhs_workspace: pointer must be non-NULL and 256-byte aligned");
     const CarveM k = carve_m(c, nrhs);
-    if (bytes < k.total) return fail(c, COLA_ENOMEM, "cola_set_mrhs_workspace: workspace smaller than cola_mrhs_workspace_bytes()");
+    if (bytes < k.op_total) return fail(c, COLA_ENOMEM, "cola_set_mrhs_workspace: workspace smaller than cola_mrhs_workspace_bytes()");
+    c->m_solver = bytes >= k.total;   // room for the batched solver's vectors as well
     char *w = (char *)dev_ptr;
     c->m_tmp32 = w + k.tmp32; c->m_r64 = w + k.r64; c->m_rhs = w + k.rhs; c->m_qs = w + k.qs;
     c->m_x32 = w + k.x32; c->m_r32 = w + k.r32; c->m_p32 = w + k.p32; c->m_q32 = w + k.q32;

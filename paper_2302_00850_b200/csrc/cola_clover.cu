@@ -170,7 +170,7 @@ __device__ __forceinline__ void store_block(char *c64, char *c32, char *c16, siz
 }
 
 // one thread per site: tid < 2*Vh, parity = tid / Vh
-__global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *gauge64, double k, int trace_sub, char *A64, char *A32, char *A16)
+__global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *gauge64, double k, int trace_sub, char *A64, char *A32, int a32_parities, char *A16)
 {
     const long tid = (long)blockIdx.x * CB + threadIdx.x;
     if (tid >= 2L * g.Vh) return;
@@ -195,8 +195,8 @@ __global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *ga
     field_strength(g, gauge64, c, 2, 3, trace_sub, Fzt);
     const size_t Vh = g.Vh;
     char *a64 = A64 + (size_t)parity * 72 * 8 * Vh;
-    char *a32 = A32 ? A32 + (size_t)parity * 72 * 4 * Vh : nullptr;
-    char *a16 = A16 ? A16 + (size_t)parity * CLOVER_H16_BYTES * Vh : nullptr;
+    char *a32 = (A32 && parity < a32_parities) ? A32 + (size_t)parity * 72 * 4 * Vh : nullptr;   // fp32 A on the odd parity is optional
+    char *a16 = (A16 && parity < a32_parities) ? A16 + (size_t)parity * CLOVER_H16_BYTES * Vh : nullptr;
 #pragma unroll
     for (int blk = 0; blk < 2; blk++) {
         const double sg = blk == 0 ? 1.0 : -1.0;
@@ -227,10 +227,18 @@ __global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *ga
 }
 
 // one thread per (site, block) of one parity: tid < 2*Vh, blk = tid / Vh
-__global__ void __launch_bounds__(CB) clover_invert_kernel(Geom g, const char *A64, char *I64, char *I32, char *I16)
+// order-preserving map of a double onto unsigned 64-bit keys (atomicMin on the key = min of the doubles, any sign)
+__device__ __forceinline__ unsigned long long order_key(double v)
+{
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+
+__global__ void __launch_bounds__(CB) clover_invert_kernel(Geom g, const char *A64, char *I64, char *I32, char *I16, unsigned long long *min_pivot_key)
 {
     const long tid = (long)blockIdx.x * CB + threadIdx.x;
-    if (tid >= 2L * g.Vh) return;
+    unsigned long long key = ~0ull;    // threads past the end take part in the warp minimum with the neutral key
+    if (tid < 2L * g.Vh) {
     const int blk = (int)(tid / g.Vh);
     const int i = (int)(tid - (long)blk * g.Vh);
     const size_t Vh = g.Vh;
@@ -248,9 +256,12 @@ __global__ void __launch_bounds__(CB) clover_invert_kernel(Geom g, const char *A
             ai[6 * c + r] = -p[k + 1];
         }
     }
-    // in-place Gauss-Jordan inverse without pivoting (Hermitian positive definite: pivots are real > 0 up to rounding)
+    // in-place Gauss-Jordan inverse without pivoting (Hermitian positive definite: pivots are real > 0 up to rounding).
+    // The smallest pivot met is reported; a pivot <= 0 means the block is not positive definite.
+    double pmin = 1e300;
     for (int c = 0; c < 6; c++) {
         const double pr = ar[7 * c], pi = ai[7 * c];
+        pmin = (pr < pmin || !(pr == pr)) ? pr : pmin;
         const double den = 1.0 / (pr * pr + pi * pi);
         const double ir = pr * den, ii = -pi * den;   // 1/pivot
         ar[7 * c] = 1.0;
@@ -274,6 +285,15 @@ __global__ void __launch_bounds__(CB) clover_invert_kernel(Geom g, const char *A
     double q[36];
     pack_block(ar, ai, q);
     store_block(I64, I32, I16, Vh, blk, i, q);
+    key = (pmin == pmin) ? order_key(pmin) : 0ull;   // NaN pivots map to a key below every number's (reported as not positive definite)
+    }
+    if (min_pivot_key) {
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
+            key = other < key ? other : key;
+        }
+        if ((threadIdx.x & 31) == 0) atomicMin(min_pivot_key, key);
+    }
 }
 
 // expand packed blocks to canonical 12x12 complex per lex site; parity_mask bit p set => parity p is
@@ -316,17 +336,17 @@ __global__ void __launch_bounds__(CB) clover_unpack_kernel(Geom g, const char *c
 
 }  // namespace
 
-cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, void *clovA16, cudaStream_t s)
+cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, int a32_parities, void *clovA16, cudaStream_t s)
 {
     const long n = 2L * g.Vh;
-    clover_build_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)gauge64, kappa_csw, trace_sub, (char *)clovA64, (char *)clovA32, (char *)clovA16);
+    clover_build_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)gauge64, kappa_csw, trace_sub, (char *)clovA64, (char *)clovA32, a32_parities, (char *)clovA16);
     return cudaGetLastError();
 }
 
-cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, void *clovI16, cudaStream_t s)
+cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, void *clovI16, unsigned long long *min_pivot_key, cudaStream_t s)
 {
     const long n = 2L * g.Vh;
-    clover_invert_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)clovA64_odd, (char *)clovI64, (char *)clovI32, (char *)clovI16);
+    clover_invert_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)clovA64_odd, (char *)clovI64, (char *)clovI32, (char *)clovI16, min_pivot_key);
     return cudaGetLastError();
 }
 

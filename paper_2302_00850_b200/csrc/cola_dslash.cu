@@ -12,7 +12,7 @@
 //   (1 + s gamma_mu) psi = [ h ; s A_mu^+ h ],   h = psi_upper + s A_mu psi_lower,   s = +-1.
 #include <string.h>
 
-#include "cola_device.cuh"
+#include "cola_hop.cuh"
 
 namespace cola {
 
@@ -37,102 +37,6 @@ namespace {
 #endif
 constexpr int DSLASH_BLOCK = COLA_DSLASH_BLOCK;
 template <int FMT> struct MinBlocks { static constexpr int value = (FMT == LINK_F64_18) ? COLA_DSLASH_MINB_F64 : COLA_DSLASH_MINB_F32; };
-
-// h (2 spins x 3 colours, complex) = upper + s * A_mu * lower of the 24-real spinor p
-template <int MU, typename T>
-__device__ __forceinline__ void project(const T (&p)[24], T s, T (&h)[12])
-{
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        const int u0 = 2 * c, u1 = 6 + 2 * c, l0 = 12 + 2 * c, l1 = 18 + 2 * c;   // spin 0,1,2,3 colour c (re)
-        if (MU == 0) {          // A = [[0,-i],[-i,0]]
-            h[2 * c] = p[u0] + s * p[l1 + 1];
-            h[2 * c + 1] = p[u0 + 1] - s * p[l1];
-            h[6 + 2 * c] = p[u1] + s * p[l0 + 1];
-            h[6 + 2 * c + 1] = p[u1 + 1] - s * p[l0];
-        } else if (MU == 1) {   // A = [[0,-1],[1,0]]
-            h[2 * c] = p[u0] - s * p[l1];
-            h[2 * c + 1] = p[u0 + 1] - s * p[l1 + 1];
-            h[6 + 2 * c] = p[u1] + s * p[l0];
-            h[6 + 2 * c + 1] = p[u1 + 1] + s * p[l0 + 1];
-        } else if (MU == 2) {   // A = [[-i,0],[0,i]]
-            h[2 * c] = p[u0] + s * p[l0 + 1];
-            h[2 * c + 1] = p[u0 + 1] - s * p[l0];
-            h[6 + 2 * c] = p[u1] - s * p[l1 + 1];
-            h[6 + 2 * c + 1] = p[u1 + 1] + s * p[l1];
-        } else {                // A = 1
-            h[2 * c] = p[u0] + s * p[l0];
-            h[2 * c + 1] = p[u0 + 1] + s * p[l0 + 1];
-            h[6 + 2 * c] = p[u1] + s * p[l1];
-            h[6 + 2 * c + 1] = p[u1 + 1] + s * p[l1 + 1];
-        }
-    }
-}
-
-// acc += eta * [ g ; s A_mu^+ g ]
-template <int MU, typename T>
-__device__ __forceinline__ void reconstruct_accumulate(const T (&g)[12], T eta, T s, T (&acc)[24])
-{
-    const T se = s * eta;
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        const int u0 = 2 * c, u1 = 6 + 2 * c, l0 = 12 + 2 * c, l1 = 18 + 2 * c;
-        const T g0r = g[2 * c], g0i = g[2 * c + 1], g1r = g[6 + 2 * c], g1i = g[6 + 2 * c + 1];
-        acc[u0] += eta * g0r;
-        acc[u0 + 1] += eta * g0i;
-        acc[u1] += eta * g1r;
-        acc[u1 + 1] += eta * g1i;
-        if (MU == 0) {          // A^+ = [[0,i],[i,0]]: lower0 = i g1, lower1 = i g0
-            acc[l0] -= se * g1i;
-            acc[l0 + 1] += se * g1r;
-            acc[l1] -= se * g0i;
-            acc[l1 + 1] += se * g0r;
-        } else if (MU == 1) {   // A^+ = [[0,1],[-1,0]]: lower0 = g1, lower1 = -g0
-            acc[l0] += se * g1r;
-            acc[l0 + 1] += se * g1i;
-            acc[l1] -= se * g0r;
-            acc[l1 + 1] -= se * g0i;
-        } else if (MU == 2) {   // A^+ = [[i,0],[0,-i]]: lower0 = i g0, lower1 = -i g1
-            acc[l0] -= se * g0i;
-            acc[l0 + 1] += se * g0r;
-            acc[l1] += se * g1i;
-            acc[l1 + 1] -= se * g1r;
-        } else {                // A^+ = 1
-            acc[l0] += se * g0r;
-            acc[l0 + 1] += se * g0i;
-            acc[l1] += se * g1r;
-            acc[l1 + 1] += se * g1i;
-        }
-    }
-}
-
-// g = U h (DAG = false) or U^+ h (DAG = true) on both spin components of the half spinor
-template <bool DAG, typename T>
-__device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&g)[12])
-{
-#pragma unroll
-    for (int sp = 0; sp < 2; sp++) {
-#pragma unroll
-        for (int a = 0; a < 3; a++) {
-            T re = 0, im = 0;
-#pragma unroll
-            for (int b = 0; b < 3; b++) {
-                const T ur = DAG ? u[2 * (3 * b + a)] : u[2 * (3 * a + b)];
-                const T ui = DAG ? -u[2 * (3 * b + a) + 1] : u[2 * (3 * a + b) + 1];
-                const T hr = h[6 * sp + 2 * b], hi = h[6 * sp + 2 * b + 1];
-                if (b == 0) {
-                    re = fma_(-ui, hi, ur * hr);
-                    im = fma_(ui, hr, ur * hi);
-                } else {
-                    re = fma_(-ui, hi, fma_(ur, hr, re));
-                    im = fma_(ui, hr, fma_(ur, hi, im));
-                }
-            }
-            g[6 * sp + 2 * a] = re;
-            g[6 * sp + 2 * a + 1] = im;
-        }
-    }
-}
 
 // one hop: neighbour index nb (parity 1-p), link at site li of the given gauge block
 template <int FMT, int MU, bool BACK, bool STREAM, typename T>
@@ -269,33 +173,7 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
         hop<FMT, 3, true, STREAM>(in, gq + 3 * lb, Vh, tb, tb, et_b, sb, acc);
         }
 
-        if (XPAY != 0) {
-            T yv[24];
-            load_reals<T, 24, true>(yin, Vh, i, yv);
-            const T cf = (T)a.coef;
-            if (XPAY == 2) {
-                T cy[24];
-                clover_apply<T, STREAM, FMT == LINK_I16_12>(a.clov_y, Vh, i, yv, cy);
-#pragma unroll
-                for (int k = 0; k < 24; k++) acc[k] = cy[k] + cf * acc[k];
-            } else {
-#pragma unroll
-                for (int k = 0; k < 24; k++) acc[k] = yv[k] + cf * acc[k];
-            }
-        }
-        if (POST != 0) {
-            T w[24];
-            clover_apply<T, STREAM, FMT == LINK_I16_12>(a.clov_post, Vh, i, acc, w);
-#pragma unroll
-            for (int k = 0; k < 24; k++) acc[k] = w[k];
-        }
-        store_reals<T, 24>(out, Vh, i, acc);
-        if (want_norm) {
-            T s2 = 0;
-#pragma unroll
-            for (int k = 0; k < 24; k++) s2 += acc[k] * acc[k];
-            nrm = (double)s2;
-        }
+        nrm = dslash_epilogue<FMT, XPAY, POST, STREAM>(a, i, acc, yin, out, want_norm);
     }
     return nrm;
 }

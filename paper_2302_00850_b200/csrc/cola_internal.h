@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stddef.h>
 #include <stdint.h>
+#include <string.h>
 
 #include "../../include/cola.h"
 
@@ -147,6 +148,27 @@ struct DslashArgs {
     const int *skip;        // if non-null and *skip != 0 the launch is a no-op (speculatively queued iteration)
 };
 
+// Shared-memory-staged variant of the kernel family (cola_dslash_tile.cu): a block owns the 4-D tile Xh x TY x TZ x TT
+// of output sites and stages the tile's input spinors plus its six faces (nent spinors) in shared memory.
+struct TileShape {
+    int ok;
+    int TY, TZ, TT;
+    int nthr;     // sites (threads) per tile
+    int nent;     // staged input spinors per tile
+};
+TileShape choose_tile(const Geom &g);
+struct TileArgs {
+    DslashArgs d;          // d.sweep is ignored (tiles are swept y, z, t)
+    int TX, TY, TZ, TT;
+    int nthr, nent, ntiles;
+    int stride;            // shared-memory entries per 16-byte chunk plane
+    int off[6];            // first entry of the y-, y+, z-, z+, t-, t+ face
+    FastDiv dTX, dTY, dTZ, d1;
+    FastDiv nby, nbz;      // tiles along y and z
+};
+// cudaErrorNotSupported if the format or the geometry has no staged kernel (the caller falls back to launch_dslash)
+cudaError_t launch_dslash_tile(int fmt, const DslashArgs &a, cudaStream_t s);
+
 // Multi-right-hand-side launch of the same kernel family: `nrhs` vectors share one pass over
 // the links and the clover field.  Vector k of the launch is vector list[k] of the caller's arrays: `in`, `out`, `y`
 // of `d` point at vector 0 and consecutive vectors are `*_stride` bytes apart.  A thread block covers the sites of a
@@ -195,8 +217,17 @@ cudaError_t launch_gauge_reorder(const Geom &g, const double *canon_dev, long si
 cudaError_t launch_spinor_pack(cola_prec prec, const Geom &g, const void *canon, void *internal, cudaStream_t s);
 cudaError_t launch_spinor_unpack(cola_prec prec, const Geom &g, const void *internal, void *canon, cudaStream_t s);
 cudaError_t launch_spinor_convert(cola_prec dst_prec, const void *src, void *dst, size_t n_sites, cudaStream_t s);
-cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, void *clovA16, cudaStream_t s);
-cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, void *clovI16, cudaStream_t s);
+// a32_parities: 2 = fp32 copy of A on both parities, 1 = even parity only (no COLA_FEAT_FULL_M)
+cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, int a32_parities, void *clovA16, cudaStream_t s);
+// *min_pivot_key (device, initialised to ~0ull) receives the order-preserving key of the smallest Gauss-Jordan pivot: decode with pivot_from_key
+cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, void *clovI16, unsigned long long *min_pivot_key, cudaStream_t s);
+inline double pivot_from_key(unsigned long long k)
+{
+    const unsigned long long b = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+    double v;
+    memcpy(&v, &b, sizeof(v));
+    return v;
+}
 cudaError_t launch_clover_unpack(const Geom &g, const void *clov64, int parity_mask, void *canon, cudaStream_t s);
 
 // fused BLAS-1 (cola_blas.cu).  n = number of sites of the vectors (Vh or V).

@@ -42,10 +42,15 @@ def run(k):
         t0 = time.time()
         r = oracle.cgnr(dims, inputs.BC, U, A, Ainv, c["kappa"], b, even_odd=eo, tol=1e-10)
         sites = sample_sites(inputs.volume(dims), k)
+        # |r_0| / |b| of the iterated system and the residual history |r_{k+1}| / |b|: what the reliable-update schedule
+        # of the mixed-precision solvers follows from (tests/schedule.py)
+        rhs = oracle.eo_prepare(dims, inputs.BC, U, Ainv, c["kappa"], b) if eo else b
+        rmax0 = float(np.linalg.norm(rhs.ravel()) / np.linalg.norm(b.ravel()))
         xs = r["x"].reshape(-1, 12)[sites]
         entry[name] = dict(iters=int(r["iters"]), converged=bool(r["converged"]), true_residual=float(r["true_residual"]),
                            x_norm=float(np.linalg.norm(r["x"].ravel())), sites=[int(s) for s in sites],
                            x_re=[[float(v) for v in row.real] for row in xs], x_im=[[float(v) for v in row.imag] for row in xs],
+                           rmax0=rmax0, history=[float(v) for v in r["history"]],
                            seconds=time.time() - t0)
         print(k, name, entry[name]["iters"], entry[name]["true_residual"], entry[name]["seconds"], flush=True)
     return entry

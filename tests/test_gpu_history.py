@@ -28,10 +28,15 @@ def test_residual_history_follows_the_oracle(dims, even_odd):
     h_ref = np.asarray(ref["history"])
     c = binding.Cola(dims, kappa, csw, bc=BC)
     c.gauge_upload(U)
-    # relative deviation of the histories allowed per mode (measured: fp64 1e-14 everywhere; fp32 inner 3e-7...3e-6 and
-    # 16-bit inner 4e-4...4e-3 on the Schur system; on the worse-conditioned unpreconditioned 4^4 system the mixed
-    # recurrences drift to 9 % / 14 % in the last decade before convergence while still converging in the same pass)
-    for mixed, tol_rel in ((0, 1e-12), (1, 1e-4 if even_odd else 0.25), (2, 2e-2 if even_odd else 0.25)):
+    # Relative deviation of the histories allowed per mode.  fp64: rounding only.  Mixed modes on the Schur system: the
+    # inner recurrence is re-anchored to the fp64 residual every decade (delta = 0.1), so it drifts by at most
+    # eps_op * cond(S) / delta with eps_op = 6e-8 (fp32) or 2.4e-4 (16-bit fields) and cond(S) ~ 30: 1.8e-5 and
+    # 7e-2; the fp32 bound is set to 1e-4 = 5 x that, for the rounding of the recurrence's own updates.  On the
+    # unpreconditioned M (cond ~ 10^3) the rounded recurrence loses conjugacy and LAGS the fp64 one; the derived bound is
+    # "by less than one pass": the deviation stays below the largest residual reduction of a single fp64 pass
+    # (the same bound pins the oracle's own float model in tests/test_oracle_pins.py).
+    one_pass = float(np.max(1.0 - h_ref[1:] / h_ref[:-1]))
+    for mixed, tol_rel in ((0, 1e-12), (1, 1e-4 if even_odd else one_pass), (2, 7e-2 if even_odd else one_pass)):
         x, info = c.cg_solve_history(b.cuda(), tol=1e-10, even_odd=even_odd, mixed=mixed)
         h = np.asarray(info["history"])
         assert info["converged"] and len(h) == info["iters"]

@@ -129,12 +129,20 @@ def test_batched_solve_matches_oracle_and_sequential_solves(binding):
         res = np.linalg.norm((bn - oracle.M(lat.dims, lat.bc, lat.Un, lat.A, lat.kappa, xn)).ravel()) / np.linalg.norm(bn.ravel())
         assert res <= 1.05e-10
         assert infos[n]["reliable_updates"] >= 1
-    # oracle fp64 CGNR on a sample of the systems: iteration counts and solutions
+    # oracle fp64 CGNR on a sample of the systems: iteration counts, solutions and the number of reliable updates the
+    # oracle's fp64 history implies for that system (SURVEY O8 per system; tests/schedule.py)
+    from schedule import reliable_update_schedule
+
     for n in (0, 5, 11):
-        ref = oracle.cgnr(lat.dims, lat.bc, lat.Un, lat.A, lat.Ainv, lat.kappa, srcs[n].numpy(), even_odd=True, tol=1e-10)
+        bn = srcs[n].numpy()
+        ref = oracle.cgnr(lat.dims, lat.bc, lat.Un, lat.A, lat.Ainv, lat.kappa, bn, even_odd=True, tol=1e-10)
         assert ref["converged"]
         assert iter_ok(infos[n]["iters"], ref["iters"]), (n, infos[n]["iters"], ref["iters"])
         assert rel(x[n].cpu().numpy(), ref["x"]) < 5e-9
+        rhs = oracle.eo_prepare(lat.dims, lat.bc, lat.Un, lat.Ainv, lat.kappa, bn)
+        want_upd, margin = reliable_update_schedule(ref["history"], np.linalg.norm(rhs.ravel()) / np.linalg.norm(bn.ravel()), 0.1, 1e-10)
+        if margin > 1e-3:
+            assert infos[n]["reliable_updates"] == len(want_upd), (n, infos[n]["reliable_updates"], want_upd)
     # the single-rhs solver on the same sources: each system follows its own schedule, so counts agree
     for n in (0, 7):
         xs, info = c.cg_solve(b[n].contiguous(), tol=1e-10, even_odd=True, mixed=True)
@@ -185,6 +193,7 @@ def test_mrhs_error_codes(binding):
         c.set_mrhs_workspace(17)
     assert e.value.status == b.COLA_EINVAL
     assert c.mrhs_workspace_bytes(0) == 0 and c.mrhs_workspace_bytes(17) == 0
+    assert 0 < c.mrhs_workspace_bytes(3, for_solver=False) < c.mrhs_workspace_bytes(3, for_solver=True)
     assert b._lib.cola_schur_apply_mrhs(c._h, b.COLA_F32, 0, 0, v.data_ptr(), out.data_ptr()) in (b.COLA_EINVAL, b.COLA_ENOTREADY)   # empty batch
     c.set_mrhs_workspace(2)
     st = b._lib.cola_schur_apply_mrhs(c._h, b.COLA_F32, 0, 3, v.data_ptr(), out.data_ptr())

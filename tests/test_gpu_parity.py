@@ -27,6 +27,19 @@ def rel(a, b):
     return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
 
 
+EPS = {torch.float64: 2.0 ** -52, torch.float32: 2.0 ** -23}
+
+
+def check_op(got, want, dtype):
+    """north_star's tolerance on the relative L2 error, and beside it a bound on every single real component: on a
+    large lattice one component wrong by a per cent moves the L2 norm by less than the fp32 tolerance, so the norm
+    alone would not see it.  An output component is a sum of ~100 products of magnitude <= max|psi|; its rounding
+    error (inputs rounded to the working precision included) is a few eps * sqrt(100) * rms, far below
+    64 eps * max|want|, while a dropped or mis-signed term is of order rms ~ 0.1 max|want|."""
+    assert rel(got, want) < TOL[dtype]
+    assert np.abs(np.asarray(got) - np.asarray(want)).max() <= 64 * EPS[dtype] * np.abs(want).max()
+
+
 @pytest.fixture(scope="module")
 def cola_mod():
     from paper_2302_00850_b200 import binding
@@ -152,7 +165,7 @@ def test_parity_dslash(case, dtype, compress12, parity):
     out = torch.zeros_like(internal)
     c.dslash_apply(parity, internal[1 - parity].contiguous(), out=out[parity])
     got = c.spinor_unpack(out).cpu().numpy()
-    assert rel(got, want) < TOL[dtype]
+    check_op(got, want, dtype)
     assert np.abs(got[case.par != parity]).max() == 0
 
 
@@ -163,7 +176,7 @@ def test_fermion_matrix(case, dtype, compress12, dagger):
     psi = case.spinor(12)
     want = oracle.M(case.dims, case.bc, case.Un, case.A, case.kappa, psi.numpy(), dagger=dagger)
     got = c.spinor_unpack(c.fermion_matrix_apply(c.spinor_pack(to_dev(psi, dtype)), dagger=dagger)).cpu().numpy()
-    assert rel(got, want) < TOL[dtype]
+    check_op(got, want, dtype)
 
 
 @pytest.mark.parametrize("dtype,compress12", FORMATS)
@@ -176,7 +189,7 @@ def test_schur_operator(case, dtype, compress12, dagger):
     out = torch.zeros_like(internal)
     c.schur_apply(internal[0].contiguous(), dagger=dagger, out=out[0])
     got = c.spinor_unpack(out).cpu().numpy()
-    assert rel(got, want) < TOL[dtype]
+    check_op(got, want, dtype)
 
 
 def test_host_entry_points_match_device_entry_points(case):
@@ -184,9 +197,9 @@ def test_host_entry_points_match_device_entry_points(case):
     psi = case.spinor(14)
     want = oracle.M(case.dims, case.bc, case.Un, case.A, case.kappa, psi.numpy())
     got = c.fermion_matrix_apply_host(psi.pin_memory())
-    assert rel(got.numpy(), want) < 1e-12
+    check_op(got.numpy(), want, torch.float64)
     got32 = c.fermion_matrix_apply_host(psi.to(torch.complex64).pin_memory())
-    assert rel(got32.numpy(), want) < 2e-6
+    check_op(got32.numpy(), want, torch.float32)
     wantd = oracle.dslash_parity(case.dims, case.bc, case.Un, 1, psi.numpy())
     gotd = c.dslash_apply_host(1, psi.pin_memory())
     assert rel(gotd.numpy(), wantd) < 1e-12
@@ -219,12 +232,28 @@ def test_cg_solve_small(case, even_odd, mixed):
     assert iter_ok(info["iters"], ref["iters"]), (info["iters"], ref["iters"])
     assert rel(xn, ref["x"]) < 5e-9
     if mixed:
-        assert info["reliable_updates"] >= 1
+        # SURVEY O8's reliable-update schedule: the passes after which the fp64 residual is recomputed follow from the
+        # ORACLE's fp64 residual history alone (tests/schedule.py; pinned against oracle.cgnr_mixed on the CPU)
+        from schedule import reliable_update_schedule
+
+        rhs = oracle.eo_prepare(case.dims, case.bc, case.Un, case.Ainv, case.kappa, b.numpy()) if even_odd else b.numpy()
+        rmax0 = np.linalg.norm(rhs.ravel()) / np.linalg.norm(b.numpy().ravel())
+        want_upd, margin = reliable_update_schedule(ref["history"], rmax0, 0.1, 1e-10)
+        xh_, ih = c.cg_solve_history(b.cuda(), tol=1e-10, even_odd=even_odd, mixed=mixed)
+        assert ih["iters"] == info["iters"] and ih["reliable_updates"] == info["reliable_updates"] and torch.equal(xh_, x)
+        assert len(ih["update_iters"]) == info["reliable_updates"]
+        own, own_margin = reliable_update_schedule(ih["history"], rmax0, 0.1, 1e-10)
+        if own_margin > 1e-5:
+            assert ih["update_iters"] == own, (ih["update_iters"], own)     # the rule on the solver's own recurrence
+        if even_odd and margin > 1e-3:
+            assert ih["update_iters"] == want_upd, (ih["update_iters"], want_upd)
+        else:   # unpreconditioned M: the fp32 recurrence lags the fp64 one by less than a pass (test_oracle_pins.py)
+            assert abs(info["reliable_updates"] - len(want_upd)) <= 1
+            assert all(min(abs(u - w) for w in want_upd) <= 1 for u in ih["update_iters"]), (ih["update_iters"], want_upd)
     # host-buffer entry point gives the same answer
-    if even_odd or not mixed:
-        xh, infoh = c.cg_solve(b.pin_memory(), tol=1e-10, even_odd=even_odd, mixed=mixed)
-        assert infoh["iters"] == info["iters"]
-        assert rel(xh.numpy(), xn) < 1e-12
+    xh, infoh = c.cg_solve(b.pin_memory(), tol=1e-10, even_odd=even_odd, mixed=mixed)
+    assert infoh["iters"] == info["iters"] and infoh["reliable_updates"] == info["reliable_updates"]
+    assert rel(xh.numpy(), xn) < 1e-12
 
 
 def test_cg_dense_inverse_on_2to4(cola_mod):
@@ -321,6 +350,20 @@ def test_error_codes(cola_mod):
     c18 = b.Cola((4, 4, 4, 4), 0.12, 1.0, compress12=False)
     c18.gauge_upload(bad)
     assert c18.gauge_info() > 1e-4
+    # ... but their 16-bit copy (always 12 reals + rebuilt third row) would be wrong: the H16 operator and mixed = 2 refuse
+    v18 = c18.spinor_pack(inputs.source_gaussian((4, 4, 4, 4), 2).to(torch.complex64).cuda())
+    c18.fermion_matrix_apply(v18)                                   # fp32 x18: fine
+    with pytest.raises(b.ColaError) as e:
+        c18.fermion_matrix_apply(v18, h16=True)
+    assert e.value.status == b.COLA_EINVAL and "16-bit" in str(e.value)
+    for solve in (lambda: c18.cg_solve(inputs.source_gaussian((4, 4, 4, 4), 2).cuda(), mixed=2),
+                  lambda: c18.cg_solve_mrhs(torch.stack([inputs.source_gaussian((4, 4, 4, 4), 2).cuda()] * 2), mixed=2)):
+        with pytest.raises(b.ColaError) as e:
+            solve()
+        assert e.value.status == b.COLA_EINVAL
+    xx18, info18 = c18.cg_solve(inputs.source_gaussian((4, 4, 4, 4), 2).cuda(), mixed=1)
+    assert info18["converged"]
+    c18.close()
     # max_iter -> COLA_ENOCONV with info filled and the last iterate returned
     c.gauge_upload(U)
     src = inputs.source_gaussian((4, 4, 4, 4), 2).cuda()
@@ -338,6 +381,15 @@ def test_error_codes(cola_mod):
     with pytest.raises(b.ColaError) as e:
         c.cg_solve_mrhs(torch.stack([src, bad_src]))
     assert e.value.status == b.COLA_EINVAL
+    # spinor layout calls take COLA_F64 / COLA_F32 only (COLA_F32_H16 is an operator precision, not a spinor format)
+    import ctypes
+    lib = ctypes.CDLL(b.lib_path())
+    v64 = c.spinor_pack(src)
+    dst = torch.empty_like(v64)
+    for call in (lambda: lib.cola_spinor_convert(c._h, b.COLA_F32_H16, ctypes.c_void_p(v64.data_ptr()), ctypes.c_void_p(dst.data_ptr()), 2),
+                 lambda: lib.cola_spinor_pack(c._h, b.COLA_F32_H16, ctypes.c_void_p(src.data_ptr()), ctypes.c_void_p(dst.data_ptr())),
+                 lambda: lib.cola_spinor_unpack(c._h, 7, ctypes.c_void_p(v64.data_ptr()), ctypes.c_void_p(dst.data_ptr()))):
+        assert call() == b.COLA_EINVAL
     xx, info = c.cg_solve(src)                       # the context is still usable afterwards
     assert info["converged"]
 
@@ -411,3 +463,164 @@ def test_everything_runs_on_the_callers_stream(cola_mod):
     assert torch.equal(x2, x0)
     c0.close()
     c1.close()
+
+
+def test_nan_links_stop_the_solvers_instead_of_iterating_to_max_iter(cola_mod):
+    """A NaN that enters through the gauge field (not the source) never satisfies a stopping test: the solvers must
+    notice the non-finite residual and return COLA_EINVAL (single and batched), not run to max_iter."""
+    b = cola_mod
+    dims = (4, 4, 4, 4)
+    U = inputs.links_haar(dims, 1)
+    bad = U.clone()
+    bad[1, 2, 3, 0, 2, 1, 1] = float("nan")
+    c = b.Cola(dims, 0.12, 1.0, compress12=False)      # compress12 would reject the link (NaN is "not unitary")
+    try:
+        c.gauge_upload(bad)
+    except b.ColaError as ex:                          # NaN pivot in the clover inverse: also a clean refusal
+        assert ex.status == b.COLA_EINVAL
+        return
+    src = inputs.source_gaussian(dims, 2).cuda()
+    for solve in (lambda: c.cg_solve(src, mixed=1, max_iter=200), lambda: c.cg_solve(src, mixed=0, max_iter=200),
+                  lambda: c.cg_solve_mrhs(torch.stack([src, src]), max_iter=200)):
+        with pytest.raises(b.ColaError) as e:
+            solve()
+        assert e.value.status == b.COLA_EINVAL
+    c.close()
+
+
+def test_features_select_the_carved_fields(cola_mod):
+    """cola_set_features: without COLA_FEAT_FULL_M / COLA_FEAT_H16 the workspace is smaller, everything the even-odd
+    mixed solver needs still works and gives the same bits, and calls that need a missing field return COLA_EINVAL."""
+    b = cola_mod
+    dims = (8, 8, 8, 16)
+    U = inputs.links_smooth(dims, 0.3, 9)
+    src = inputs.source_gaussian(dims, 5).cuda()
+    full = b.Cola(dims, 0.1245, 1.0)
+    lean = b.Cola(dims, 0.1245, 1.0, features=0)
+    assert lean.workspace_bytes() < 0.86 * full.workspace_bytes()
+    full.gauge_upload(U)
+    lean.gauge_upload(U)
+    x0, i0 = full.cg_solve(src, mixed=1)
+    x1, i1 = lean.cg_solve(src, mixed=1)
+    assert torch.equal(x0, x1) and i0["iters"] == i1["iters"]
+    xh, ih = lean.cg_solve(src.cpu().pin_memory(), mixed=1)
+    assert torch.equal(xh.cuda(), x1)
+    v32 = lean.spinor_pack(src.to(torch.complex64))
+    v64 = lean.spinor_pack(src)
+    assert torch.equal(lean.schur_apply(v32[0].contiguous()), full.schur_apply(v32[0].contiguous()))
+    assert torch.equal(lean.dslash_apply(1, v32[0].contiguous()), full.dslash_apply(1, v32[0].contiguous()))
+    assert torch.equal(lean.fermion_matrix_apply(v64), full.fermion_matrix_apply(v64))      # fp64 M is always there
+    for call in (lambda: lean.fermion_matrix_apply(v32), lambda: lean.schur_apply(v32[0].contiguous(), h16=True),
+                 lambda: lean.cg_solve(src, mixed=2), lambda: lean.cg_solve(src, even_odd=False),
+                 lambda: lean.fermion_matrix_apply_mrhs(torch.stack([v32, v32]))):
+        with pytest.raises(b.ColaError) as e:
+            call()
+        assert e.value.status == b.COLA_EINVAL
+    assert torch.equal(lean.schur_apply_mrhs(torch.stack([v32[0], v32[0]]))[1], full.schur_apply(v32[0].contiguous()))
+    # operators-only multi-rhs workspace: smaller, and the batched solver says it needs the large one
+    assert lean.mrhs_workspace_bytes(4, for_solver=False) < 0.3 * lean.mrhs_workspace_bytes(4, for_solver=True)
+    lean.set_mrhs_workspace(2, for_solver=False)
+    import ctypes
+    sp = lean._solve_params(1e-10, 100, True, 1, 0.1)
+    infos = (b.ColaSolveInfo * 2)()
+    bs = torch.stack([src, src])
+    xs = torch.empty_like(bs)
+    st = ctypes.CDLL(b.lib_path()).cola_cg_solve_mrhs(lean._h, ctypes.byref(sp), 2, ctypes.c_void_p(bs.data_ptr()), ctypes.c_void_p(xs.data_ptr()), infos)
+    assert st == b.COLA_ENOTREADY
+    xs, infos = lean.cg_solve_mrhs(bs)        # the binding re-lends a solver-sized workspace
+    assert torch.equal(xs[0], x1) and torch.equal(xs[1], x1)
+    # H16 alone
+    h = b.Cola(dims, 0.1245, 1.0, features=b.COLA_FEAT_H16)
+    h.gauge_upload(U)
+    x2, i2 = h.cg_solve(src, mixed=2)
+    x3, i3 = full.cg_solve(src, mixed=2)
+    assert torch.equal(x2, x3)
+    for c in (full, lean, h):
+        c.close()
+
+
+def test_smallest_pivot_is_reported_and_indefinite_blocks_are_refused(cola_mod):
+    """the upload reports the smallest pivot of the 6x6 inversions; a block that is not positive definite
+    (here: csw pushed far beyond anything physical on rough links) is COLA_EINVAL, not a silent garbage inverse."""
+    b = cola_mod
+    dims = (4, 4, 4, 4)
+    U = inputs.links_haar(dims, 3)
+    Un = U.numpy()
+    c = b.Cola(dims, 0.12, 1.0)
+    c.gauge_upload(U)
+    A = oracle.clover(dims, Un, 0.12, 1.0)
+    odd = oracle.parity_mask(dims) == 1
+    ev = np.linalg.eigvalsh(np.concatenate([A[odd][:, :6, :6], A[odd][:, 6:, 6:]]))
+    piv = c.clover_info()
+    # an unpivoted elimination of a Hermitian positive-definite block has pivots between its extreme eigenvalues
+    assert ev.min() - 1e-12 <= piv <= ev.max() and piv > 0
+    # brute force: the same elimination in numpy on the oracle's blocks
+    blocks = np.concatenate([A[odd][:, :6, :6], A[odd][:, 6:, 6:]])
+    pmin = np.inf
+    for blk in blocks:
+        m = blk.copy()
+        for k in range(6):
+            pmin = min(pmin, m[k, k].real)
+            m[k + 1:, :] -= np.outer(m[k + 1:, k] / m[k, k], m[k, :])
+    assert abs(piv - pmin) <= 1e-12
+    c.close()
+    csw_bad = 40.0
+    Abad = oracle.clover(dims, Un, 0.12, csw_bad)
+    assert np.linalg.eigvalsh(np.concatenate([Abad[odd][:, :6, :6], Abad[odd][:, 6:, 6:]])).min() < 0
+    cb = b.Cola(dims, 0.12, csw_bad)
+    with pytest.raises(b.ColaError) as e:
+        cb.gauge_upload(U)
+    assert e.value.status == b.COLA_EINVAL and "positive definite" in str(e.value)
+    assert cb.clover_info() <= 0
+    with pytest.raises(b.ColaError) as e:
+        cb.dslash_apply(0, torch.zeros(6, cb.Vh, 4, device="cuda"))
+    assert e.value.status == b.COLA_ENOTREADY
+    cb.close()
+
+
+def test_cuda_failures_surface_as_COLA_ECUDA(cola_mod):
+    """COLA_ECUDA (SURVEY 8(b) error cases).  (1) a device ordinal that does not exist; (2) in a child process, because
+    the fault poisons its CUDA context: a workspace that is freed behind the library's back -- the kernels fault, the
+    next synchronising call reports COLA_ECUDA with the CUDA message, and nothing hangs."""
+    import subprocess
+    import sys
+
+    b = cola_mod
+    import ctypes
+    lib = ctypes.CDLL(b.lib_path())
+    lib.cola_last_error.restype = ctypes.c_char_p
+    lib.cola_last_error.argtypes = [ctypes.c_void_p]
+    p = b.ColaParams()
+    p.dims[:] = (4, 4, 4, 4)
+    p.bc[:] = (1, 1, 1, -1)
+    p.kappa, p.csw, p.device = 0.12, 1.0, torch.cuda.device_count() + 7
+    h = ctypes.c_void_p()
+    assert lib.cola_create(ctypes.byref(h), ctypes.byref(p)) == b.COLA_ECUDA and not h.value
+    assert b"cudaSetDevice" in lib.cola_last_error(None)
+    torch.cuda.set_device(0)
+    child = r"""
+import ctypes, sys, torch
+sys.path.insert(0, %r)
+from paper_2302_00850_b200 import binding as b, inputs
+dims = (8, 8, 8, 16)
+c = b.Cola(dims, 0.1245, 1.0)
+ws = torch.empty(c.workspace_bytes(), dtype=torch.uint8, device="cuda")
+c.set_workspace(ws)
+c.gauge_upload(inputs.links_smooth(dims, 0.3, 9))
+src = inputs.source_gaussian(dims, 5).cuda()
+x, info = c.cg_solve(src, mixed=1)
+assert info["converged"]
+c._ws = None
+del ws
+torch.cuda.empty_cache()          # cudaFree: the library still holds the pointer
+try:
+    c.cg_solve(src, mixed=1)
+except b.ColaError as ex:
+    print("STATUS", ex.status, str(ex)[:120])
+    sys.exit(0 if ex.status == b.COLA_ECUDA else 3)
+print("no error raised")
+sys.exit(4)
+""" % os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", child], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, (r.returncode, r.stdout[-500:], r.stderr[-500:])
+    assert "STATUS 2" in r.stdout

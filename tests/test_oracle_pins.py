@@ -314,6 +314,54 @@ def test_mixed_precision_model_matches_fp64_iteration_count():
     assert rel(mix["x"], ref["x"]) < 5e-9
 
 
+@pytest.mark.parametrize("dims,even_odd", [((4, 4, 4, 8), True), ((4, 4, 4, 8), False), ((8, 8, 8, 16), True)])
+@pytest.mark.parametrize("delta", [0.1, 0.01])
+def test_reliable_update_schedule_is_pinned_by_the_fp64_history(dims, even_odd, delta):
+    """SURVEY O8's schedule (rmax tracking, the delta test, when updates fire) pinned by something other than
+    oracle_cgnr_mixed itself: the firing iterations follow from oracle_cgnr's fp64 residual history alone
+    (tests/schedule.py), because the float-rounded recurrence tracks it to ~1e-6.  A mistake in the model -- rmax never
+    reset, reset to the wrong value, delta off by a factor, <= for <, the update placed before the residual test --
+    moves at least one firing iteration."""
+    from schedule import reliable_update_schedule
+
+    kappa, csw, tol = 0.1245, 1.0, 1e-10
+    U = np_links("smooth", dims, seed=61)
+    A = oracle.clover(dims, U, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    b = rand_spinor(dims, 62)
+    ref = oracle.cgnr(dims, BC, U, A, Ainv, kappa, b, even_odd=even_odd, tol=tol)
+    mix = oracle.cgnr_mixed(dims, BC, U, A, Ainv, kappa, b, even_odd=even_odd, tol=tol, delta=delta)
+    assert ref["converged"] and mix["converged"]
+    rhs = oracle.eo_prepare(dims, BC, U, Ainv, kappa, b) if even_odd else b
+    rmax0 = np.linalg.norm(rhs.ravel()) / np.linalg.norm(b.ravel())
+    want, margin = reliable_update_schedule(ref["history"], rmax0, delta, tol)
+    assert margin > 1e-4, "a delta decision sits on its threshold: pick another seed"
+    # the float-rounded recurrence follows the fp64 one closely enough for the rule to be decided identically
+    n = min(len(mix["history"]), len(ref["history"]))
+    dev = np.abs(mix["history"][:n] - ref["history"][:n]) / ref["history"][:n]
+    # Schur system: eps_fp32 * cond / delta ~ 6e-8 * 30 / 0.01 stays below 1e-4.  Unpreconditioned M: the rounded
+    # recurrence loses conjugacy and LAGS the fp64 one; the bound is "by less than one pass", i.e. the deviation is
+    # below the largest residual reduction of a single fp64 pass
+    h = np.asarray(ref["history"])
+    one_pass = float(np.max(1.0 - h[1:] / h[:-1]))
+    assert dev.max() < (1e-4 if even_odd else one_pass), (float(dev.max()), one_pass)
+    own, own_margin = reliable_update_schedule(mix["history"], rmax0, delta, tol)
+    if even_odd:
+        # well-conditioned Schur system: the recurrences agree to ~1e-6, so the fp64 history alone fixes the schedule
+        assert mix["update_iters"] == want, (mix["update_iters"], want)
+        assert mix["updates"] == len(want) and mix["iters"] == want[-1] == ref["iters"]
+    else:
+        # unpreconditioned M: the float-rounded recurrence drifts by per cent in the last decades, so a firing may move
+        # by one pass against the fp64 prediction; the count may not
+        assert len(mix["update_iters"]) == len(want)
+        assert max(abs(a - b) for a, b in zip(mix["update_iters"], want)) <= 1, (mix["update_iters"], want)
+    # the rule re-applied (here, in Python) to the recurrence's recorded history reproduces the firings exactly
+    assert own_margin > 1e-6 and own == mix["update_iters"], (own, mix["update_iters"])
+    # delta = 0.1 fires about once per decade, delta = 0.01 once per two decades
+    decades = -np.log10(tol)
+    assert abs(len(want) - decades / -np.log10(delta)) <= 2
+
+
 # ---------------------------------------------------------------------------------------------
 # Pin 9: clover block invariants
 # ---------------------------------------------------------------------------------------------
@@ -359,3 +407,70 @@ def test_apply_sites_matches_full_operators():
         ref = oracle.schur(dims, BC, U, A, Ainv, kappa, psi * mask_e, dagger=dg)
         got = oracle.apply_sites(dims, BC, U, kappa, csw, which, psi, sites)   # odd part of psi is ignored
         assert rel(got, ref.reshape(V, 4, 3)) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------
+# BiCGStab: pinned by the dense inverse, by CGNR's solution and by scipy's implementation
+# ---------------------------------------------------------------------------------------------
+def test_bicgstab_against_dense_inverse_and_cgnr():
+    dims, kappa, csw = (2, 2, 2, 2), 0.12, 1.0
+    U = np_links("haar", dims, seed=51)
+    A = oracle.clover(dims, U, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    Md = bf.dense_M(dims, BC, U, kappa, csw)
+    b = rand_spinor(dims, 52)
+    x_exact = np.linalg.solve(Md, b.ravel())
+    for eo in (False, True):
+        res = oracle.bicgstab(dims, BC, U, A, Ainv, kappa, b, even_odd=eo)
+        assert res["converged"] and not res["breakdown"]
+        assert res["true_residual"] <= 1.05e-10
+        assert rel(res["x"].ravel(), x_exact) < 5e-9
+    dims = (4, 4, 4, 8)
+    U = np_links("smooth", dims, seed=61)
+    A = oracle.clover(dims, U, 0.1245, 1.0)
+    Ainv = oracle.clover_inverse(A)
+    b = rand_spinor(dims, 62)
+    cg = oracle.cgnr(dims, BC, U, A, Ainv, 0.1245, b, even_odd=True)
+    for eo in (False, True):
+        bi = oracle.bicgstab(dims, BC, U, A, Ainv, 0.1245, b, even_odd=eo)
+        assert bi["converged"] and bi["true_residual"] <= 1.05e-10
+        assert rel(bi["x"], cg["x"]) < 5e-9
+    # half the operator applications per pass of CGNR's, and fewer passes: the point of the method
+    assert bi["iters"] < cg["iters"]
+
+
+def test_bicgstab_iterates_match_scipy():
+    """The same recurrence in a library: scipy.sparse.linalg.bicgstab on a LinearOperator that applies the oracle's Schur
+    operator, x0 = 0, no preconditioner.  Iterate by iterate (scipy's callback) the two agree to rounding until rounding
+    differences have been amplified (late in the solve); a wrong coefficient, a swapped conjugation in <t, s> or a
+    wrong update order shows in the first iterate."""
+    from scipy.sparse.linalg import LinearOperator, bicgstab as sp_bicgstab
+
+    dims, kappa, csw = (4, 4, 4, 4), 0.124, 1.0
+    U = np_links("smooth", dims, seed=91)
+    A = oracle.clover(dims, U, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    b = rand_spinor(dims, 92)
+    mask_e = (oracle.parity_mask(dims) == 0)[..., None, None]
+    shape = b.shape
+    idx = np.flatnonzero(np.broadcast_to(mask_e, shape).ravel())
+
+    def S(xe):
+        full = np.zeros(b.size, dtype=np.complex128)
+        full[idx] = xe
+        return oracle.schur(dims, BC, U, A, Ainv, kappa, full.reshape(shape)).ravel()[idx]
+
+    n = idx.size
+    op = LinearOperator((n, n), matvec=S, dtype=np.complex128)
+    bhat = oracle.eo_prepare(dims, BC, U, Ainv, kappa, b).ravel()[idx]
+    iterates = []
+    x_sp, info = sp_bicgstab(op, bhat, x0=np.zeros(n, dtype=np.complex128), rtol=1e-12, atol=0.0, maxiter=12,
+                             callback=lambda xk: iterates.append(xk.copy()))
+    assert len(iterates) >= 8
+    bnorm = np.linalg.norm(b.ravel())
+    for k, xk in enumerate(iterates[:8]):
+        ours = oracle.bicgstab(dims, BC, U, A, Ainv, kappa, b, even_odd=True, tol=1e-30, max_iter=k + 1)
+        xe = ours["x"].ravel()[idx]          # even part of the reconstructed solution = the Schur iterate
+        assert rel(xe, xk) < 1e-9, (k, rel(xe, xk))
+        # and the recorded residual is the residual of that iterate
+        assert abs(ours["history"][k] - np.linalg.norm(bhat - S(xk)) / bnorm) <= 1e-9 * ours["history"][0]
