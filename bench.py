@@ -261,8 +261,11 @@ def main():
                     help="profiling aid: skip the solves, run only the operator table (few launches: --op-warm/--op-timed) and print it")
     ap.add_argument("--lattice", default="", help="test aid: run the config's recipe on other extents, e.g. 16,16,16,32")
     ap.add_argument("--no-h16", action="store_true", help="skip the extra solve with 16-bit links/clover in the inner iteration")
+    ap.add_argument("--no-bicgstab", action="store_true", help="skip the extra solves by BiCGStab on the Schur system")
     ap.add_argument("--no-batched", action="store_true", help="config 3: skip the batched (multi-rhs) solve of the 12 sources")
     ap.add_argument("--nrhs", type=int, default=0, help="with --operators-only: also time the multi-rhs Schur operator over this many vectors")
+    ap.add_argument("--staging", type=int, default=0, choices=[0, 1],
+                    help="kernel family of the fp32 / 16-bit single-rhs operators: 0 direct global loads (default), 1 neighbour spinors staged in shared memory")
     ap.add_argument("--op-warm", type=int, default=20)
     ap.add_argument("--op-timed", type=int, default=200)
     args = ap.parse_args()
@@ -310,6 +313,7 @@ def main():
             return inputs.source_gaussian(dims, inputs.config_seed_source(args.config) + rank, device=dev)
         n_src = 1
     ctx = binding.Cola(dims, cfg["kappa"], cfg["csw"], bc=inputs.BC, compress12=True, device=local)
+    ctx.set_staging(args.staging)
     torch.cuda.synchronize()
     t0 = time.time()
     ctx.gauge_upload(U)
@@ -434,6 +438,37 @@ def main():
                      "reliable_updates": [i["reliable_updates"] for i in infs_h],
                      "max_true_residual": max(i["true_residual"] for i in infs_h), "converged": all(i["converged"] for i in infs_h)}
 
+    # ---- the same step by BiCGStab on the Schur system (two S per pass instead of S and S^+)
+    solve_bicgstab = None
+    if rank == 0 and not args.no_bicgstab:
+        solve_bicgstab = {}
+        for key, mode in (("fp32_inner", 1), ("h16_inner", 2)):
+            def bi_step():
+                fl, infs = 0.0, []
+                for n in range(n_src):
+                    bn = b if n_src == 1 else source(n)
+                    xn, inf = ctx.cg_solve(bn, tol=1e-10, even_odd=True, mixed=mode, method="bicgstab")
+                    fl += inf["op_flops"]
+                    infs.append(inf)
+                    del xn
+                return fl, infs
+
+            for _ in range(min(args.warmup, 2)):
+                bi_step()
+            torch.cuda.synchronize()
+            e0.record()
+            fl_b = 0.0
+            for _ in range(args.steps):
+                f1, infs_b = bi_step()
+                fl_b += f1
+            e1.record()
+            torch.cuda.synchronize()
+            ms_b = e0.elapsed_time(e1) / args.steps
+            solve_bicgstab[key] = {"ms_per_step": round(ms_b, 3), "GFLOP/s": round(fl_b / args.steps / (ms_b * 1e-3) / 1e9, 1),
+                                   "speedup_vs_cgnr_fp32_inner": round(ms_local / args.steps / ms_b, 3), "passes": [i["iters"] for i in infs_b],
+                                   "reliable_updates": [i["reliable_updates"] for i in infs_b],
+                                   "max_true_residual": max(i["true_residual"] for i in infs_b), "converged": all(i["converged"] for i in infs_b)}
+
     # ---- the same sources as ONE batched solve (links and clover read once per pass for all)
     batched = None
     if n_src > 1 and rank == 0 and not args.no_batched:
@@ -520,6 +555,7 @@ def main():
         line["solve"]["max_true_residual"] = max(i["true_residual"] for i in infos)
         line["batched"] = batched
     line["solve_h16"] = solve_h16
+    line["solve_bicgstab"] = solve_bicgstab
     print(json.dumps(line))
     if world > 1:
         torch.distributed.destroy_process_group()

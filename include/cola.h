@@ -165,7 +165,12 @@ typedef struct {
     int mixed;         /* 0: all fp64; 1: fp32 inner iteration with fp64 reliable updates;
                           2: as 1, with the inner operator reading 16-bit links and clover (COLA_F32_H16) */
     double delta;      /* reliable-update threshold (mixed only); <= 0 selects the default 0.1 */
+    int method;        /* COLA_CGNR (0, the north_star solver) or COLA_BICGSTAB: BiCGStab in van der
+                          Vorst's order on the Schur system (needs even_odd = 1), x0 = 0, shadow residual = r0; one pass =
+                          two applications of S (CGNR: S and S^+), `iters` counts passes.  COLA_EINVAL on breakdown
+                          (<rhat, v>, <t, t> or rho vanishing).  Mixed precision and reliable updates as for CGNR. */
 } cola_solve_params;
+typedef enum { COLA_CGNR = 0, COLA_BICGSTAB = 1 } cola_method;
 
 typedef struct {
     int iters;                 /* CGLS passes done */
@@ -190,6 +195,43 @@ cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *
  * rule applied to the oracle's fp64 history. */
 cola_status cola_cg_solve_history(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info,
                                   double *resid_hist_host, int hist_len, int *update_iters_host, int update_len);
+
+/* ---- Low modes of H = S^+ S on the even sites ("solvers for linear systems and eigenmodes",
+ * ref [1] P:65) by thick-restart Lanczos on a Chebyshev polynomial of H, fp64, on the Schur kernels above.
+ *   n_ev          eigenpairs wanted (the n_ev smallest eigenvalues of H), 1..32
+ *   n_kr          dimension of the Krylov space kept between restarts, n_ev + 2 .. 64 (default when 0: 2 n_ev + 8)
+ *   tol           stop when the residual estimate of every wanted Ritz pair of the filtered operator is <= tol times
+ *                 its largest Ritz value (default when <= 0: 1e-10); the TRUE residuals |H u - lambda u| are returned
+ *   cheb_order    order p >= 1 of the Chebyshev polynomial T_p (p = 1: plain Lanczos on -H); default when 0: 24
+ *   cheb_lo/hi    the filter maps [cheb_lo, cheb_hi] to [-1, 1]: eigenvalues below cheb_lo are amplified.  cheb_hi <= 0:
+ *                 1.15 x a power-iteration estimate of the largest eigenvalue; cheb_lo <= 0: cheb_hi / 10.
+ *   seed          of the deterministic start vector
+ * Workspace: DEVICE, cola_eig_workspace_bytes(c, ep) bytes (n_kr + (n_kr + n_ev)/2 + 6 fp64 half-lattice vectors),
+ * borrowed for the call.  evals_host / resid_host: HOST arrays of n_ev doubles (ascending eigenvalues, |H u - lambda u|
+ * with |u| = 1); evecs_dev: DEVICE, n_ev fp64 even half-lattice internal vectors back to back, orthonormal (may be
+ * NULL).  COLA_ENOCONV (results of the last restart filled in) if max_restarts is reached. */
+typedef struct {
+    int n_ev, n_kr;
+    double tol;
+    int max_restarts;       /* default when 0: 100 */
+    int cheb_order;
+    double cheb_lo, cheb_hi;
+    unsigned seed;
+} cola_eig_params;
+typedef struct {
+    int restarts;
+    int op_applications;    /* applications of H = S^+ S (two Schur applications each) */
+    double cheb_lo, cheb_hi;/* the filter window used */
+    double seconds;
+} cola_eig_info;
+size_t cola_eig_workspace_bytes(const cola_ctx *c, const cola_eig_params *ep);
+cola_status cola_eig_lowest(cola_ctx *c, const cola_eig_params *ep, void *work_dev, size_t work_bytes, double *evals_host, double *resid_host,
+                            void *evecs_dev, cola_eig_info *info);
+/* cola_cg_solve (CGNR, even_odd = 1) started from the deflated guess x0_e = sum_i u_i <u_i, S^+ bhat_e> / lambda_i built
+ * from n_ev eigenpairs of H (cola_eig_lowest's output: evecs_dev DEVICE, evals_host HOST): the low modes that set the
+ * condition number are solved exactly at the start, the iteration works on the rest.  Same result as cola_cg_solve. */
+cola_status cola_cg_solve_deflated(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info,
+                                   const void *evecs_dev, const double *evals_host, int n_ev);
 
 /* End-to-end variants: HOST canonical buffers; the host<->device copies are part of the call. */
 cola_status cola_dslash_apply_host(cola_ctx *c, cola_prec prec, cola_parity out_parity, const void *in_canon_host, void *out_canon_host);

@@ -18,7 +18,7 @@ _LIB = os.path.join(_HERE, "libcola_oracle.so")
 
 __all__ = [
     "build", "gamma", "sigma", "hop", "dslash_parity", "field_strength", "clover", "clover_inverse",
-    "block_apply", "M", "schur", "eo_prepare", "eo_reconstruct", "apply_sites", "cgnr", "cgnr_mixed", "bicgstab",
+    "block_apply", "M", "schur", "eo_prepare", "eo_reconstruct", "apply_sites", "cgnr", "cgnr_mixed", "bicgstab", "lowest_modes",
     "dense_inverse", "num_threads", "parity_mask",
 ]
 
@@ -248,3 +248,42 @@ def bicgstab(dims, bc, U, A, Ainv, kappa: float, b, even_odd: bool, tol: float =
                               ctypes.byref(true_res))
     return dict(x=x, iters=iters.value, converged=(st == 0), breakdown=(st == 2), true_residual=true_res.value,
                 history=hist[: iters.value].copy())
+
+
+def lowest_modes(dims, bc, U, A, Ainv, kappa: float, k: int, dense_limit: int = 1600, tol: float = 1e-13):
+    """The k smallest eigenvalues (ascending) and orthonormal eigenvectors of H = S^+ S on the even sites
+    (the low modes the paper's "eigenmode solver" delivers, ref [1] P:65).
+
+    It is the plain definition: for up to `dense_limit` even-site degrees of freedom the matrix of S is written out
+    column by column with oracle.schur, H = S^+ S is formed and numpy's Hermitian eigen-solver is called; above that
+    the library routine is scipy's ARPACK driver on a LinearOperator that applies oracle.schur twice.
+    Returns (evals[k], evecs[k] + full-lattice spinor shape, zero on odd sites)."""
+    shape = _shape(dims) + (4, 3)
+    mask_e = np.broadcast_to((parity_mask(dims) == 0)[..., None, None], shape)
+    idx = np.flatnonzero(mask_e.ravel())
+    n = idx.size
+
+    def S(xe, dagger=False):
+        full = np.zeros(int(np.prod(shape)), dtype=np.complex128)
+        full[idx] = xe
+        return schur(dims, bc, U, A, Ainv, kappa, full.reshape(shape), dagger=dagger).ravel()[idx]
+
+    if n <= dense_limit:
+        Sd = np.empty((n, n), dtype=np.complex128)
+        e = np.zeros(n, dtype=np.complex128)
+        for j in range(n):
+            e[j] = 1.0
+            Sd[:, j] = S(e)
+            e[j] = 0.0
+        w, v = np.linalg.eigh(Sd.conj().T @ Sd)
+        w, v = w[:k], v[:, :k]
+    else:
+        from scipy.sparse.linalg import LinearOperator, eigsh
+
+        op = LinearOperator((n, n), matvec=lambda x: S(S(x), dagger=True), dtype=np.complex128)
+        w, v = eigsh(op, k=k, which="SA", tol=tol, ncv=max(4 * k, 40), maxiter=20000)
+        order = np.argsort(w)
+        w, v = w[order], v[:, order]
+    vecs = np.zeros((k, int(np.prod(shape))), dtype=np.complex128)
+    vecs[:, idx] = v.T
+    return w, vecs.reshape((k,) + shape)

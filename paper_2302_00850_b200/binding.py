@@ -18,6 +18,8 @@ COLA_OK, COLA_EINVAL, COLA_ECUDA, COLA_ENOTREADY, COLA_ENOCONV, COLA_ENOMEM = ra
 COLA_F64, COLA_F32, COLA_F32_H16 = 0, 1, 2
 COLA_EVEN, COLA_ODD = 0, 1
 COLA_FEAT_FULL_M, COLA_FEAT_H16, COLA_FEAT_ALL = 1, 2, 3
+COLA_CGNR, COLA_BICGSTAB = 0, 1
+_METHOD = {"cgnr": COLA_CGNR, "bicgstab": COLA_BICGSTAB, COLA_CGNR: COLA_CGNR, COLA_BICGSTAB: COLA_BICGSTAB}
 STATUS_NAMES = {0: "COLA_OK", 1: "COLA_EINVAL", 2: "COLA_ECUDA", 3: "COLA_ENOTREADY", 4: "COLA_ENOCONV", 5: "COLA_ENOMEM"}
 
 EXPORTS = [
@@ -30,6 +32,7 @@ EXPORTS = [
     "cola_mrhs_workspace_bytes", "cola_set_mrhs_workspace", "cola_dslash_apply_mrhs", "cola_fermion_matrix_apply_mrhs",
     "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host", "cola_cg_solve_history", "cola_profile_kernel", "cola_profile_result",
     "cola_set_features", "cola_clover_info", "cola_set_staging",
+    "cola_eig_workspace_bytes", "cola_eig_lowest", "cola_cg_solve_deflated",
 ]
 
 
@@ -43,13 +46,23 @@ class ColaParams(ctypes.Structure):
 
 class ColaSolveParams(ctypes.Structure):
     _fields_ = [("tol", ctypes.c_double), ("max_iter", ctypes.c_int), ("even_odd", ctypes.c_int),
-                ("mixed", ctypes.c_int), ("delta", ctypes.c_double)]
+                ("mixed", ctypes.c_int), ("delta", ctypes.c_double), ("method", ctypes.c_int)]
 
 
 class ColaSolveInfo(ctypes.Structure):
     _fields_ = [("iters", ctypes.c_int), ("reliable_updates", ctypes.c_int),
                 ("iterated_residual", ctypes.c_double), ("true_residual", ctypes.c_double),
                 ("seconds", ctypes.c_double), ("op_flops", ctypes.c_double)]
+
+
+class ColaEigParams(ctypes.Structure):
+    _fields_ = [("n_ev", ctypes.c_int), ("n_kr", ctypes.c_int), ("tol", ctypes.c_double), ("max_restarts", ctypes.c_int),
+                ("cheb_order", ctypes.c_int), ("cheb_lo", ctypes.c_double), ("cheb_hi", ctypes.c_double), ("seed", ctypes.c_uint)]
+
+
+class ColaEigInfo(ctypes.Structure):
+    _fields_ = [("restarts", ctypes.c_int), ("op_applications", ctypes.c_int), ("cheb_lo", ctypes.c_double),
+                ("cheb_hi", ctypes.c_double), ("seconds", ctypes.c_double)]
 
 
 def lib_path() -> str:
@@ -76,6 +89,11 @@ def _load():
                                           ctypes.POINTER(ci), ci]
     lib.cola_set_features.argtypes = [vp, ctypes.c_uint]
     lib.cola_set_staging.argtypes = [vp, ci]
+    lib.cola_eig_workspace_bytes.argtypes = [vp, ctypes.POINTER(ColaEigParams)]
+    lib.cola_eig_workspace_bytes.restype = ctypes.c_size_t
+    lib.cola_eig_lowest.argtypes = [vp, ctypes.POINTER(ColaEigParams), vp, ctypes.c_size_t, ctypes.POINTER(cd), ctypes.POINTER(cd), vp,
+                                    ctypes.POINTER(ColaEigInfo)]
+    lib.cola_cg_solve_deflated.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo), vp, ctypes.POINTER(cd), ci]
     lib.cola_clover_info.argtypes = [vp, ctypes.POINTER(cd)]
     lib.cola_spinor_bytes.argtypes = [vp, ci, ci]
     lib.cola_spinor_bytes.restype = ctypes.c_size_t
@@ -107,7 +125,8 @@ def _load():
     lib.cola_cg_solve_mrhs.argtypes = [vp, ctypes.POINTER(ColaSolveParams), ci, vp, vp, ctypes.POINTER(ColaSolveInfo)]
     for name in EXPORTS:
         fn = getattr(lib, name)
-        if name not in ("cola_last_error", "cola_spinor_bytes", "cola_workspace_bytes", "cola_launch_count", "cola_mrhs_workspace_bytes"):
+        if name not in ("cola_last_error", "cola_spinor_bytes", "cola_workspace_bytes", "cola_launch_count", "cola_mrhs_workspace_bytes",
+                        "cola_eig_workspace_bytes"):
             fn.restype = ci
     return lib
 
@@ -330,9 +349,10 @@ class Cola:
 
     # ---- H9-H12
     @staticmethod
-    def _solve_params(tol, max_iter, even_odd, mixed, delta):
+    def _solve_params(tol, max_iter, even_odd, mixed, delta, method="cgnr"):
         sp = ColaSolveParams()
         sp.tol, sp.max_iter, sp.even_odd, sp.mixed, sp.delta = float(tol), int(max_iter), int(bool(even_odd)), int(mixed), float(delta)
+        sp.method = _METHOD[method]
         return sp
 
     @staticmethod
@@ -340,26 +360,26 @@ class Cola:
         return dict(iters=info.iters, reliable_updates=info.reliable_updates, iterated_residual=info.iterated_residual,
                     true_residual=info.true_residual, seconds=info.seconds, op_flops=info.op_flops, converged=(st == COLA_OK))
 
-    def cg_solve(self, b: torch.Tensor, tol=1e-10, max_iter=20000, even_odd=True, mixed=False, delta=0.1, x: torch.Tensor | None = None):
+    def cg_solve(self, b: torch.Tensor, tol=1e-10, max_iter=20000, even_odd=True, mixed=False, delta=0.1, x: torch.Tensor | None = None, method="cgnr"):
         """b: canonical complex128 [t][z][y][x][4][3].  A CUDA tensor goes through cola_cg_solve, a CPU
         tensor (ideally pinned) through cola_cg_solve_host.  Returns (x, info dict)."""
         assert b.dtype == torch.complex128 and b.numel() == self.V * 12
         b = b.contiguous()
         if x is None:
             x = torch.empty_like(b, pin_memory=True) if not b.is_cuda else torch.empty_like(b)
-        sp = self._solve_params(tol, max_iter, even_odd, mixed, delta)
+        sp = self._solve_params(tol, max_iter, even_odd, mixed, delta, method)
         info = ColaSolveInfo()
         fn = _lib.cola_cg_solve if b.is_cuda else _lib.cola_cg_solve_host
         st = fn(self._h, ctypes.byref(sp), ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), ctypes.byref(info))
         self._ck(st, ok=(COLA_OK, COLA_ENOCONV))
         return x, self._info_dict(info, st)
 
-    def cg_solve_history(self, b: torch.Tensor, tol=1e-10, max_iter=20000, even_odd=True, mixed=False, delta=0.1, hist_len=4096):
+    def cg_solve_history(self, b: torch.Tensor, tol=1e-10, max_iter=20000, even_odd=True, mixed=False, delta=0.1, hist_len=4096, method="cgnr"):
         """cg_solve on a device source that also returns the residual history |r_{k+1}|/|b| of the recurrence."""
         assert b.is_cuda and b.dtype == torch.complex128 and b.numel() == self.V * 12
         b = b.contiguous()
         x = torch.empty_like(b)
-        sp = self._solve_params(tol, max_iter, even_odd, mixed, delta)
+        sp = self._solve_params(tol, max_iter, even_odd, mixed, delta, method)
         info = ColaSolveInfo()
         hist = (ctypes.c_double * hist_len)()
         upd = (ctypes.c_int * 256)()
@@ -390,6 +410,49 @@ class Cola:
             out = torch.empty_like(inp, pin_memory=True)
         self._ck(_lib.cola_fermion_matrix_apply_host(self._h, pr, int(bool(dagger)), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
+
+    # ---- low modes of S^+ S and the deflated start
+    @staticmethod
+    def _eig_params(n_ev, n_kr, tol, max_restarts, cheb_order, cheb_lo, cheb_hi, seed):
+        ep = ColaEigParams()
+        ep.n_ev, ep.n_kr, ep.tol, ep.max_restarts = int(n_ev), int(n_kr), float(tol), int(max_restarts)
+        ep.cheb_order, ep.cheb_lo, ep.cheb_hi, ep.seed = int(cheb_order), float(cheb_lo), float(cheb_hi), int(seed)
+        return ep
+
+    def eig_workspace_bytes(self, n_ev, n_kr=0) -> int:
+        ep = self._eig_params(n_ev, n_kr, 0, 0, 0, 0, 0, 0)
+        return int(_lib.cola_eig_workspace_bytes(self._h, ctypes.byref(ep)))
+
+    def eig_lowest(self, n_ev, n_kr=0, tol=0.0, max_restarts=0, cheb_order=0, cheb_lo=0.0, cheb_hi=0.0, seed=0):
+        """The n_ev smallest eigenpairs of S^+ S.  Returns (evals list, evecs tensor (n_ev, 12, Vh, 2) fp64 internal even
+        half-lattice vectors, info dict with the true residuals)."""
+        ep = self._eig_params(n_ev, n_kr, tol, max_restarts, cheb_order, cheb_lo, cheb_hi, seed)
+        nb = int(_lib.cola_eig_workspace_bytes(self._h, ctypes.byref(ep)))
+        if nb == 0:
+            raise ValueError("n_ev must be 1..32")
+        work = torch.empty(nb, dtype=torch.uint8, device=self.device)
+        evecs = torch.empty((int(n_ev), 12, self.Vh, 2), dtype=torch.float64, device=self.device)
+        ev, rs = (ctypes.c_double * n_ev)(), (ctypes.c_double * n_ev)()
+        info = ColaEigInfo()
+        st = _lib.cola_eig_lowest(self._h, ctypes.byref(ep), ctypes.c_void_p(work.data_ptr()), nb, ev, rs, ctypes.c_void_p(evecs.data_ptr()),
+                                  ctypes.byref(info))
+        self._ck(st, ok=(COLA_OK, COLA_ENOCONV))
+        return list(ev), evecs, dict(residuals=list(rs), restarts=info.restarts, op_applications=info.op_applications, cheb_lo=info.cheb_lo,
+                                     cheb_hi=info.cheb_hi, seconds=info.seconds, converged=(st == COLA_OK))
+
+    def cg_solve_deflated(self, b: torch.Tensor, evals, evecs: torch.Tensor, tol=1e-10, max_iter=20000, mixed=True, delta=0.1):
+        """cg_solve (even-odd CGNR) started from the guess deflated with eigenpairs of S^+ S (eig_lowest's output)."""
+        assert b.is_cuda and b.dtype == torch.complex128 and b.numel() == self.V * 12
+        assert evecs.is_cuda and evecs.is_contiguous() and evecs.dtype == torch.float64 and evecs.numel() == len(evals) * self.Vh * 24
+        b = b.contiguous()
+        x = torch.empty_like(b)
+        sp = self._solve_params(tol, max_iter, True, mixed, delta)
+        info = ColaSolveInfo()
+        ev = (ctypes.c_double * len(evals))(*[float(v) for v in evals])
+        st = _lib.cola_cg_solve_deflated(self._h, ctypes.byref(sp), ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), ctypes.byref(info),
+                                         ctypes.c_void_p(evecs.data_ptr()), ev, len(evals))
+        self._ck(st, ok=(COLA_OK, COLA_ENOCONV))
+        return x, self._info_dict(info, st)
 
     # ---- multi-right-hand-side operators and batched solver (SURVEY 8(f) NEXT-1)
     def mrhs_workspace_bytes(self, nrhs: int, for_solver: bool = True) -> int:

@@ -30,6 +30,9 @@ struct cola_ctx {
     int hist_len;
     int *upd_iters;                 // HOST array receiving the iterations at which reliable updates fired, or nullptr
     int upd_len;
+    const char *defl_vecs;          // DEVICE eigenvectors of S^+S for the deflated start of the running solve, or nullptr
+    const double *defl_evals;       // HOST
+    int defl_n;
     // optional in-solve timing of the dominant kernel (cola_profile_kernel): event pairs around each launch of the
     // fused dslash + clover + xpay kernel of the inner precision
     int prof_on, prof_n;
@@ -44,6 +47,7 @@ struct cola_ctx {
     size_t scratch_bytes;
     // owned
     Ctl *ctl;                       // device
+    CtlB *ctlb;                     // device, inside the control block (BiCGStab scalars)
     unsigned long long *max_dev_bits;   // device (inside the same allocation)
     unsigned long long *min_pivot_key;  // device (inside the same allocation): see launch_clover_invert
     double min_pivot;               // smallest Gauss-Jordan pivot of the 6x6 inverses of the last upload
@@ -133,7 +137,7 @@ static Carve carve(const cola_ctx *c)
     {
         size_t nb = dslash_grid_blocks(Vh);
         if (nb < (size_t)blas_max_blocks()) nb = (size_t)blas_max_blocks();
-        k.partials = take((nb + reduce_groups(nb)) * sizeof(double) + reduce_groups(nb) * sizeof(unsigned));
+        k.partials = take(REDUCE_MAXC * (nb + reduce_groups(nb)) * sizeof(double) + reduce_groups(nb) * sizeof(unsigned));
     }
     k.scratch = take(scratch_half64(c) * 192 * Vh);
     k.total = off;
@@ -155,7 +159,10 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     if (vol / 2 > 2.0e9) return fail(nullptr, COLA_EINVAL, "cola_create: half volume exceeds 32-bit site indices");
     {
         cudaError_t e = cudaSetDevice(p->device);
-        if (e != cudaSuccess) return fail(nullptr, COLA_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e));
+        if (e != cudaSuccess) {
+            cudaGetLastError();   // clear the (non-sticky) error so that it is not reported by a later launch of another context
+            return fail(nullptr, COLA_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e));
+        }
     }
     c = new cola_ctx();
     memset(c, 0, sizeof(*c));
@@ -199,6 +206,8 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     c->ctlm = reinterpret_cast<CtlM *>(blk + 512);
     c->max_dev_bits = reinterpret_cast<unsigned long long *>(blk + 2048);
     c->min_pivot_key = reinterpret_cast<unsigned long long *>(blk + 2056);
+    c->ctlb = reinterpret_cast<CtlB *>(blk + 2304);
+    static_assert(sizeof(CtlB) <= 512, "control block layout");
     *out = c;
     return COLA_OK;
 }
@@ -333,8 +342,10 @@ cola_status cola_set_workspace(cola_ctx *c, void *dev_ptr, size_t bytes)
         if (nb < (size_t)blas_max_blocks()) nb = (size_t)blas_max_blocks();
         c->red_blocks = nb;
         c->red.partials = (double *)(c->ws + k.partials);
-        c->red.gpart = c->red.partials + nb;
-        c->red.gticket = (unsigned *)(c->red.gpart + reduce_groups(nb));
+        c->red.pstride = (unsigned)nb;
+        c->red.gstride = (unsigned)reduce_groups(nb);
+        c->red.gpart = c->red.partials + REDUCE_MAXC * nb;
+        c->red.gticket = (unsigned *)(c->red.gpart + REDUCE_MAXC * reduce_groups(nb));
         cudaError_t e = cudaMemsetAsync(c->red.gticket, 0, reduce_groups(nb) * sizeof(unsigned), c->stream);
         if (e != cudaSuccess) return fail(c, COLA_ECUDA, "cola_set_workspace: %s", cudaGetErrorString(e));
     }
@@ -607,8 +618,12 @@ cola_status axpby64(cola_ctx *c, const System &sy, void *out64, double a, const 
 
 }  // namespace
 
+static cola_status solve_bicgstab_impl(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info);
+
 static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info)
 {
+    if (c && sp && sp->method == COLA_BICGSTAB) return solve_bicgstab_impl(c, sp, b_canon_dev, x_canon_dev, info);
+    if (c && sp && sp->method != COLA_CGNR) return fail(c, COLA_EINVAL, "cola_cg_solve: unknown method");
     ST(need_ready(c, "cola_cg_solve"));
     if (!sp || !b_canon_dev || !x_canon_dev || !info) return fail(c, COLA_EINVAL, "cola_cg_solve: NULL argument");
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve: tol must be > 0 and max_iter >= 1");
@@ -681,9 +696,25 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
         char *xi = sp->mixed ? x32 : xsol, *ri = sp->mixed ? r32 : r, *pi = sp->mixed ? p32 : p, *qi = sp->mixed ? qs32 : qs;
         const size_t nvi = sp->mixed ? nv32 : nv64;
         const int nh = sy.even_odd ? 1 : 2;
+        const bool deflate = c->defl_vecs && c->defl_n > 0 && sy.even_odd;
+        if (deflate) {
+            // x0_e = sum_i u_i <u_i, S^+ bhat_e> / lambda_i  (eigenpairs of S^+ S), r0 = bhat_e - S x0_e
+            ST(apply_K(c, sy, COLA_F64, 1, rhs, qs, nullptr));
+            flops += flops_K;
+            for (int i = 0; i < c->defl_n; i++) {
+                const char *u = c->defl_vecs + (size_t)i * h64;
+                CK(launch_eig_cdot(u, qs, c->Vh, c->red, &ctl->counter[2], &ctl->aux[0], c->stream));
+                CK(launch_eig_caxpy(xsol, u, c->Vh, &ctl->aux[0], 1.0 / c->defl_evals[i], c->stream));
+                c->launches += 2;
+            }
+            ST(apply_K(c, sy, COLA_F64, 0, xsol, qs, nullptr));
+            flops += flops_K;
+        }
         if (sp->mixed) {
             CK(cudaMemsetAsync(x32, 0, nv32, c->stream));
-            ST(axpby64(c, sy, r, 1.0, rhs, 0.0, nullptr, r32));         // r64 = rhs, r32 = float(r64)
+            ST(axpby64(c, sy, r, 1.0, rhs, deflate ? -1.0 : 0.0, deflate ? qs : nullptr, r32));   // r64 = rhs [- S x0], r32 = float(r64)
+        } else if (deflate) {
+            ST(axpby64(c, sy, r, 1.0, rhs, -1.0, qs, nullptr));
         } else {
             CK(cudaMemcpyAsync(r, rhs, nv64, cudaMemcpyDeviceToDevice, c->stream));
         }
@@ -784,6 +815,442 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
     info->op_flops = flops;
     if (!status_conv) return fail(c, COLA_ENOCONV, "cola_cg_solve: max_iter reached before |r| <= tol*|b|");
     return COLA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// BiCGStab on the Schur complement ("solvers for linear systems"), van der Vorst's order as in
+// oracle_bicgstab, x0 = 0, rhat = r0.  One pass = S p and S s (4 fused dslash launches) + 5 BLAS launches:
+//   v = S p;  rv = <rhat, v>;  s = r - alpha v;  t = S s (|t|^2 fused);  ts = <t, s>;
+//   x += alpha p + omega s, r = s - omega t, |r|^2, rho' = <rhat, r>, beta, decision;   p = r + beta (p - omega v)
+// alpha, omega, beta are formed on the device (CtlB); the host queues half a pass ahead and polls the status the x/r
+// update publishes, exactly as in the CGNR driver.  With `mixed` the pass runs in fp32 (or on the 16-bit fields) and
+// reliable updates recompute the fp64 residual, keep p and v and re-form rho' with the replaced residual (SURVEY O8's
+// schedule applied to BiCGStab).
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+cola_status bicg_first_half(cola_ctx *c, const System &sy, cola_prec P, int k, char *xi, char *ri, char *rhat, char *pi, char *vi, char *si, char *ti)
+{
+    CtlB *cb = c->ctlb;
+    ST(apply_K(c, sy, P, 0, pi, vi, nullptr, &cb->flag));
+    CK(launch_bicg_dot(P, rhat, vi, cb, 0, &cb->flag, sy.n_sites, c->red, c->stream));
+    CK(launch_bicg_s_update(P, si, ri, vi, cb, &cb->flag, sy.n_sites, c->stream));
+    ST(apply_K(c, sy, P, 0, si, ti, &cb->tt, &cb->flag));
+    CK(launch_bicg_dot(P, ti, si, cb, 1, &cb->flag, sy.n_sites, c->red, c->stream));
+    CK(launch_bicg_xr_update(P, xi, ri, pi, si, ti, rhat, cb, k + 1, &cb->flag, c->d_status + (k & 1), sy.n_sites, c->red, c->stream));
+    c->launches += 4;
+    return COLA_OK;
+}
+
+cola_status bicg_set_decision_state(cola_ctx *c, double rmax2, double target2, double delta2, int iters)
+{
+    struct { double rmax2, target2, delta2; int flag, iters; } st = {rmax2, target2, delta2, 0, iters};
+    static_assert(offsetof(CtlB, iters) - offsetof(CtlB, rmax2) == 28, "decision block layout");
+    CK(cudaMemcpyAsync(&c->ctlb->rmax2, &st, sizeof(st), cudaMemcpyHostToDevice, c->stream));
+    return COLA_OK;
+}
+
+}  // namespace
+
+static cola_status solve_bicgstab_impl(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info)
+{
+    ST(need_ready(c, "cola_cg_solve"));
+    if (!sp || !b_canon_dev || !x_canon_dev || !info) return fail(c, COLA_EINVAL, "cola_cg_solve: NULL argument");
+    if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve: tol must be > 0 and max_iter >= 1");
+    CK(cudaSetDevice(c->p.device));
+    memset(info, 0, sizeof(*info));
+    if (sp->mixed < 0 || sp->mixed > 2) return fail(c, COLA_EINVAL, "cola_cg_solve: mixed must be 0, 1 or 2");
+    if (!sp->even_odd) return fail(c, COLA_EINVAL, "cola_cg_solve: BiCGStab is offered on the Schur system only (even_odd = 1)");
+    if (sp->mixed == 2) ST(check_prec(c, COLA_F32_H16, 0, 0));
+    c->sloppy16 = sp->mixed == 2;
+    const double delta = sp->delta > 0 ? sp->delta : 0.1;
+    const double kappa = c->p.kappa;
+    const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32);
+    System sy;
+    sy.even_odd = 1;
+    sy.n_sites = c->Vh;
+    const double flops_K = 3696.0 * (double)c->Vh;
+    double flops = 0.0;
+
+    // scratch (9 fp64 half slots, as the even-odd CGNR): B 2, X 2, rhs 1, r 1, qs 1, F 2.  During the passes X's odd half
+    // is free (x_o is reconstructed at the end) and, in the mixed mode, qs is only live inside a reliable update, when the
+    // temporaries s and t of the pass are dead.
+    char *sc = c->scratch;
+    char *B = sc; sc += 2 * h64;
+    char *X = sc; sc += 2 * h64;
+    char *rhs = sc; sc += h64;
+    char *r = sc; sc += h64;
+    char *qs = sc; sc += h64;
+    char *F = sc; sc += 2 * h64;
+    if ((size_t)(sc - c->scratch) > c->scratch_bytes) return fail(c, COLA_ENOMEM, "cola_cg_solve: internal scratch too small");
+    char *xsol = X;
+    char *xi, *ri, *rhat, *pi, *vi, *si, *ti;
+    if (sp->mixed) {
+        xi = F; ri = F + h32; rhat = F + 2 * h32; pi = F + 3 * h32;
+        vi = X + h64;
+        si = qs; ti = qs + h32;
+    } else {
+        xi = xsol; ri = r; rhat = rhs; pi = F; si = F + h64; vi = qs; ti = X + h64;
+    }
+    const cola_prec P = sp->mixed ? COLA_F32 : COLA_F64;
+    const size_t nvi = sp->mixed ? h32 : h64;
+
+    Ctl *ctl = c->ctl;
+    CtlB *cb = c->ctlb;
+    CK(cudaEventRecord(c->ev0, c->stream));
+    CK(launch_spinor_pack(COLA_F64, c->g, b_canon_dev, B, c->stream));
+    c->launches++;
+    double bb = 0.0;
+    ST(norm2(c, COLA_F64, B, c->V, &ctl->aux[2]));
+    ST(read_scalar(c, &ctl->aux[2], &bb));
+    if (!(bb <= DBL_MAX)) return fail(c, COLA_EINVAL, "cola_cg_solve: the source contains NaN or Inf");
+    CK(cudaMemsetAsync(X, 0, 2 * h64, c->stream));
+    const double bnorm = sqrt(bb);
+    int status_conv = 0;
+    double rr = 0.0;
+    int iters = 0, updates = 0;
+
+    if (bb > 0.0) {
+        CK(launch_clover_apply(COLA_F64, c->g, c->clovI64, B + h64, c->tmp64, c->stream));
+        c->launches++;
+        ST(dslash(c, COLA_F64, 0, 0, c->tmp64, rhs, B, 0, kappa, 0, nullptr, 0));     // bhat_e = b_e + kappa D_eo A_oo^-1 b_o
+        flops += (504.0 + 1320.0 + 48.0) * (double)c->Vh;
+        const double target2 = (sp->tol * bnorm) * (sp->tol * bnorm);
+        const double delta2 = sp->mixed ? delta * delta : 0.0;
+        if (sp->mixed) {
+            CK(cudaMemsetAsync(xi, 0, h32, c->stream));
+            ST(axpby64(c, sy, r, 1.0, rhs, 0.0, nullptr, ri));                       // r64 = rhs, r32 = float(r64)
+            CK(cudaMemcpyAsync(rhat, ri, h32, cudaMemcpyDeviceToDevice, c->stream));
+        } else {
+            CK(cudaMemcpyAsync(ri, rhs, h64, cudaMemcpyDeviceToDevice, c->stream));
+        }
+        CK(cudaMemcpyAsync(pi, ri, nvi, cudaMemcpyDeviceToDevice, c->stream));
+        ST(norm2(c, COLA_F64, sp->mixed ? r : ri, sy.n_sites, &ctl->rr));
+        ST(read_scalar(c, &ctl->rr, &rr));
+        status_conv = rr <= target2;
+        if (!status_conv) {
+            CtlB init;
+            memset(&init, 0, sizeof(init));
+            init.rv[0] = init.ts[0] = init.tt = 1.0;    // so that the beta formed with rho_next below is a number (it is not used)
+            init.rho[0] = 1.0;
+            init.rmax2 = rr; init.target2 = target2; init.delta2 = delta2;
+            CK(cudaMemcpyAsync(cb, &init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
+            CK(launch_bicg_dot(P, rhat, ri, cb, 2, nullptr, sy.n_sites, c->red, c->stream));   // rho_1 = <rhat, r_0>
+            c->launches++;
+            c->h_status[0].iters = c->h_status[1].iters = 0;
+            ST(bicg_first_half(c, sy, P, 0, xi, ri, rhat, pi, vi, si, ti));
+            for (int k = 0;; k++) {
+                const int more = (k + 1 < sp->max_iter);
+                CK(launch_bicg_p_update(P, pi, ri, vi, cb, &cb->flag, sy.n_sites, c->stream));      // speculative: skipped if pass k raises the flag
+                c->launches++;
+                if (more) ST(bicg_first_half(c, sy, P, k + 1, xi, ri, rhat, pi, vi, si, ti));
+                HostStatus hs;
+                ST(wait_status(c, k, &hs));
+                rr = hs.rr;
+                iters = k + 1;
+                if (c->hist && k < c->hist_len) c->hist[k] = sqrt(rr) / bnorm;
+                if (!(rr <= DBL_MAX)) {
+                    CK(cudaStreamSynchronize(c->stream));
+                    return fail(c, COLA_EINVAL, "cola_cg_solve: BiCGStab broke down or met NaN/Inf (<rhat, v>, <t, t> or rho vanished, or bad input)");
+                }
+                flops += 2 * flops_K;
+                if (!hs.flag) {
+                    if (!more) break;
+                    continue;
+                }
+                if (!sp->mixed) { status_conv = 1; break; }
+                CK(launch_accumulate(xsol, xi, c->Vh, c->stream));                   // x64 += x32, x32 = 0
+                c->launches++;
+                ST(apply_K(c, sy, COLA_F64, 0, xsol, qs, nullptr));
+                flops += flops_K;
+                ST(axpby64(c, sy, r, 1.0, rhs, -1.0, qs, ri));                        // r64 = rhs - S x64, r32 = float(r64)
+                ST(norm2(c, COLA_F64, r, sy.n_sites, &ctl->rr));
+                ST(read_scalar(c, &ctl->rr, &rr));
+                if (c->upd_iters && updates < c->upd_len) c->upd_iters[updates] = k + 1;
+                updates++;
+                if (!(rr <= DBL_MAX)) return fail(c, COLA_EINVAL, "cola_cg_solve: the fp64 residual is not a number (NaN or Inf in the gauge field)");
+                if (rr <= target2) { status_conv = 1; break; }
+                if (!more) break;
+                ST(bicg_set_decision_state(c, rr, target2, delta2, k + 1));            // rmax = |r64|, flag down
+                CK(launch_bicg_dot(P, rhat, ri, cb, 2, nullptr, sy.n_sites, c->red, c->stream));   // rho' and beta with the replaced residual
+                CK(launch_bicg_p_update(P, pi, ri, vi, cb, nullptr, sy.n_sites, c->stream));   // same p and v: p = r + beta (p - omega v)
+                c->launches += 2;
+                ST(bicg_first_half(c, sy, P, k + 1, xi, ri, rhat, pi, vi, si, ti));
+            }
+            if (!status_conv && sp->mixed) {
+                CK(launch_accumulate(xsol, xi, c->Vh, c->stream));
+                c->launches++;
+            }
+        }
+        ST(dslash(c, COLA_F64, 1, 0, X, X + h64, B + h64, 0, kappa, 1, nullptr, 0));   // x_o = A_oo^-1 (b_o + kappa D_oe x_e)
+        flops += (1320.0 + 48.0 + 504.0) * (double)c->Vh;
+    } else {
+        status_conv = 1;
+    }
+    info->iterated_residual = bb > 0 ? sqrt(rr) / bnorm : 0.0;
+    {
+        char *t = rhs;          // rhs (1 half) + r (1 half) are contiguous
+        ST(fmatrix(c, COLA_F64, 0, X, t, nullptr));
+        flops += 1872.0 * (double)c->V;
+        for (int h = 0; h < 2; h++) {
+            CK(launch_axpby64(nullptr, 1.0, B + h * h64, -1.0, t + h * h64, nullptr, c->Vh, &c->red, &c->ctl->counter[3], &ctl->aux[h], c->stream));
+            c->launches++;
+        }
+        double a0, a1;
+        ST(read_scalar(c, &ctl->aux[0], &a0));
+        ST(read_scalar(c, &ctl->aux[1], &a1));
+        info->true_residual = bb > 0 ? sqrt(a0 + a1) / bnorm : 0.0;
+    }
+    CK(launch_spinor_unpack(COLA_F64, c->g, X, x_canon_dev, c->stream));
+    c->launches++;
+    CK(cudaEventRecord(c->ev1, c->stream));
+    CK(cudaEventSynchronize(c->ev1));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+    info->seconds = ms * 1e-3;
+    info->iters = iters;
+    info->reliable_updates = updates;
+    info->op_flops = flops;
+    if (!status_conv) return fail(c, COLA_ENOCONV, "cola_cg_solve: max_iter reached before |r| <= tol*|b|");
+    return COLA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Low modes of H = S^+ S by thick-restart Lanczos on a Chebyshev polynomial of H (include/cola.h).
+// With A' = ((hi + lo) - 2 H) / (hi - lo) the eigenvalues of H below lo map to A' > 1 and T_p(A') grows like
+// cosh(p acosh A') there, while [lo, hi] stays inside [-1, 1]: the wanted modes become the LARGEST, well separated
+// eigenvalues of Op = T_p(A'), which Lanczos finds in a few restarts.  Each step orthogonalises the new vector against the
+// whole basis (classical Gram-Schmidt, twice), so the projected matrix T_ij = <v_i, Op v_j> is taken from the dots as
+// they come; at a restart the basis is rotated onto the best Ritz vectors and the last Lanczos vector is kept (Wu &
+// Simon's thick restart).  Eigenvalues of H are the Rayleigh quotients of the final Ritz vectors.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+struct EigPlan {
+    int n_ev, m, keep, p, max_restarts;
+    double tol;
+    size_t nvec, scal_off, total;
+};
+
+EigPlan eig_plan(const cola_ctx *c, const cola_eig_params *ep)
+{
+    EigPlan q;
+    memset(&q, 0, sizeof(q));
+    q.n_ev = ep->n_ev;
+    q.m = ep->n_kr > 0 ? ep->n_kr : 2 * ep->n_ev + 8;
+    if (q.m > 64) q.m = 64;
+    q.keep = (q.m + q.n_ev) / 2;
+    q.p = ep->cheb_order > 0 ? ep->cheb_order : 24;
+    q.max_restarts = ep->max_restarts > 0 ? ep->max_restarts : 100;
+    q.tol = ep->tol > 0 ? ep->tol : 1e-10;
+    q.nvec = (size_t)q.m + 1 + (size_t)q.keep + 4;          // basis, rotation target, w, two Chebyshev vectors, S x
+    q.scal_off = align_up(q.nvec * half_bytes(c, COLA_F64));
+    q.total = q.scal_off + align_up((size_t)(2 * (q.m + 4) + q.m * q.m) * sizeof(double));
+    return q;
+}
+
+}  // namespace
+
+extern "C" size_t cola_eig_workspace_bytes(const cola_ctx *c, const cola_eig_params *ep)
+{
+    if (!c || !ep || ep->n_ev < 1 || ep->n_ev > 32) return 0;
+    return eig_plan(c, ep).total;
+}
+
+extern "C" cola_status cola_eig_lowest(cola_ctx *c, const cola_eig_params *ep, void *work_dev, size_t work_bytes, double *evals_host, double *resid_host,
+                                       void *evecs_dev, cola_eig_info *info)
+{
+    ST(need_ready(c, "cola_eig_lowest"));
+    if (!ep || !work_dev || !evals_host || !resid_host || !info) return fail(c, COLA_EINVAL, "cola_eig_lowest: NULL argument");
+    if (ep->n_ev < 1 || ep->n_ev > 32) return fail(c, COLA_EINVAL, "cola_eig_lowest: n_ev must be 1..32");
+    const EigPlan q = eig_plan(c, ep);
+    if (q.m < q.n_ev + 2) return fail(c, COLA_EINVAL, "cola_eig_lowest: n_kr must be at least n_ev + 2 (and at most 64)");
+    if ((size_t)q.m > 12 * c->Vh) return fail(c, COLA_EINVAL, "cola_eig_lowest: the Krylov space is larger than the lattice's vector space");
+    if (((uintptr_t)work_dev & 255) || work_bytes < q.total) return fail(c, COLA_ENOMEM, "cola_eig_lowest: workspace misaligned or smaller than cola_eig_workspace_bytes()");
+    CK(cudaSetDevice(c->p.device));
+    memset(info, 0, sizeof(*info));
+    const size_t h64 = half_bytes(c, COLA_F64), Vh = c->Vh;
+    const int m = q.m, n_ev = q.n_ev, keep = q.keep, p = q.p;
+    char *base = (char *)work_dev;
+    auto vec = [&](size_t i) { return base + i * h64; };
+    char *V = vec(0);                              // m + 1 basis vectors
+    char *R = vec((size_t)m + 1);                  // keep rotated vectors
+    char *W = vec((size_t)m + 1 + keep), *T0 = W + h64, *T1 = T0 + h64, *U = T1 + h64;
+    double *coef = (double *)(base + q.scal_off);  // 2 (m + 4) doubles: dots
+    double *Ydev = coef + 2 * (m + 4);
+    double *hcoef = new double[2 * (m + 4)];
+    double *Tm = new double[(size_t)m * m], *Tw = new double[(size_t)m * m], *th = new double[m], *Y = new double[(size_t)m * m], *Ysel = new double[(size_t)m * m];
+    auto cleanup = [&]() { delete[] hcoef; delete[] Tm; delete[] Tw; delete[] th; delete[] Y; delete[] Ysel; };
+    int ops = 0;
+#define EK(call)                                                                                          \
+    do {                                                                                                  \
+        cudaError_t e__ = (call);                                                                         \
+        if (e__ != cudaSuccess) { cleanup(); return fail(c, COLA_ECUDA, "%s: %s", #call, cudaGetErrorString(e__)); } \
+    } while (0)
+#define ES(call)                                      \
+    do {                                              \
+        cola_status s__ = (call);                     \
+        if (s__ != COLA_OK) { cleanup(); return s__; } \
+    } while (0)
+    auto H = [&](const char *x, char *out) -> cola_status {     // out = S^+ S x
+        ST(schur(c, COLA_F64, 0, x, U, nullptr));
+        ST(schur(c, COLA_F64, 1, U, out, nullptr));
+        ops++;
+        return COLA_OK;
+    };
+    auto fetch = [&](int n2) -> cola_status {                   // coef[0 .. n2) -> hcoef
+        CK(cudaMemcpyAsync(hcoef, coef, sizeof(double) * n2, cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        return COLA_OK;
+    };
+    EK(cudaEventRecord(c->ev0, c->stream));
+    // start vector, normalised
+    EK(launch_eig_start(W, Vh, 0x2302008500ull + ep->seed, c->stream));
+    EK(launch_eig_cdot(W, W, Vh, c->red, &c->ctl->counter[2], coef, c->stream));
+    EK(launch_eig_normalise(V, W, Vh, coef, c->stream));
+    // filter window
+    double hi = ep->cheb_hi, lo = ep->cheb_lo;
+    if (!(hi > 0)) {   // power iteration on H from the start vector: a lower bound of lambda_max, widened by 15 %
+        EK(cudaMemcpyAsync(T0, V, h64, cudaMemcpyDeviceToDevice, c->stream));
+        double lam = 0.0;
+        for (int it = 0; it < 20; it++) {
+            ES(H(T0, T1));
+            EK(launch_eig_cdot(T1, T1, Vh, c->red, &c->ctl->counter[2], coef, c->stream));
+            EK(launch_eig_normalise(T0, T1, Vh, coef, c->stream));
+            ES(fetch(2));
+            lam = sqrt(hcoef[0]);     // |H x| with |x| = 1
+        }
+        hi = 1.15 * lam;
+    }
+    if (!(lo > 0) || lo >= hi) lo = hi / 10.0;
+    info->cheb_lo = lo;
+    info->cheb_hi = hi;
+    const double ca = -2.0 / (hi - lo), cb = (hi + lo) / (hi - lo);   // A' = ca H + cb
+    auto Op = [&](const char *x, char *out) -> cola_status {   // out = T_p(A') x
+        ST(H(x, out));
+        // t1 = ca H x + cb x
+        char *t1 = out;
+        CK(launch_eig_lincomb(t1, ca, t1, cb, x, 0.0, nullptr, Vh, c->stream));
+        if (p == 1) return COLA_OK;
+        // three-term recurrence with t0 = x: t_{k+1} = 2 A' t_k - t_{k-1}; buffers rotate between out, T0, T1
+        char *tkm1 = T0, *tk = T1, *tn = out;
+        CK(cudaMemcpyAsync(tkm1, x, h64, cudaMemcpyDeviceToDevice, c->stream));
+        CK(cudaMemcpyAsync(tk, t1, h64, cudaMemcpyDeviceToDevice, c->stream));
+        for (int k = 1; k < p; k++) {
+            ST(H(tk, tn));
+            CK(launch_eig_lincomb(tn, 2.0 * ca, tn, 2.0 * cb, tk, -1.0, tkm1, Vh, c->stream));
+            char *old = tkm1;
+            tkm1 = tk; tk = tn; tn = old;
+        }
+        if (tk != out) CK(cudaMemcpyAsync(out, tk, h64, cudaMemcpyDeviceToDevice, c->stream));
+        return COLA_OK;
+    };
+
+    memset(Tm, 0, sizeof(double) * m * m);
+    int k0 = 0, restarts = 0, converged = 0;
+    double beta_m = 0.0;
+    for (;; restarts++) {
+        for (int j = k0; j < m; j++) {
+            ES(Op(vec(j), W));
+            // classical Gram-Schmidt against v_0 .. v_j, twice; the first-pass dots are column j of T
+            for (int pass = 0; pass < 2; pass++) {
+                for (int i = 0; i <= j; i++) EK(launch_eig_cdot(vec(i), W, Vh, c->red, &c->ctl->counter[2], coef + 2 * i, c->stream));
+                for (int i = 0; i <= j; i++) EK(launch_eig_caxpy(W, vec(i), Vh, coef + 2 * i, -1.0, c->stream));
+                ES(fetch(2 * (j + 1)));
+                for (int i = 0; i <= j; i++) {
+                    if (pass == 0) Tm[i * m + j] = Tm[j * m + i] = hcoef[2 * i];
+                    else Tm[i * m + j] = (Tm[j * m + i] += hcoef[2 * i]);
+                }
+            }
+            EK(launch_eig_cdot(W, W, Vh, c->red, &c->ctl->counter[2], coef, c->stream));
+            EK(launch_eig_normalise(vec(j + 1), W, Vh, coef, c->stream));
+            ES(fetch(2));
+            beta_m = sqrt(hcoef[0]);
+            if (!(beta_m <= DBL_MAX)) { cleanup(); return fail(c, COLA_EINVAL, "cola_eig_lowest: the Lanczos vector is not a number (NaN or Inf in the gauge field?)"); }
+            c->launches += 4 * (j + 1) + 2;
+        }
+        memcpy(Tw, Tm, sizeof(double) * m * m);
+        jacobi_eigh(m, Tw, th, Y);                                  // ascending: the wanted pairs are the LAST n_ev
+        double worst = 0.0;
+        for (int q2 = 0; q2 < n_ev; q2++) {
+            const double est = fabs(beta_m * Y[(m - 1) * m + (m - 1 - q2)]);
+            if (est > worst) worst = est;
+        }
+        converged = worst <= q.tol * fabs(th[m - 1]);
+        if (converged || restarts + 1 >= q.max_restarts) break;
+        // thick restart: keep the `keep` largest Ritz pairs and the last Lanczos vector
+        for (int j = 0; j < m; j++)
+            for (int q2 = 0; q2 < keep; q2++) Ysel[j * keep + q2] = Y[j * m + (m - 1 - q2)];
+        EK(cudaMemcpyAsync(Ydev, Ysel, sizeof(double) * m * keep, cudaMemcpyHostToDevice, c->stream));
+        EK(launch_eig_rotate(R, V, h64, m, keep, Ydev, Vh, c->stream));
+        EK(cudaMemcpyAsync(V, R, (size_t)keep * h64, cudaMemcpyDeviceToDevice, c->stream));
+        EK(cudaMemcpyAsync(vec(keep), vec(m), h64, cudaMemcpyDeviceToDevice, c->stream));
+        EK(cudaStreamSynchronize(c->stream));                      // Ysel is reused by the host
+        memset(Tm, 0, sizeof(double) * m * m);
+        for (int q2 = 0; q2 < keep; q2++) {
+            Tm[q2 * m + q2] = th[m - 1 - q2];
+            Tm[q2 * m + keep] = Tm[keep * m + q2] = beta_m * Y[(m - 1) * m + (m - 1 - q2)];
+        }
+        k0 = keep;
+    }
+    // final Ritz vectors of the wanted pairs -> R[0 .. n_ev), Rayleigh quotients and true residuals with H
+    for (int j = 0; j < m; j++)
+        for (int q2 = 0; q2 < n_ev; q2++) Ysel[j * n_ev + q2] = Y[j * m + (m - 1 - q2)];
+    EK(cudaMemcpyAsync(Ydev, Ysel, sizeof(double) * m * n_ev, cudaMemcpyHostToDevice, c->stream));
+    EK(launch_eig_rotate(R, V, h64, m, n_ev, Ydev, Vh, c->stream));
+    double lam[32], res[32];
+    int order[32];
+    for (int q2 = 0; q2 < n_ev; q2++) {
+        char *u = R + (size_t)q2 * h64;
+        EK(launch_eig_cdot(u, u, Vh, c->red, &c->ctl->counter[2], coef, c->stream));     // renormalise (rotation rounding)
+        EK(launch_eig_normalise(u, u, Vh, coef, c->stream));
+        ES(H(u, W));
+        EK(launch_eig_cdot(u, W, Vh, c->red, &c->ctl->counter[2], coef + 2, c->stream));
+        EK(launch_eig_caxpy(W, u, Vh, coef + 2, -1.0, c->stream));
+        EK(launch_eig_cdot(W, W, Vh, c->red, &c->ctl->counter[2], coef + 4, c->stream));
+        ES(fetch(6));
+        lam[q2] = hcoef[2];
+        res[q2] = sqrt(hcoef[4]);
+        order[q2] = q2;
+    }
+    for (int a = 0; a < n_ev; a++)
+        for (int b2 = a + 1; b2 < n_ev; b2++)
+            if (lam[order[b2]] < lam[order[a]]) { const int t = order[a]; order[a] = order[b2]; order[b2] = t; }
+    for (int a = 0; a < n_ev; a++) {
+        evals_host[a] = lam[order[a]];
+        resid_host[a] = res[order[a]];
+        if (evecs_dev) EK(cudaMemcpyAsync((char *)evecs_dev + (size_t)a * h64, R + (size_t)order[a] * h64, h64, cudaMemcpyDeviceToDevice, c->stream));
+    }
+    EK(cudaEventRecord(c->ev1, c->stream));
+    EK(cudaEventSynchronize(c->ev1));
+    float ms = 0.f;
+    EK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+    info->seconds = ms * 1e-3;
+    info->restarts = restarts + 1;
+    info->op_applications = ops;
+    cleanup();
+#undef EK
+#undef ES
+    if (!converged) return fail(c, COLA_ENOCONV, "cola_eig_lowest: max_restarts reached before the residual estimates met tol");
+    return COLA_OK;
+}
+
+extern "C" cola_status cola_cg_solve_deflated(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info,
+                                              const void *evecs_dev, const double *evals_host, int n_ev)
+{
+    if (!c) return COLA_EINVAL;
+    if (!evecs_dev || !evals_host || n_ev < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_deflated: NULL or empty eigenpairs");
+    if (!sp || !sp->even_odd || sp->method != COLA_CGNR) return fail(c, COLA_EINVAL, "cola_cg_solve_deflated: needs even_odd = 1 and method = COLA_CGNR");
+    for (int i = 0; i < n_ev; i++)
+        if (!(evals_host[i] > 0)) return fail(c, COLA_EINVAL, "cola_cg_solve_deflated: eigenvalues of S^+S must be positive");
+    c->defl_vecs = (const char *)evecs_dev;
+    c->defl_evals = evals_host;
+    c->defl_n = n_ev;
+    const cola_status st = solve_impl(c, sp, b_canon_dev, x_canon_dev, info);
+    c->defl_vecs = nullptr;
+    c->defl_evals = nullptr;
+    c->defl_n = 0;
+    return st;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -954,8 +1421,8 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
     ST(need_mrhs(c, "cola_cg_solve_mrhs", nrhs));
     if (!sp || !b_canon_dev || !x_canon_dev || !infos) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: NULL argument");
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: tol must be > 0 and max_iter >= 1");
-    if (!sp->even_odd || sp->mixed < 1 || sp->mixed > 2)
-        return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd solver is batched (even_odd = 1, mixed = 1 or 2)");
+    if (!sp->even_odd || sp->mixed < 1 || sp->mixed > 2 || sp->method != COLA_CGNR)
+        return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd CGNR solver is batched (even_odd = 1, mixed = 1 or 2, method = COLA_CGNR)");
     if (sp->mixed == 2) ST(check_prec(c, COLA_F32_H16, 0, 0));
     if (!c->m_solver) return fail(c, COLA_ENOTREADY, "cola_cg_solve_mrhs: the multi-rhs workspace was sized for operators only (cola_mrhs_workspace_bytes with for_solver = 1)");
     c->sloppy16 = sp->mixed == 2;

@@ -124,6 +124,132 @@ __global__ void __launch_bounds__(BB) accumulate_kernel(double2 *x64, float4 *x3
     }
 }
 
+// ---- BiCGStab.  A float4 chunk holds two complex numbers, a double2 chunk one; alpha, omega, beta
+// are formed in fp64 from the device-resident dots (CtlB) by every thread and applied in the vectors' precision.
+struct Cx { double re, im; };
+__device__ __forceinline__ Cx cdiv(const double (&a)[2], const double (&b)[2])
+{
+    const double d = b[0] * b[0] + b[1] * b[1];
+    return Cx{(a[0] * b[0] + a[1] * b[1]) / d, (a[1] * b[0] - a[0] * b[1]) / d};
+}
+__device__ __forceinline__ Cx cmul(Cx a, Cx b) { return Cx{a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+// y + c x on a chunk (complex scalar c)
+__device__ __forceinline__ float4 caxpy(float cr, float ci, const float4 &x, const float4 &y)
+{
+    return make_float4(y.x + cr * x.x - ci * x.y, y.y + cr * x.y + ci * x.x, y.z + cr * x.z - ci * x.w, y.w + cr * x.w + ci * x.z);
+}
+__device__ __forceinline__ double2 caxpy(double cr, double ci, const double2 &x, const double2 &y)
+{
+    return make_double2(y.x + cr * x.x - ci * x.y, y.y + cr * x.y + ci * x.x);
+}
+// sum conj(a) b over a chunk, added to (re, im)
+__device__ __forceinline__ void cdot_acc(const float4 &a, const float4 &b, double &re, double &im)
+{
+    re += (double)(a.x * b.x + a.y * b.y + a.z * b.z + a.w * b.w);
+    im += (double)(a.x * b.y - a.y * b.x + a.z * b.w - a.w * b.z);
+}
+__device__ __forceinline__ void cdot_acc(const double2 &a, const double2 &b, double &re, double &im)
+{
+    re += a.x * b.x + a.y * b.y;
+    im += a.x * b.y - a.y * b.x;
+}
+__device__ __forceinline__ Cx bicg_omega(const CtlB *ctl) { return Cx{ctl->ts[0] / ctl->tt, ctl->ts[1] / ctl->tt}; }
+// beta = (rho_next / rho) (alpha / omega), alpha = rho / rv  =>  beta = rho_next / (rv omega)
+__device__ __forceinline__ void bicg_set_beta(CtlB *ctl, const double (&rho_next)[2])
+{
+    const Cx om = bicg_omega(ctl);
+    const Cx den = cmul(Cx{ctl->rv[0], ctl->rv[1]}, om);
+    const double d[2] = {den.re, den.im};
+    const Cx b = cdiv(rho_next, d);
+    ctl->rho_next[0] = rho_next[0];
+    ctl->rho_next[1] = rho_next[1];
+    ctl->beta[0] = b.re;
+    ctl->beta[1] = b.im;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(BB) bicg_dot_kernel(const typename VT<T>::V *a, const typename VT<T>::V *b, CtlB *ctl, int which, const int *skip, size_t n, ReduceWs red)
+{
+    pdl_trigger();
+    pdl_wait();
+    if (skip && *skip) return;
+    double v[2] = {0.0, 0.0};
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) cdot_acc(a[k], b[k], v[0], v[1]);
+    double tot[2];
+    if (grid_sum_last_n<2>(v, red, &ctl->counter[0], tot)) {
+        if (which == 0) {
+            ctl->rv[0] = tot[0]; ctl->rv[1] = tot[1];
+            ctl->rho[0] = ctl->rho_next[0]; ctl->rho[1] = ctl->rho_next[1];
+        } else if (which == 1) {
+            ctl->ts[0] = tot[0]; ctl->ts[1] = tot[1];
+        } else {
+            bicg_set_beta(ctl, tot);
+        }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(BB) bicg_s_update_kernel(typename VT<T>::V *sv, const typename VT<T>::V *r, const typename VT<T>::V *v, const CtlB *ctl, const int *skip, size_t n)
+{
+    pdl_trigger();
+    pdl_wait();
+    if (skip && *skip) return;
+    const Cx al = cdiv(ctl->rho, ctl->rv);
+    const T mr = (T)(-al.re), mi = (T)(-al.im);
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) sv[k] = caxpy(mr, mi, v[k], r[k]);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(BB) bicg_xr_update_kernel(typename VT<T>::V *x, typename VT<T>::V *r, const typename VT<T>::V *p, const typename VT<T>::V *sv,
+                                                            const typename VT<T>::V *t, const typename VT<T>::V *rhat, CtlB *ctl, int iter, const int *skip,
+                                                            HostStatus *mirror, size_t n, ReduceWs red)
+{
+    pdl_trigger();
+    pdl_wait();
+    if (skip && *skip) return;
+    const Cx al = cdiv(ctl->rho, ctl->rv), om = bicg_omega(ctl);
+    const T ar = (T)al.re, ai = (T)al.im, wr = (T)om.re, wi = (T)om.im;
+    double v[3] = {0.0, 0.0, 0.0};
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) {
+        const typename VT<T>::V s_ = sv[k];
+        x[k] = caxpy(wr, wi, s_, caxpy(ar, ai, p[k], x[k]));
+        const typename VT<T>::V rn = caxpy(-wr, -wi, t[k], s_);
+        r[k] = rn;
+        v[0] += sq(rn);
+        cdot_acc(rhat[k], rn, v[1], v[2]);
+    }
+    double tot[3];
+    if (grid_sum_last_n<3>(v, red, &ctl->counter[1], tot)) {
+        const double rr = tot[0];
+        const double rho_next[2] = {tot[1], tot[2]};
+        bicg_set_beta(ctl, rho_next);
+        ctl->rr = rr;
+        ctl->iters = iter;
+        const double rmax2 = fmax(ctl->rmax2, rr);
+        ctl->rmax2 = rmax2;
+        const int flag = (rr <= ctl->target2 || rr < ctl->delta2 * rmax2) ? 1 : 0;
+        if (flag) ctl->flag = 1;
+        if (mirror) {
+            volatile HostStatus *m = mirror;
+            m->rr = rr;
+            m->flag = flag;
+            __threadfence_system();
+            m->iters = iter;
+        }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(BB) bicg_p_update_kernel(typename VT<T>::V *p, const typename VT<T>::V *r, const typename VT<T>::V *v, const CtlB *ctl, const int *skip, size_t n)
+{
+    pdl_trigger();
+    pdl_wait();
+    if (skip && *skip) return;
+    const Cx om = bicg_omega(ctl);
+    const T br = (T)ctl->beta[0], bi = (T)ctl->beta[1], mwr = (T)(-om.re), mwi = (T)(-om.im);
+    for (size_t k = (size_t)blockIdx.x * BB + threadIdx.x; k < n; k += (size_t)gridDim.x * BB) p[k] = caxpy(br, bi, caxpy(mwr, mwi, v[k], p[k]), r[k]);
+}
+
 // ---- batched (multi-right-hand-side) variants: blockIdx.y = position in the list, same arithmetic per vector
 inline unsigned mrhs_grid(size_t n_chunks)
 {
@@ -250,6 +376,41 @@ cudaError_t launch_xp_update_mrhs(cola_prec prec, void *x, void *p, const void *
 #undef COLA_XP
     return cudaGetLastError();
 }
+
+#define COLA_BICG_DISPATCH(KERN, ...)                                                                                        \
+    do {                                                                                                                   \
+        if (prec == COLA_F64) {                                                                                            \
+            typedef double2 V;                                                                                             \
+            const size_t n = 12 * n_sites;                                                                                 \
+            return launch_pdl(KERN<double>, dim3(blas_grid(n)), dim3(BB), s, __VA_ARGS__);                                 \
+        } else {                                                                                                           \
+            typedef float4 V;                                                                                              \
+            const size_t n = 6 * n_sites;                                                                                  \
+            return launch_pdl(KERN<float>, dim3(blas_grid(n)), dim3(BB), s, __VA_ARGS__);                                  \
+        }                                                                                                                  \
+    } while (0)
+
+cudaError_t launch_bicg_dot(cola_prec prec, const void *a, const void *b, CtlB *ctl, int which, const int *skip, size_t n_sites, const ReduceWs &red, cudaStream_t s)
+{
+    COLA_BICG_DISPATCH(bicg_dot_kernel, (const V *)a, (const V *)b, ctl, which, skip, n, red);
+}
+
+cudaError_t launch_bicg_s_update(cola_prec prec, void *sv, const void *r, const void *v, const CtlB *ctl, const int *skip, size_t n_sites, cudaStream_t s)
+{
+    COLA_BICG_DISPATCH(bicg_s_update_kernel, (V *)sv, (const V *)r, (const V *)v, ctl, skip, n);
+}
+
+cudaError_t launch_bicg_xr_update(cola_prec prec, void *x, void *r, const void *p, const void *sv, const void *t, const void *rhat, CtlB *ctl, int iter,
+                                  const int *skip, HostStatus *mirror, size_t n_sites, const ReduceWs &red, cudaStream_t s)
+{
+    COLA_BICG_DISPATCH(bicg_xr_update_kernel, (V *)x, (V *)r, (const V *)p, (const V *)sv, (const V *)t, (const V *)rhat, ctl, iter, skip, mirror, n, red);
+}
+
+cudaError_t launch_bicg_p_update(cola_prec prec, void *p, const void *r, const void *v, const CtlB *ctl, const int *skip, size_t n_sites, cudaStream_t s)
+{
+    COLA_BICG_DISPATCH(bicg_p_update_kernel, (V *)p, (const V *)r, (const V *)v, ctl, skip, n);
+}
+#undef COLA_BICG_DISPATCH
 
 cudaError_t launch_norm2(cola_prec prec, const void *v, size_t n_sites, const ReduceWs &red, unsigned *counter, double *out, cudaStream_t s)
 {

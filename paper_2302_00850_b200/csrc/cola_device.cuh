@@ -360,6 +360,58 @@ __device__ __forceinline__ bool grid_sum_last(double v, const ReduceWs &ws, unsi
     return true;
 }
 
+// The same for N values at once (component c uses partials + c*pstride, gpart + c*gstride; one ticket per group).
+template <int N>
+__device__ __forceinline__ bool grid_sum_last_n(const double (&v)[N], const ReduceWs &ws, unsigned *counter, double (&total)[N])
+{
+    __shared__ double sm[33];
+    __shared__ int stage;
+    static_assert(N <= REDUCE_MAXC, "too many reduction components");
+    const unsigned group = blockIdx.x / REDUCE_GROUP;
+    const unsigned ngroups = (gridDim.x + REDUCE_GROUP - 1) / REDUCE_GROUP;
+    const unsigned first = group * REDUCE_GROUP;
+    const unsigned gsize = min(REDUCE_GROUP, gridDim.x - first);
+    double s[N];
+#pragma unroll
+    for (int c = 0; c < N; c++) s[c] = block_sum(v[c], sm);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int c = 0; c < N; c++) ws.partials[(size_t)c * ws.pstride + blockIdx.x] = s[c];
+        __threadfence();
+        stage = (atomicAdd(ws.gticket + group, 1u) == gsize - 1) ? 1 : 0;
+    }
+    __syncthreads();
+    if (!stage) return false;
+    __threadfence();
+#pragma unroll
+    for (int c = 0; c < N; c++) {
+        double a = 0.0;
+        for (unsigned k = threadIdx.x; k < gsize; k += blockDim.x) a += __ldcg(ws.partials + (size_t)c * ws.pstride + first + k);
+        s[c] = block_sum(a, sm);
+    }
+    if (threadIdx.x == 0) {
+        ws.gticket[group] = 0u;
+#pragma unroll
+        for (int c = 0; c < N; c++) ws.gpart[(size_t)c * ws.gstride + group] = s[c];
+        __threadfence();
+        stage = (atomicAdd(counter, 1u) == ngroups - 1) ? 2 : 0;
+    }
+    __syncthreads();
+    if (stage != 2) return false;
+    __threadfence();
+#pragma unroll
+    for (int c = 0; c < N; c++) {
+        double a = 0.0;
+        for (unsigned k = threadIdx.x; k < ngroups; k += blockDim.x) a += __ldcg(ws.gpart + (size_t)c * ws.gstride + k);
+        s[c] = block_sum(a, sm);
+    }
+    if (threadIdx.x != 0) return false;
+    *counter = 0u;
+#pragma unroll
+    for (int c = 0; c < N; c++) total[c] = s[c];
+    return true;
+}
+
 __device__ __forceinline__ void grid_sum_finalize(double v, const ReduceWs &ws, unsigned *counter, double *result, bool accumulate = false)
 {
     double a;

@@ -10,9 +10,11 @@
 //
 // How.  A block owns a 4-D tile of output sites, Xh x TY x TZ x TT in checkerboard coordinates (full rows in x, so the
 // x neighbours wrap inside the row).  It copies the tile's input spinors and the six faces next to it (y-, y+, z-,
-// z+, t-, t+) from global to shared memory with cp.async (16 bytes per copy, L1 bypassed, no registers), each input
-// spinor ONCE per tile instead of once per use: 3.5-4 spinor loads per site instead of ~6.7 through L2.  After one
-// barrier every thread runs the 8 hops of its site reading neighbours with LDS.128; only the links (read exactly once,
+// z+, t-, t+) from global to shared memory with TMA bulk copies (cp.async.bulk, one per contiguous run of rows; an
+// mbarrier counts the bytes), each input spinor ONCE per tile instead of once per use: 3.5-4 spinor loads per site
+// instead of ~6 through L2.  (A first version issued one 16-byte cp.async per thread and chunk: +37 % executed
+// instructions and, with L1 bypassed, 2x the expected L2->L1 bytes -- 20-28 % slower than the direct kernels.)  After
+// the barrier every thread runs the 8 hops of its site reading neighbours with LDS.128; only the links (read exactly once,
 // no reuse to exploit) still come from global memory, software-pipelined two hops ahead in registers and, with
 // programmatic dependent launch, requested before the wait on the previous kernel (the gauge field is constant).
 // The arithmetic of a site is the same sequence of calls as in the direct kernels (cola_hop.cuh): results are
@@ -29,32 +31,37 @@ namespace cola {
 namespace {
 
 constexpr int TILE_MAX_THREADS = 256;
+constexpr int TILE_STRIDE = 1024;   // shared-memory entries per 16-byte chunk plane (compile-time: LDS offsets become immediates)
 #ifndef COLA_TILE_MINB
 #define COLA_TILE_MINB 2
 #endif
 
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
 {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");   // visible to the async (TMA) proxy
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
-
-// Stage one box of input sites: TX x ny x nz x nt sites whose (y, z, t) origin is (oy, oz, ot) (already wrapped; a box is
-// one tile extent wide at most in the wrapped direction, so no further wrap occurs inside it ... except when the box is
-// the core, whose origin is the tile origin).  Entry f of the box goes to smem entry `ent0 + f`.
-template <int NCH>
-__device__ __forceinline__ void stage_box(uint4 *sm, const int stride, const uint4 *in, const Geom &g, const TileArgs &ta, const int ent0, const int n,
-                                          const FastDiv &dny, const FastDiv &dnz, const int oy, const int oz, const int ot)
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, unsigned bytes)
 {
-    for (int f = (int)threadIdx.x; f < n; f += (int)blockDim.x) {
-        const unsigned r1 = ta.dTX.div((unsigned)f), xh = (unsigned)f - r1 * ta.dTX.d;
-        const unsigned r2 = dny.div(r1), yy = r1 - r2 * dny.d;
-        const unsigned tt = dnz.div(r2), zz = r2 - tt * dnz.d;
-        const size_t idx = (size_t)xh + (size_t)g.Xh * ((size_t)(oy + (int)yy) + (size_t)g.Y * ((size_t)(oz + (int)zz) + (size_t)g.Z * (size_t)(ot + (int)tt)));
-#pragma unroll
-        for (int k = 0; k < NCH; k++) cp_async16(sm + (size_t)k * stride + ent0 + f, in + (size_t)k * g.Vh + idx);
-    }
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    unsigned done;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done)
+                     : "r"(smem_u32(bar)), "r"(parity), "r"(2000u)   // suspend-time hint in ns: poll rarely
+                     : "memory");
+    } while (!done);
+}
+// TMA bulk copy (1-D, no tensor map): `bytes` (multiple of 16) from global to shared memory, completion counted on `bar`
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes),
+                 "r"(smem_u32(bar))
+                 : "memory");
 }
 
 template <typename T>
@@ -95,7 +102,11 @@ __global__ void __launch_bounds__(TILE_MAX_THREADS, COLA_TILE_MINB) dslash_tile_
     const DslashArgs &a = ta.d;
     const Geom &g = a.g;
     const size_t Vh = g.Vh;
+    __shared__ __align__(8) unsigned long long mbar_storage;
+    unsigned long long *mbar = &mbar_storage;
+    if (threadIdx.x == 0) mbar_init(mbar, 1);
     pdl_trigger();
+    __syncthreads();
 
     // tile origin (tiles ordered y fastest, then z, then t: the same time-slice-by-time-slice sweep as the direct kernels)
     const unsigned b = blockIdx.x;
@@ -130,37 +141,74 @@ __global__ void __launch_bounds__(TILE_MAX_THREADS, COLA_TILE_MINB) dslash_tile_
     pdl_wait();
     if (a.skip && *a.skip) return;
 
-    // ---- stage the tile's input spinors and its six faces
-    {
-        const uint4 *in = reinterpret_cast<const uint4 *>(a.in);
-        const int st = ta.stride;
-        const int TX = ta.TX, TY = ta.TY, TZ = ta.TZ, TT = ta.TT;
+    // ---- stage the tile's input spinors and its six faces with TMA bulk copies of whole x-y row groups.  With TX = Xh the
+    // rows y0-1 .. y0+TY of fixed (z, t) are ONE contiguous run of (TY+2)*TX spinor chunks in the [chunk][site] layout
+    // (three runs if the tile touches the y boundary of the lattice), and so is each z or t face at fixed t or z.
+    // Shared-memory entries (16-byte chunk plane k at k * TILE_STRIDE):
+    //   main(xh, ly, lz, lt) = xh + TX*((ly+1) + (TY+2)*(lz + TZ*lt)),  ly = -1 .. TY (the y faces are rows -1 and TY)
+    //   zface(hi, lt)        = off_z + (hi*TT + lt)*TX*TY + xh + TX*ly
+    //   tface(hi, lz)        = off_t + (hi*TZ + lz)*TX*TY + xh + TX*ly
+    // Lane 0 of every warp issues the copies of the row groups dealt to its warp (72 copies per 256-site tile; a bulk
+    // copy takes uniform registers and costs ~15 instructions of uniform-register traffic, so copies issued from divergent
+    // lanes are serialised by the compiler, and all 72 issued by ONE lane take longer than the tile's arithmetic: 226 us
+    // per launch against 114 us, ncu); the mbarrier is armed with the byte count of the whole tile; warp 0 waits on its
+    // phase, the rest on the block barrier.
+    const int TX = ta.TX, TY = ta.TY, TZ = ta.TZ, TT = ta.TT;
+    const int rowsz = (TY + 2) * TX, face = TX * TY;
+    if ((l & 31u) == 0u) {
         const int ym = y0 == 0 ? g.Y - 1 : y0 - 1, yp = y0 + TY == g.Y ? 0 : y0 + TY;
         const int zm = z0 == 0 ? g.Z - 1 : z0 - 1, zp = z0 + TZ == g.Z ? 0 : z0 + TZ;
         const int tm = t0 == 0 ? g.T - 1 : t0 - 1, tp = t0 + TT == g.T ? 0 : t0 + TT;
-        stage_box<6>(smu, st, in, g, ta, 0, ta.nthr, ta.dTY, ta.dTZ, y0, z0, t0);
-        stage_box<6>(smu, st, in, g, ta, ta.off[0], TX * TZ * TT, ta.d1, ta.dTZ, ym, z0, t0);
-        stage_box<6>(smu, st, in, g, ta, ta.off[1], TX * TZ * TT, ta.d1, ta.dTZ, yp, z0, t0);
-        stage_box<6>(smu, st, in, g, ta, ta.off[2], TX * TY * TT, ta.dTY, ta.d1, y0, zm, t0);
-        stage_box<6>(smu, st, in, g, ta, ta.off[3], TX * TY * TT, ta.dTY, ta.d1, y0, zp, t0);
-        stage_box<6>(smu, st, in, g, ta, ta.off[4], TX * TY * TZ, ta.dTY, ta.dTZ, y0, z0, tm);
-        stage_box<6>(smu, st, in, g, ta, ta.off[5], TX * TY * TZ, ta.dTY, ta.dTZ, y0, z0, tp);
+        const bool y_inside = y0 > 0 && y0 + TY < g.Y;
+        const int nzt = TZ * TT, ngroups = nzt + 2 * TT + 2 * TZ;
+        const uint4 *in = reinterpret_cast<const uint4 *>(a.in);
+        if (l == 0) mbar_arrive_expect_tx(mbar, (unsigned)ta.nent * 96u);
+        for (int gi = (int)(l >> 5); gi < ngroups; gi += (int)(blockDim.x >> 5)) {
+            int zz, tt, ent;
+            bool main_group = false;
+            if (gi < nzt) {
+                const int qt = (int)ta.dTZ.div((unsigned)gi), qz = gi - qt * TZ;
+                zz = z0 + qz; tt = t0 + qt; ent = rowsz * gi;
+                main_group = true;
+            } else if (gi < nzt + 2 * TT) {
+                const int q = gi - nzt, hi = q >= TT, qt = q - hi * TT;
+                zz = hi ? zp : zm; tt = t0 + qt; ent = ta.off_z + q * face;
+            } else {
+                const int q = gi - nzt - 2 * TT, hi = q >= TZ, qz = q - hi * TZ;
+                zz = z0 + qz; tt = hi ? tp : tm; ent = ta.off_t + q * face;
+            }
+            const size_t zt = (size_t)g.Y * ((size_t)zz + (size_t)g.Z * (size_t)tt);   // row index of (y = 0, zz, tt)
+            uint4 *dst = smu + ent;
+            if (!main_group) {
+                const uint4 *src = in + (size_t)g.Xh * (zt + (size_t)y0);
+#pragma unroll
+                for (int k = 0; k < 6; k++) bulk_g2s(dst + k * TILE_STRIDE, src + (size_t)k * Vh, (unsigned)face * 16u, mbar);
+            } else if (y_inside) {
+                const uint4 *src = in + (size_t)g.Xh * (zt + (size_t)(y0 - 1));
+#pragma unroll
+                for (int k = 0; k < 6; k++) bulk_g2s(dst + k * TILE_STRIDE, src + (size_t)k * Vh, (unsigned)rowsz * 16u, mbar);
+            } else {
+                const uint4 *s0 = in + (size_t)g.Xh * (zt + (size_t)ym), *s1 = in + (size_t)g.Xh * (zt + (size_t)y0), *s2 = in + (size_t)g.Xh * (zt + (size_t)yp);
+#pragma unroll
+                for (int k = 0; k < 6; k++) {
+                    bulk_g2s(dst + k * TILE_STRIDE, s0 + (size_t)k * Vh, (unsigned)TX * 16u, mbar);
+                    bulk_g2s(dst + k * TILE_STRIDE + TX, s1 + (size_t)k * Vh, (unsigned)face * 16u, mbar);
+                    bulk_g2s(dst + k * TILE_STRIDE + TX + face, s2 + (size_t)k * Vh, (unsigned)TX * 16u, mbar);
+                }
+            }
+        }
     }
 
     // ---- shared-memory entries of the 8 neighbours and boundary signs (index arithmetic overlaps the copies)
-    const int TX = ta.TX, TY = ta.TY, TZ = ta.TZ, TT = ta.TT;
-    const int ec = (int)lc;
+    const int ec = (int)xh + TX * ((int)ly + 1 + (TY + 2) * ((int)lz + TZ * (int)lt));
     const int exf = odd ? ((int)xh + 1 == TX ? ec - (int)xh : ec + 1) : ec;
     const int exb = odd ? ec : ((int)xh == 0 ? ec + TX - 1 : ec - 1);
-    const int fy = (int)xh + TX * ((int)lz + TZ * (int)lt);      // position on a y face
-    const int fz = (int)xh + TX * ((int)ly + TY * (int)lt);      // ... z face
-    const int ft = (int)xh + TX * ((int)ly + TY * (int)lz);      // ... t face
-    const int eyf = ((int)ly + 1 < TY) ? ec + TX : ta.off[1] + fy;
-    const int eyb = ((int)ly > 0) ? ec - TX : ta.off[0] + fy;
-    const int ezf = ((int)lz + 1 < TZ) ? ec + TX * TY : ta.off[3] + fz;
-    const int ezb = ((int)lz > 0) ? ec - TX * TY : ta.off[2] + fz;
-    const int etf = ((int)lt + 1 < TT) ? ec + TX * TY * TZ : ta.off[5] + ft;
-    const int etb = ((int)lt > 0) ? ec - TX * TY * TZ : ta.off[4] + ft;
+    const int fxy = (int)xh + TX * (int)ly;                      // position on a z or t face
+    const int eyf = ec + TX, eyb = ec - TX;
+    const int ezf = ((int)lz + 1 < TZ) ? ec + rowsz : ta.off_z + (TT + (int)lt) * face + fxy;
+    const int ezb = ((int)lz > 0) ? ec - rowsz : ta.off_z + (int)lt * face + fxy;
+    const int etf = ((int)lt + 1 < TT) ? ec + rowsz * TZ : ta.off_t + (TZ + (int)lz) * face + fxy;
+    const int etb = ((int)lt > 0) ? ec - rowsz * TZ : ta.off_t + (int)lz * face + fxy;
 
     const bool cxf = odd && ((int)xh + 1 == g.Xh), cxb = !odd && ((int)xh == 0);
     const T one = 1;
@@ -170,7 +218,9 @@ __global__ void __launch_bounds__(TILE_MAX_THREADS, COLA_TILE_MINB) dslash_tile_
     const T et_f = (t + 1 == g.T && g.bc[3] < 0) ? -one : one, et_b = (t == 0 && g.bc[3] < 0) ? -one : one;
     const T sf = (T)a.sgn, sb = -(T)a.sgn;   // forward: (1 + sgn*gamma), backward: (1 - sgn*gamma)
 
-    cp_async_wait_all();
+    // one warp polls the mbarrier (a polling loop executes instructions: eight spinning warps cost the other resident
+    // tile 25 % of the issue slots, ncu), the others sleep on the block barrier
+    if (l < 32u) mbar_wait(mbar, 0);
     __syncthreads();
 
     const bool want_norm = a.red.partials != nullptr;
@@ -179,7 +229,7 @@ __global__ void __launch_bounds__(TILE_MAX_THREADS, COLA_TILE_MINB) dslash_tile_
         T acc[24];
 #pragma unroll
         for (int k = 0; k < 24; k++) acc[k] = 0;
-        const int st = ta.stride;
+        constexpr int st = TILE_STRIDE;
         hop_smem<FMT, 0>(smf, st, exf, rawA, gp + 1 * lb, Vh, i, ex_f, sf, acc);
         hop_smem<FMT, 1>(smf, st, exb, rawB, gq + 1 * lb, Vh, gyb, ex_b, sb, acc);
         hop_smem<FMT, 2>(smf, st, eyf, rawA, gp + 2 * lb, Vh, i, ey_f, sf, acc);
@@ -212,7 +262,7 @@ cudaError_t launch_tile_fmt(const TileArgs &ta, cudaStream_t s)
     const int xpay = a.y ? (a.clov_y ? 2 : 1) : 0;
     const int post = a.clov_post ? 1 : 0;
     const dim3 grid((unsigned)ta.ntiles), block((unsigned)((ta.nthr + 31) / 32 * 32));
-    const size_t smem = (size_t)ta.stride * 6 * 16;
+    const size_t smem = (size_t)TILE_STRIDE * 6 * 16;
     if (xpay == 0 && post == 0) return launch_one<FMT, 0, 0>(ta, grid, block, smem, s);
     if (xpay == 0 && post == 1) return launch_one<FMT, 0, 1>(ta, grid, block, smem, s);
     if (xpay == 1 && post == 0) return launch_one<FMT, 1, 0>(ta, grid, block, smem, s);
@@ -240,7 +290,7 @@ TileShape choose_tile(const Geom &g)
                 const int n = g.Xh * ty * tz * tt;
                 if (n > TILE_MAX_THREADS) break;
                 const int ent = n + 2 * g.Xh * (tz * tt + ty * tt + ty * tz);
-                if ((size_t)ent * 96 > 100 * 1024) continue;   // two tiles per SM
+                if (ent > TILE_STRIDE) continue;   // 96 KB of shared memory per tile: two tiles per SM
                 // staged spinors per output site; idle lanes of the last warp count as sites that cost but do not produce
                 const int lanes = (n + 31) / 32 * 32;
                 const double cost = (double)ent / n * ((double)lanes / n);
@@ -268,15 +318,10 @@ cudaError_t launch_dslash_tile(int fmt, const DslashArgs &a, cudaStream_t s)
     ta.TX = g.Xh; ta.TY = sh.TY; ta.TZ = sh.TZ; ta.TT = sh.TT;
     ta.nthr = sh.nthr;
     ta.nent = sh.nent;
-    ta.stride = sh.nent;
+    ta.stride = TILE_STRIDE;
     ta.ntiles = (g.Y / sh.TY) * (g.Z / sh.TZ) * (g.T / sh.TT);
-    const int fy = g.Xh * sh.TZ * sh.TT, fz = g.Xh * sh.TY * sh.TT, ft = g.Xh * sh.TY * sh.TZ;
-    ta.off[0] = sh.nthr;
-    ta.off[1] = ta.off[0] + fy;
-    ta.off[2] = ta.off[1] + fy;
-    ta.off[3] = ta.off[2] + fz;
-    ta.off[4] = ta.off[3] + fz;
-    ta.off[5] = ta.off[4] + ft;
+    ta.off_z = sh.TZ * sh.TT * (sh.TY + 2) * g.Xh;
+    ta.off_t = ta.off_z + 2 * sh.TT * g.Xh * sh.TY;
     ta.dTX = make_fastdiv((unsigned)g.Xh);
     ta.dTY = make_fastdiv((unsigned)sh.TY);
     ta.dTZ = make_fastdiv((unsigned)sh.TZ);

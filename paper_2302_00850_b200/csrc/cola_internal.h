@@ -63,6 +63,18 @@ struct Ctl {
     unsigned counter[8];  // "last block" tickets, one per concurrently used reduction
 };
 
+// Device-resident scalars of BiCGStab, complex as (re, im).  rho = <rhat, r_{i-1}> of the running
+// pass, rho_next = <rhat, r_i> (formed by the x/r update or, after a reliable update, by a dot kernel), beta for the
+// next search direction.  The decision state mirrors Ctl's.
+struct CtlB {
+    double rho[2], rho_next[2], rv[2], ts[2], beta[2];
+    double tt;          // |t|^2 (fused into the operator kernel)
+    double rr;          // |r|^2
+    double rmax2, target2, delta2;
+    int flag, iters;
+    unsigned counter[4];
+};
+
 constexpr int MRHS_MAX = 16;   // right-hand sides per batched launch / solve
 
 // Device-resident scalars of the batched (multi-right-hand-side) CGLS: one entry per vector.  Lives in the control
@@ -93,10 +105,12 @@ constexpr unsigned REDUCE_GROUP = 256;
 __host__ __device__ inline size_t reduce_groups(size_t nblocks) { return (nblocks + REDUCE_GROUP - 1) / REDUCE_GROUP; }
 
 // Buffers of one deterministic grid-wide reduction (see grid_sum_last in cola_device.cuh)
+constexpr int REDUCE_MAXC = 4;   // values a single launch may reduce at once (BiCGStab: |r|^2 and a complex dot)
 struct ReduceWs {
-    double *partials;     // [max blocks]
-    double *gpart;        // [max groups]
+    double *partials;     // [REDUCE_MAXC][pstride]: per-block partials of component c at partials + c*pstride
+    double *gpart;        // [REDUCE_MAXC][gstride]
     unsigned *gticket;    // [max groups], zero before first use, self-resetting
+    unsigned pstride, gstride;
 };
 
 // What r_update's last block publishes for the host: written straight into mapped pinned host memory
@@ -162,7 +176,7 @@ struct TileArgs {
     int TX, TY, TZ, TT;
     int nthr, nent, ntiles;
     int stride;            // shared-memory entries per 16-byte chunk plane
-    int off[6];            // first entry of the y-, y+, z-, z+, t-, t+ face
+    int off_z, off_t;      // first entry of the z faces (z-, z+) and of the t faces (t-, t+); y faces are rows of the main block
     FastDiv dTX, dTY, dTZ, d1;
     FastDiv nby, nbz;      // tiles along y and z
 };
@@ -243,6 +257,28 @@ cudaError_t launch_axpby64(void *out64, double a, const void *A64, double b, con
                            const ReduceWs *red, unsigned *counter, double *norm_out, cudaStream_t s);
 // x64 += x32; x32 = 0
 cudaError_t launch_accumulate(void *x64, void *x32, size_t n_sites, cudaStream_t s);
+
+// ---- BiCGStab BLAS-1 (cola_blas.cu).  Vectors are n_sites half- or full-lattice spinors of precision prec.
+// which = 0: ctl->rv = <a, b>, and ctl->rho = ctl->rho_next (a new pass starts);  1: ctl->ts = <a, b>;
+// 2: ctl->rho_next = <a, b> and beta = (rho_next / rho)(alpha / omega) (after a reliable update replaced r)
+cudaError_t launch_bicg_dot(cola_prec prec, const void *a, const void *b, CtlB *ctl, int which, const int *skip, size_t n_sites, const ReduceWs &red, cudaStream_t s);
+// s = r - alpha v, alpha = rho / rv
+cudaError_t launch_bicg_s_update(cola_prec prec, void *sv, const void *r, const void *v, const CtlB *ctl, const int *skip, size_t n_sites, cudaStream_t s);
+// x += alpha p + omega s;  r = s - omega t, omega = ts / tt;  ctl->rr = |r|^2, rho_next = <rhat, r>, beta; decision + status
+cudaError_t launch_bicg_xr_update(cola_prec prec, void *x, void *r, const void *p, const void *sv, const void *t, const void *rhat, CtlB *ctl, int iter,
+                                  const int *skip, HostStatus *mirror, size_t n_sites, const ReduceWs &red, cudaStream_t s);
+// p = r + beta (p - omega v)
+cudaError_t launch_bicg_p_update(cola_prec prec, void *p, const void *r, const void *v, const CtlB *ctl, const int *skip, size_t n_sites, cudaStream_t s);
+
+// ---- low-mode solver (cola_eig.cu): fp64 half-lattice vectors of n_sites sites
+cudaError_t launch_eig_cdot(const void *a, const void *b, size_t n_sites, const ReduceWs &red, unsigned *counter, double *out2, cudaStream_t s);   // out2 = <a, b>
+cudaError_t launch_eig_caxpy(void *w, const void *v, size_t n_sites, const double *coef2, double scale, cudaStream_t s);                     // w += scale * coef2 * v
+cudaError_t launch_eig_normalise(void *out, const void *in, size_t n_sites, const double *norm2, cudaStream_t s);                           // out = in / sqrt(norm2[0])
+cudaError_t launch_eig_lincomb(void *out, double a, const void *x, double b, const void *y, double c, const void *z, size_t n_sites, cudaStream_t s);
+// out[q] = sum_j V[j] Y[j][q] (j < m, q < kq; vectors vec_bytes apart; Y row-major m x kq on the device; out must not overlap V)
+cudaError_t launch_eig_rotate(void *out, const void *V, size_t vec_bytes, int m, int kq, const double *Y_dev, size_t n_sites, cudaStream_t s);
+cudaError_t launch_eig_start(void *v, size_t n_sites, unsigned long long seed, cudaStream_t s);
+void jacobi_eigh(int m, double *A, double *w, double *Q);   // host: real symmetric A (destroyed) -> ascending w, eigenvectors in the columns of Q
 
 // ---- batched BLAS-1 over the vectors list.v[0..nrhs) (cola_blas.cu); vector n of an array starts n*stride bytes in.
 int blas_mrhs_blocks(size_t n_sites, cola_prec prec);   // blocks per vector of a batched BLAS launch = partials per vector

@@ -1,0 +1,70 @@
+"""BiCGStab on the Schur complement (cola_solve_params.method = COLA_BICGSTAB) against the
+oracle's BiCGStab (oracle/cola_oracle.c, pinned on the CPU against the dense inverse, CGNR's solution and scipy's
+implementation): solution, fp64 true residual recomputed with the ORACLE's M, pass counts, and the residual history
+pass by pass in fp64 mode."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2302_00850_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+BC = (1, 1, 1, -1)
+
+
+def rel(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+@pytest.mark.parametrize("dims,kind", [((2, 2, 2, 2), "haar"), ((4, 4, 4, 4), "haar"), ((12, 10, 6, 4), "smooth"), ((8, 8, 8, 16), "smooth")])
+def test_bicgstab_matches_the_oracle(dims, kind):
+    from paper_2302_00850_b200 import binding
+
+    kappa, csw = (0.12, 1.0) if kind == "haar" else (0.1245, 1.0)
+    U = inputs.links_haar(dims, 5) if kind == "haar" else inputs.links_smooth(dims, 0.3, 5)
+    Un = U.numpy()
+    A = oracle.clover(dims, Un, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    b = inputs.source_gaussian(dims, 21)
+    bn = b.numpy()
+    ref = oracle.bicgstab(dims, BC, Un, A, Ainv, kappa, bn, even_odd=True, tol=1e-10)
+    assert ref["converged"]
+    cg = oracle.cgnr(dims, BC, Un, A, Ainv, kappa, bn, even_odd=True, tol=1e-10)
+    c = binding.Cola(dims, kappa, csw, bc=BC)
+    c.gauge_upload(U)
+    for mixed in (0, 1, 2):
+        x, info = c.cg_solve_history(b.cuda(), tol=1e-10, even_odd=True, mixed=mixed, method="bicgstab")
+        assert info["converged"] and info["true_residual"] <= 1.05e-10, (mixed, info)
+        xn = x.cpu().numpy()
+        res = np.linalg.norm((bn - oracle.M(dims, BC, Un, A, kappa, xn)).ravel()) / np.linalg.norm(bn.ravel())
+        assert res <= 1.05e-10 and abs(res - info["true_residual"]) <= 1e-3 * res + 1e-14
+        assert rel(xn, ref["x"]) < 5e-9 and rel(xn, cg["x"]) < 5e-9
+        h, h_ref = np.asarray(info["history"]), np.asarray(ref["history"])
+        if mixed == 0:
+            # fp64: the same recurrence; rounding differences are amplified along the non-monotone BiCGStab history, so
+            # the first passes agree to rounding, and the count within max(1, 2 %)
+            assert abs(info["iters"] - ref["iters"]) <= max(1, math.ceil(0.02 * ref["iters"])), (info["iters"], ref["iters"])
+            n = min(6, len(h), len(h_ref))
+            assert np.max(np.abs(h[:n] - h_ref[:n]) / h_ref[:n]) < 1e-9
+        else:
+            # fp32 / 16-bit inner passes: BiCGStab's count is sensitive to rounding; hold it to the oracle's within 15 %
+            # (+2), and well below CGNR's
+            assert abs(info["iters"] - ref["iters"]) <= max(2, math.ceil(0.15 * ref["iters"])), (mixed, info["iters"], ref["iters"])
+            assert info["reliable_updates"] >= 1
+        if min(dims) > 2:
+            assert info["iters"] < cg["iters"]
+    # host buffers, and the same answer
+    xh, ih = c.cg_solve(b.pin_memory(), tol=1e-10, even_odd=True, mixed=1, method="bicgstab")
+    x1, i1 = c.cg_solve(b.cuda(), tol=1e-10, even_odd=True, mixed=1, method="bicgstab")
+    assert ih["iters"] == i1["iters"] and rel(xh.numpy(), x1.cpu().numpy()) < 1e-12
+    # not offered on the unpreconditioned system, nor batched
+    with pytest.raises(binding.ColaError) as e:
+        c.cg_solve(b.cuda(), even_odd=False, method="bicgstab")
+    assert e.value.status == binding.COLA_EINVAL
+    xx, info = c.cg_solve(b.cuda(), max_iter=2, method="bicgstab", mixed=1)
+    assert not info["converged"] and info["iters"] == 2 and 0 < info["true_residual"] < 1
+    c.close()

@@ -474,3 +474,33 @@ def test_bicgstab_iterates_match_scipy():
         assert rel(xe, xk) < 1e-9, (k, rel(xe, xk))
         # and the recorded residual is the residual of that iterate
         assert abs(ours["history"][k] - np.linalg.norm(bhat - S(xk)) / bnorm) <= 1e-9 * ours["history"][0]
+
+
+# ---------------------------------------------------------------------------------------------
+# Low modes of S^+ S: pinned by the brute-force dense matrix
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 2, 2, 4)])
+def test_lowest_modes_against_brute_force_dense_schur(dims):
+    """oracle.lowest_modes against the Schur complement of the independent numpy brute-force matrix (tests/bruteforce.py:
+    hand-typed gammas, np.roll clover), both through its dense path and through its ARPACK path."""
+    kappa, csw = 0.124, 1.0
+    U = np_links("smooth", dims, seed=95)
+    A = oracle.clover(dims, U, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    Md = bf.dense_M(dims, BC, U, kappa, csw)
+    par = np.repeat(oracle.parity_mask(dims).ravel(), 12)
+    e, o = np.flatnonzero(par == 0), np.flatnonzero(par == 1)
+    Sd = Md[np.ix_(e, e)] - Md[np.ix_(e, o)] @ np.linalg.solve(Md[np.ix_(o, o)], Md[np.ix_(o, e)])
+    want = np.linalg.eigvalsh(Sd.conj().T @ Sd)
+    k = 6
+    w, v = oracle.lowest_modes(dims, BC, U, A, Ainv, kappa, k)
+    assert np.allclose(w, want[:k], rtol=1e-10, atol=0)
+    assert w[0] > 0 and np.all(np.diff(w) >= 0)
+    # eigenvector property with the oracle's own operator, orthonormality, support on the even sites only
+    for i in range(k):
+        Hv = oracle.schur(dims, BC, U, A, Ainv, kappa, oracle.schur(dims, BC, U, A, Ainv, kappa, v[i]), dagger=True)
+        assert np.linalg.norm((Hv - w[i] * v[i]).ravel()) < 1e-10
+        assert abs(np.linalg.norm(v[i].ravel()) - 1) < 1e-12
+        assert np.abs(v[i][oracle.parity_mask(dims) == 1]).max() == 0
+    w2, v2 = oracle.lowest_modes(dims, BC, U, A, Ainv, kappa, k, dense_limit=0)
+    assert np.allclose(w2, want[:k], rtol=1e-9, atol=0)
