@@ -49,9 +49,34 @@ BYTES = {
     "dslash_clover_xpay": {"f32x12": 960, "f32x18": 1152, "f64x18": 2304, "f32h16": 624},  # + 72 clover + 24 (x)
 }
 FLOPS = {"dslash": 1320, "dslash_clover_inv": 1824, "dslash_clover_xpay": 1872}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of dslash_kernel<F32x12, XPAY=2> from the committed
-# ncu --set full capture (a number read from a profile, never a timing taken under the profiler)
-NCU_TRAFFIC = {(32, 32, 32, 64): {"bytes_per_launch": 979430000, "source": "profiles/r1d_operators_full.txt (909.2 MB read + 70.24 MB write)"}}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of dslash_kernel<F32x12, XPAY=2> is read from
+# profiles/ncu_traffic.json, which records the commit and the hash of csrc/ it was captured at: when the kernels have
+# changed since, `traffic` is reported as null rather than a stale number.
+def csrc_hash():
+    import hashlib
+
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2302_00850_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".h")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(dims):
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(path):
+        return None, "profiles/ncu_traffic.json absent"
+    rec = json.load(open(path))
+    ent = rec.get("entries", {}).get("x".join(str(d) for d in dims))
+    if ent is None:
+        return None, "no ncu capture for this lattice"
+    if rec.get("csrc_sha16") != csrc_hash():
+        return None, f"csrc/ changed since the capture at {rec.get('commit')}: stale, not reported"
+    return int(ent["bytes_per_launch"]), f"{ent['source']} (commit {rec.get('commit')})"
+
+
 CPU_SAMPLE_MAX_SITES = 1 << 22   # largest lattice the oracle's full fields are built for inside bench.py
 NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star's denominator, reported beside the measured one
 
@@ -177,8 +202,23 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
     return out
 
 
-def cpu_baseline_sample(cfg, U_cpu, n_pairs=10):
-    """The oracle as it stands on the host cores: n_pairs x (S, S^dagger) applications on the same lattice."""
+def _set_oracle_threads(n):
+    """OpenMP thread count of the oracle's site loops (the oracle itself is untouched: same library, same code)."""
+    import ctypes
+
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
+
+
+def cpu_baseline_sample(cfg, U_cpu, n_pairs=6, table=True):
+    """The oracle as it stands on the host cores.  `value`: n_pairs x (S, S^dagger) applications on the configuration's
+    lattice with all cores.  `table`: M and S, 16^3x32 and 32^3x64 extents of the same recipe, 1 core and all
+    cores, one application each; the stored times of the oracle's full CGNR solves (tests/golden/solver_golden.json, with
+    their thread count) and, labelled as such, the CPU time-to-solution extrapolated to configs 3 and 4 as (seconds per
+    S, S^dagger pair per site) x (sites) x (GPU iteration count)."""
     import numpy as np
 
     import oracle
@@ -189,6 +229,7 @@ def cpu_baseline_sample(cfg, U_cpu, n_pairs=10):
     Ainv = oracle.clover_inverse(A)
     x = (inputs.source_gaussian(dims, 77) * torch.from_numpy(oracle.parity_mask(dims) == 0)[..., None, None]).numpy()
     Vh = inputs.volume(dims) // 2
+    cores = oracle.num_threads()
     t0 = time.time()
     for _ in range(n_pairs):
         y = oracle.schur(dims, inputs.BC, Un, A, Ainv, kappa, x)
@@ -196,9 +237,48 @@ def cpu_baseline_sample(cfg, U_cpu, n_pairs=10):
         x = x / np.linalg.norm(x.ravel())
     dt = time.time() - t0
     flops = n_pairs * 2 * 3696.0 * Vh
-    return {"value": round(flops / dt / 1e9, 3), "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"{n_pairs} x (S, S^dagger) oracle applications on the full {dims} lattice = the operator work of {n_pairs} CGLS iterations, {dt:.1f} s",
-            "seconds": round(dt, 2)}
+    out = {"value": round(flops / dt / 1e9, 3), "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
+           "sample": f"{n_pairs} x (S, S^dagger) oracle applications on the full {dims} lattice = the operator work of {n_pairs} CGLS iterations, {dt:.1f} s",
+           "seconds": round(dt, 2)}
+    if not table:
+        return out
+    rows = []
+    pair_s_per_site = dt / n_pairs / Vh          # all cores, seconds per (S, S^dagger) pair and even site
+    fields = {tuple(dims): (Un, A, Ainv)}
+    for d in ((16, 16, 16, 32), (32, 32, 32, 64)):
+        if inputs.volume(d) > inputs.volume(dims):
+            continue
+        if d not in fields:
+            Ud = inputs.links_smooth(d, cfg["eps"], 20230200 + 99).numpy()
+            Ad = oracle.clover(d, Ud, kappa, csw)
+            fields[d] = (Ud, Ad, oracle.clover_inverse(Ad))
+        Ud, Ad, Aid = fields[d]
+        psi = inputs.source_gaussian(d, 78).numpy()
+        psi_e = psi * (oracle.parity_mask(d) == 0)[..., None, None]
+        V = inputs.volume(d)
+        for nthr in (1, cores):
+            if not _set_oracle_threads(nthr):
+                continue
+            for name, fl, fn in (("M", 1872.0 * V, lambda: oracle.M(d, inputs.BC, Ud, Ad, kappa, psi)),
+                                 ("S", 3696.0 * V / 2, lambda: oracle.schur(d, inputs.BC, Ud, Ad, Aid, kappa, psi_e))):
+                t1 = time.time()
+                fn()
+                el = time.time() - t1
+                rows.append({"operator": name, "lattice": list(d), "cores": nthr, "seconds": round(el, 4), "GFLOP/s": round(fl / el / 1e9, 3)})
+        _set_oracle_threads(cores)
+    out["table"] = rows
+    gold = os.path.join(ROOT, "tests", "golden", "solver_golden.json")
+    if os.path.exists(gold):
+        g = json.load(open(gold))
+        out["oracle_cgnr_solves"] = [{"config": int(k), "lattice": v["dims"], "mode": m, "iters": v[m]["iters"], "seconds": round(v[m]["seconds"], 2),
+                                      "threads": v.get("threads"), "source": "tests/golden/solver_golden.json (written by tests/golden/make_golden.py on the build box)"}
+                                     for k, v in sorted(g.items()) for m in ("full", "eo") if m in v]
+    # extrapolation, labelled: CPU seconds per iteration scale with the volume; iteration counts are the GPU's
+    out["extrapolated_cpu_time_to_solution_s"] = {
+        "note": "EXTRAPOLATED, not measured: (all-core seconds per (S, S^dagger) pair per even site, measured above) x even sites x the CUDA solver's iteration count",
+        "config3_48^3x96_per_source_97_iters": round(pair_s_per_site * (48 ** 3 * 96 // 2) * 97, 1),
+        "config4_64^3x128_136_iters": round(pair_s_per_site * (64 ** 3 * 128 // 2) * 136, 1)}
+    return out
 
 
 def reference_arm(args, cfg, workload):
@@ -516,9 +596,7 @@ def main():
                 "bound": "hbm", "achieved": k["GB/s"], "peak": peak, "unit": "GB/s", "frac": round(k["GB/s"] / peak, 4),
                 "frac_of_nominal_8TBs": round(k["GB/s"] / NOMINAL_HBM_GBS, 4), "peak_source": peak_src + " (burst figure; kernel timed alone)",
                 "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": round(k["ms"] / 2, 5), "traffic": None}
-        if tuple(dims) in NCU_TRAFFIC:
-            roof["traffic"] = NCU_TRAFFIC[tuple(dims)]["bytes_per_launch"]
-            roof["traffic_source"] = NCU_TRAFFIC[tuple(dims)]["source"]
+        roof["traffic"], roof["traffic_source"] = ncu_traffic(dims)
     if in_solve and in_solve["launches"]:
         # the same kernel inside a solve step (event pair around each launch, speculative no-op launches excluded)
         per_launch_bytes = BYTES["dslash_clover_xpay"]["f32x12"] * ctx.Vh
@@ -530,7 +608,7 @@ def main():
                     "bound": "hbm", "achieved": in_solve["achieved"], "peak": peak, "unit": "GB/s", "frac": in_solve["frac"],
                     "frac_of_nominal_8TBs": in_solve["frac_of_nominal_8TBs"], "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": in_solve["avg_launch_ms"],
-                    "traffic": NCU_TRAFFIC.get(tuple(dims), {}).get("bytes_per_launch")}
+                    "traffic": ncu_traffic(dims)[0]}
         roof["in_solve"] = in_solve
     cpu = None
     if U_cpu is not None:
