@@ -44,10 +44,13 @@ from paper_2302_00850_b200 import inputs  # noqa: E402
 # algorithmic bytes per output site, fp32 with 12-real links; fp64 x18 in the second column
 BYTES = {
     # f32h16 = COLA_F32_H16: fp32 spinors, links as 12 x int16, clover as 72 x fp16
-    "dslash": {"f32x12": 576, "f32x18": 768, "f64x18": 1536, "f32h16": 384},          # 8 links + 1 spinor in + 1 out
-    "dslash_clover_inv": {"f32x12": 864, "f32x18": 1056, "f64x18": 2112, "f32h16": 528},   # + 72 reals clover
-    "dslash_clover_xpay": {"f32x12": 960, "f32x18": 1152, "f64x18": 2304, "f32h16": 624},  # + 72 clover + 24 (x)
+    # The fp32 kernels read A in its 48-real field-strength form (192 B), A^-1 as 72 reals (288 B).
+    # f32x12_a72 = the same kernels reading the 72-real packed A (cola_set_compact(1)); f32r8 = COLA_F32_R8: links as 8 fp32 reals
+    "dslash": {"f32x12": 576, "f32x18": 768, "f64x18": 1536, "f32h16": 384, "f32r8": 448, "f32x12_a72": 576},   # 8 links + 1 spinor in + 1 out
+    "dslash_clover_inv": {"f32x12": 864, "f32x18": 1056, "f64x18": 2112, "f32h16": 528, "f32r8": 736, "f32x12_a72": 864},   # + 72 reals clover (A^-1)
+    "dslash_clover_xpay": {"f32x12": 864, "f32x18": 1056, "f64x18": 2304, "f32h16": 624, "f32r8": 736, "f32x12_a72": 960},  # + A (48 or 72 reals) + 24 (x)
 }
+R8_MASK = {"f32r8": 3, "f32x12_a72": 1}
 FLOPS = {"dslash": 1320, "dslash_clover_inv": 1824, "dslash_clover_xpay": 1872}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of dslash_kernel<F32x12, XPAY=2> is read from
 # profiles/ncu_traffic.json, which records the commit and the hash of csrc/ it was captured at: when the kernels have
@@ -161,15 +164,20 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
     peak, _ = measured_peaks()
     out = {}
     Vh = ctx.Vh
-    for prec, fmt in ((torch.float32, fmt32), (torch.float64, "f64x18"), (torch.float32, "f32h16")):
+    fmts = [(torch.float32, fmt32), (torch.float64, "f64x18"), (torch.float32, "f32h16")]
+    if fmt32 == "f32x12":   # the compact fields are measured against the 12-real links they replace
+        fmts += [(torch.float32, "f32r8"), (torch.float32, "f32x12_a72")]
+    for prec, fmt in fmts:
         full = ctx.empty_internal(prec, full=True).normal_()
         dst = ctx.empty_internal(prec, full=True)
         h = fmt == "f32h16"
+        of = "h16" if h else ("r8" if fmt == "f32r8" else None)
+        ctx.set_compact(R8_MASK.get(fmt, 3))
         rows = {
-            "dslash_even": ("dslash", 1, lambda: ctx.dslash_apply(0, full[1], out=dst[0], h16=h)),
-            "dslash_odd": ("dslash", 1, lambda: ctx.dslash_apply(1, full[0], out=dst[1], h16=h)),
-            "fermion_matrix": ("dslash_clover_xpay", 2, lambda: ctx.fermion_matrix_apply(full, out=dst, h16=h)),
-            "schur": (None, 2, lambda: ctx.schur_apply(full[0], out=dst[0], h16=h)),
+            "dslash_even": ("dslash", 1, lambda: ctx.dslash_apply(0, full[1], out=dst[0], fmt=of)),
+            "dslash_odd": ("dslash", 1, lambda: ctx.dslash_apply(1, full[0], out=dst[1], fmt=of)),
+            "fermion_matrix": ("dslash_clover_xpay", 2, lambda: ctx.fermion_matrix_apply(full, out=dst, fmt=of)),
+            "schur": (None, 2, lambda: ctx.schur_apply(full[0], out=dst[0], fmt=of)),
         }
         for name, (kind, launches, fn) in rows.items():
             ms = time_launches(fn, n_warm, n_timed)
@@ -183,7 +191,7 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
             out[f"{name}_{fmt}"] = {"ms": round(ms, 5), "launches": launches, "GB/s": round(gbs, 1), "GFLOP/s": round(flops / (ms * 1e-3) / 1e9, 1),
                                     "frac_measured": round(gbs / peak, 4), "frac_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4)}
         del full, dst
-        if nrhs > 1 and not h:
+        if nrhs > 1 and of is None:
             ctx.set_mrhs_workspace(nrhs)
             vin = ctx.empty_internal_mrhs(nrhs, prec, full=False).normal_()
             vout = torch.empty_like(vin)
@@ -199,6 +207,32 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
             del vin, vout
             ctx.release_mrhs_workspace()
             torch.cuda.empty_cache()
+    ctx.set_compact(3)
+    return out
+
+
+def ab_formats(ctx, rounds=12, burst=40):
+    """Interleaved A/B of the fp32 operator formats: short bursts of each format in turn, many rounds,
+    medians -- the SM clock drifts by ~10 % under the power cap over a run, which a format-after-format table folds into the
+    comparison.  Formats: x12 = 12-real links + 48-real A (the default); a72 = 12-real links + 72-real packed A;
+    r8 = 8-real links + 48-real A; r8_a72 = 8-real links + 72-real A; h16 = 16-bit links + fp16 clover."""
+    full = ctx.empty_internal(torch.float32, full=True).normal_()
+    dst = ctx.empty_internal(torch.float32, full=True)
+    fmts = {"x12": (None, 3), "a72": (None, 1), "r8": ("r8", 3), "r8_a72": ("r8", 1), "h16": ("h16", 3)}
+    ops = {"dslash": lambda f: ctx.dslash_apply(0, full[1], out=dst[0], fmt=f),
+           "fermion_matrix": lambda f: ctx.fermion_matrix_apply(full, out=dst, fmt=f),
+           "schur": lambda f: ctx.schur_apply(full[0], out=dst[0], fmt=f)}
+    res = {(o, k): [] for o in ops for k in fmts}
+    for _ in range(rounds):
+        for o, fn in ops.items():
+            for k, (f, mask) in fmts.items():
+                ctx.set_compact(mask)
+                res[(o, k)].append(time_launches(lambda: fn(f), 5, burst))
+    ctx.set_compact(3)
+    out = {}
+    for o in ops:
+        base = statistics.median(res[(o, "x12")][2:])
+        out[o] = {k: {"ms": round(statistics.median(res[(o, k)][2:]), 5), "vs_x12": round(statistics.median(res[(o, k)][2:]) / base, 3)} for k in fmts}
     return out
 
 
@@ -346,6 +380,7 @@ def main():
     ap.add_argument("--nrhs", type=int, default=0, help="with --operators-only: also time the multi-rhs Schur operator over this many vectors")
     ap.add_argument("--staging", type=int, default=0, choices=[0, 1],
                     help="kernel family of the fp32 / 16-bit single-rhs operators: 0 direct global loads (default), 1 neighbour spinors staged in shared memory")
+    ap.add_argument("--ab-formats", action="store_true", help="measurement aid: interleaved A/B of the fp32 link / clover storage formats, then exit")
     ap.add_argument("--op-warm", type=int, default=20)
     ap.add_argument("--op-timed", type=int, default=200)
     args = ap.parse_args()
@@ -416,6 +451,9 @@ def main():
             torch.distributed.barrier()
         torch.cuda.synchronize()
 
+    if args.ab_formats:       # not a bench line: interleaved comparison of the link / clover storage formats
+        print(json.dumps({"ab_formats": True, "lattice": list(dims), "operators": ab_formats(ctx)}))
+        return
     if args.operators_only:   # not a bench line: a short launch sequence for ncu captures of each operator kernel
         print(json.dumps({"operators_only": True, "lattice": list(dims),
                           "operators": operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed, nrhs=args.nrhs)}))
@@ -489,40 +527,45 @@ def main():
     ms_e, flops_e_all = aggregate_over_ranks(e0.elapsed_time(e1), flops_e, device=dev)
     nbytes = b_host.numel() * b_host.element_size() * n_src
 
-    # ---- the same step with the inner operator reading 16-bit links and clover (mixed = 2)
-    solve_h16 = None
-    if rank == 0 and not args.no_h16:
-        def h16_step():
+    # ---- the same step with the inner operator reading 16-bit links and clover (mixed = 2) or the
+    # 8-real links and the 48-real A (mixed = 3)
+    def extra_solve(mode):
+        def one_step():
             fl, infs = 0.0, []
             for n in range(n_src):
                 bn = b if n_src == 1 else source(n)
-                xn, inf = ctx.cg_solve(bn, tol=1e-10, even_odd=True, mixed=2)
+                xn, inf = ctx.cg_solve(bn, tol=1e-10, even_odd=True, mixed=mode)
                 fl += inf["op_flops"]
                 infs.append(inf)
                 del xn
             return fl, infs
 
         for _ in range(min(args.warmup, 2)):
-            h16_step()
+            one_step()
         torch.cuda.synchronize()
         e0.record()
         fl_h = 0.0
         for _ in range(args.steps):
-            f1, infs_h = h16_step()
+            f1, infs_h = one_step()
             fl_h += f1
         e1.record()
         torch.cuda.synchronize()
         ms_h = e0.elapsed_time(e1) / args.steps
-        solve_h16 = {"ms_per_step": round(ms_h, 3), "GFLOP/s": round(fl_h / args.steps / (ms_h * 1e-3) / 1e9, 1),
-                     "speedup_vs_fp32_inner": round(ms_local / args.steps / ms_h, 3), "iters": [i["iters"] for i in infs_h],
-                     "reliable_updates": [i["reliable_updates"] for i in infs_h],
-                     "max_true_residual": max(i["true_residual"] for i in infs_h), "converged": all(i["converged"] for i in infs_h)}
+        return {"ms_per_step": round(ms_h, 3), "GFLOP/s": round(fl_h / args.steps / (ms_h * 1e-3) / 1e9, 1),
+                "speedup_vs_fp32_inner": round(ms_local / args.steps / ms_h, 3), "iters": [i["iters"] for i in infs_h],
+                "reliable_updates": [i["reliable_updates"] for i in infs_h],
+                "max_true_residual": max(i["true_residual"] for i in infs_h), "converged": all(i["converged"] for i in infs_h)}
+
+    solve_h16 = solve_r8 = None
+    if rank == 0 and not args.no_h16:
+        solve_h16 = extra_solve(2)
+        solve_r8 = extra_solve(3)
 
     # ---- the same step by BiCGStab on the Schur system (two S per pass instead of S and S^+)
     solve_bicgstab = None
     if rank == 0 and not args.no_bicgstab:
         solve_bicgstab = {}
-        for key, mode in (("fp32_inner", 1), ("h16_inner", 2)):
+        for key, mode in (("fp32_inner", 1), ("h16_inner", 2), ("r8_inner", 3)):
             def bi_step():
                 fl, infs = 0.0, []
                 for n in range(n_src):
@@ -559,7 +602,7 @@ def main():
             xs = torch.empty_like(bs)
             ctx.set_mrhs_workspace(n_src)
             batched = {"nrhs": n_src}
-            for key, mode in (("fp32_inner", 1), ("h16_inner", 2)):
+            for key, mode in (("fp32_inner", 1), ("h16_inner", 2), ("r8_inner", 3)):
                 for _ in range(min(args.warmup, 1)):
                     ctx.cg_solve_mrhs(bs, tol=1e-10, x=xs, mixed=mode)
                 torch.cuda.synchronize()
@@ -633,6 +676,7 @@ def main():
         line["solve"]["max_true_residual"] = max(i["true_residual"] for i in infos)
         line["batched"] = batched
     line["solve_h16"] = solve_h16
+    line["solve_r8"] = solve_r8
     line["solve_bicgstab"] = solve_bicgstab
     print(json.dumps(line))
     if world > 1:

@@ -61,7 +61,17 @@ typedef enum {
  * approximate ("sloppy") operator, |K16 x - K x| / |K x| ~ 1e-4, meant for the inner iteration of the mixed-precision
  * solver (cola_solve_params.mixed = 2), whose reliable updates use the exact fp64 operator.  Spinor buffers and
  * cola_spinor_* calls take COLA_F32 for it. */
-typedef enum { COLA_F64 = 0, COLA_F32 = 1, COLA_F32_H16 = 2 } cola_prec;
+/* COLA_F32_R8 (the rest of SURVEY 8(f) NEXT-2): fp32 spinors and arithmetic, links read as 8 fp32 reals (a
+ * parametrisation of SU(3): two entries of row 1, one of column 1 and two phases; the other entries follow from unitarity
+ * and det U = 1 in registers): 1472 bytes per Schur application and site instead of 1728.  Like COLA_F32 (when
+ * trace_sub = 1) it reads A in its 48-real field-strength form: per chiral block the three traceless Hermitian 3x3 matrices
+ * of  1 + [[G3, G1 - i G2], [G1 + i G2, -G3]], expanded to the packed 6x6 block in the kernel (192 instead of 288 bytes).  The same linear map as COLA_F32 up to rounding (sin/cos, 1/x and sqrt are the
+ * hardware approximations: a link entry is good to ~4e-7 absolute); the parity tests hold
+ * it to the fp32 tolerance 2e-6.  Needs COLA_FEAT_R8 and links unitary to 1e-10 with every |U00| >= 0.1
+ * (cola_gauge_info_r8), else COLA_EINVAL.  Measured on B200 the 8-real links do not pay (the kernels become bound on the SM
+ * side: +7-10 % time for -13 % bytes); the format is kept as an option.
+ * cola_solve_params.mixed = 3 runs the inner iteration on it.  Spinor buffers and cola_spinor_* calls take COLA_F32. */
+typedef enum { COLA_F64 = 0, COLA_F32 = 1, COLA_F32_H16 = 2, COLA_F32_R8 = 3 } cola_prec;
 typedef enum { COLA_EVEN = 0, COLA_ODD = 1 } cola_parity;
 
 typedef struct {
@@ -95,8 +105,13 @@ cola_status cola_set_l2_budget(cola_ctx *c, size_t bytes);
  *                     cola_fermion_matrix_apply* in COLA_F32 / COLA_F32_H16 and by solves with even_odd = 0.  The fp64
  *                     operator on the full lattice is always available (the true residual |b - M x| needs it).
  *   COLA_FEAT_H16     16-bit links + fp16 clover: COLA_F32_H16 operators and mixed = 2.
+ *   COLA_FEAT_R8      8-real fp32 links: COLA_F32_R8 operators and mixed = 3.
+ *   COLA_FEAT_A72     the fp32 copy of A as packed 6x6 blocks (72 reals).  The fp32 kernels read A in its 48-real
+ *                     field-strength form (see COLA_F32_R8 above; -10 % bytes on M, measured -9 % time); the 72-real copy is
+ *                     only read after cola_set_compact cleared bit 1 (A/B measurements) and is always carved when
+ *                     trace_sub = 0, where the 48-real form does not exist.
  * A call that needs a missing feature returns COLA_EINVAL. */
-typedef enum { COLA_FEAT_FULL_M = 1, COLA_FEAT_H16 = 2, COLA_FEAT_ALL = 3 } cola_feature;
+typedef enum { COLA_FEAT_FULL_M = 1, COLA_FEAT_H16 = 2, COLA_FEAT_R8 = 4, COLA_FEAT_A72 = 8, COLA_FEAT_ALL = 15 } cola_feature;
 cola_status cola_set_features(cola_ctx *c, unsigned features);
 /* Tuning: which kernel family the single-right-hand-side fp32 / 16-bit operators use.  0: every thread loads its 8
  * neighbour spinors from global memory through L1; 1: a thread block owns a 4-D tile of sites and stages the tile's
@@ -105,6 +120,10 @@ cola_status cola_set_features(cola_ctx *c, unsigned features);
  * both modes (fused norms differ in summation order).  fp64 operators and lattices the tiles do not fit (X > 512) use
  * mode 0 regardless.  Default: DESIGN.md section 6 says which and why. */
 cola_status cola_set_staging(cola_ctx *c, int mode);
+/* Measurement aid.  bit 0: COLA_F32_R8 reads the 8-real links (else the context's fp32 links, 12 or 18 reals, i.e. it is
+ * COLA_F32); bit 1: the fp32 operators (COLA_F32, COLA_F32_R8) read A in its 48-real form (else the 72-real packed blocks,
+ * which needs COLA_FEAT_A72).  Default 3.  COLA_EINVAL outside 0..3. */
+cola_status cola_set_compact(cola_ctx *c, int mask);
 /* Change the stream subsequent calls launch on. */
 cola_status cola_set_stream(cola_ctx *c, void *stream);
 
@@ -131,6 +150,10 @@ cola_status cola_gauge_upload(cola_ctx *c, const double *host_links);
 cola_status cola_gauge_upload_dev(cola_ctx *c, const double *dev_links);
 /* Diagnostics of the last upload: max |U U^+ - 1| over all links. */
 cola_status cola_gauge_info(const cola_ctx *c, double *max_unitarity_dev);
+/* Diagnostics of the last upload for COLA_F32_R8: the smallest |U00| over all links.  The 8-real format rebuilds
+ * |U00| = sqrt(1 - |U01|^2 - |U02|^2), whose absolute error grows like eps/(2 |U00|); it is offered only when every
+ * |U00| >= 0.1 (true of the smooth ensembles of the configs, not of Haar-random links). */
+cola_status cola_gauge_info_r8(const cola_ctx *c, double *min_abs_u00);
 /* Diagnostics of the last upload (SURVEY O6 "report the smallest pivot it meets"): the smallest pivot of the unpivoted
  * Gauss-Jordan inversions of the 6x6 blocks of A_oo.  Valid (and <= 0) also after an upload that failed for it. */
 cola_status cola_clover_info(const cola_ctx *c, double *min_pivot);
@@ -163,7 +186,8 @@ typedef struct {
     int max_iter;      /* CGLS passes (one K and one K^+ each) */
     int even_odd;      /* 0: CGNR on M (BJ:c0); 1: CGNR on the Schur complement + reconstruction */
     int mixed;         /* 0: all fp64; 1: fp32 inner iteration with fp64 reliable updates;
-                          2: as 1, with the inner operator reading 16-bit links and clover (COLA_F32_H16) */
+                          2: as 1, with the inner operator reading 16-bit links and clover (COLA_F32_H16);
+                          3: as 1, with the inner operator reading 8-real links and the 48-real A (COLA_F32_R8) */
     double delta;      /* reliable-update threshold (mixed only); <= 0 selects the default 0.1 */
     int method;        /* COLA_CGNR (0, the north_star solver) or COLA_BICGSTAB: BiCGStab in van der
                           Vorst's order on the Schur system (needs even_odd = 1), x0 = 0, shadow residual = r0; one pass =

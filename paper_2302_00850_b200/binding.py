@@ -15,9 +15,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("COLA_LIBRARY_PATH") or os.path.join(_HERE, "libcola.so")
 
 COLA_OK, COLA_EINVAL, COLA_ECUDA, COLA_ENOTREADY, COLA_ENOCONV, COLA_ENOMEM = range(6)
-COLA_F64, COLA_F32, COLA_F32_H16 = 0, 1, 2
+COLA_F64, COLA_F32, COLA_F32_H16, COLA_F32_R8 = 0, 1, 2, 3
 COLA_EVEN, COLA_ODD = 0, 1
-COLA_FEAT_FULL_M, COLA_FEAT_H16, COLA_FEAT_ALL = 1, 2, 3
+COLA_FEAT_FULL_M, COLA_FEAT_H16, COLA_FEAT_R8, COLA_FEAT_A72, COLA_FEAT_ALL = 1, 2, 4, 8, 15
 COLA_CGNR, COLA_BICGSTAB = 0, 1
 _METHOD = {"cgnr": COLA_CGNR, "bicgstab": COLA_BICGSTAB, COLA_CGNR: COLA_CGNR, COLA_BICGSTAB: COLA_BICGSTAB}
 STATUS_NAMES = {0: "COLA_OK", 1: "COLA_EINVAL", 2: "COLA_ECUDA", 3: "COLA_ENOTREADY", 4: "COLA_ENOCONV", 5: "COLA_ENOMEM"}
@@ -31,7 +31,7 @@ EXPORTS = [
     "cola_launch_count",
     "cola_mrhs_workspace_bytes", "cola_set_mrhs_workspace", "cola_dslash_apply_mrhs", "cola_fermion_matrix_apply_mrhs",
     "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host", "cola_cg_solve_history", "cola_profile_kernel", "cola_profile_result",
-    "cola_set_features", "cola_clover_info", "cola_set_staging",
+    "cola_set_features", "cola_clover_info", "cola_set_staging", "cola_set_compact", "cola_gauge_info_r8",
     "cola_eig_workspace_bytes", "cola_eig_lowest", "cola_cg_solve_deflated",
 ]
 
@@ -89,6 +89,8 @@ def _load():
                                           ctypes.POINTER(ci), ci]
     lib.cola_set_features.argtypes = [vp, ctypes.c_uint]
     lib.cola_set_staging.argtypes = [vp, ci]
+    lib.cola_set_compact.argtypes = [vp, ci]
+    lib.cola_gauge_info_r8.argtypes = [vp, ctypes.POINTER(cd)]
     lib.cola_eig_workspace_bytes.argtypes = [vp, ctypes.POINTER(ColaEigParams)]
     lib.cola_eig_workspace_bytes.restype = ctypes.c_size_t
     lib.cola_eig_lowest.argtypes = [vp, ctypes.POINTER(ColaEigParams), vp, ctypes.c_size_t, ctypes.POINTER(cd), ctypes.POINTER(cd), vp,
@@ -221,6 +223,16 @@ class Cola:
         """0: neighbour spinors through L1; 1: staged in shared memory per 4-D tile (fp32 / 16-bit single-rhs kernels)."""
         self._ck(_lib.cola_set_staging(self._h, int(mode)))
 
+    def set_compact(self, mask: int):
+        """bit 0: COLA_F32_R8 reads the 8-real links; bit 1: the fp32 operators read A in its 48-real form (else 72 reals)."""
+        self._ck(_lib.cola_set_compact(self._h, int(mask)))
+
+    def gauge_info_r8(self) -> float:
+        """Smallest |U00| over the links of the last upload (COLA_F32_R8 needs >= 0.1)."""
+        v = ctypes.c_double()
+        self._ck(_lib.cola_gauge_info_r8(self._h, ctypes.byref(v)))
+        return v.value
+
     def set_features(self, features: int):
         """COLA_FEAT_* parts of the workspace to carve; call before set_workspace / gauge_upload."""
         self._ck(_lib.cola_set_features(self._h, int(features)))
@@ -313,34 +325,37 @@ class Cola:
         self._ck(_lib.cola_spinor_convert(self._h, dp, ctypes.c_void_p(src.data_ptr()), ctypes.c_void_p(out.data_ptr()), 2 if full else 1))
         return out
 
-    # ---- H3-H8.  h16=True (fp32 tensors only): COLA_F32_H16, the operator that reads 16-bit links and clover
+    # ---- H3-H8.  fp32 tensors only: h16=True (or fmt="h16") selects COLA_F32_H16, the operator that reads 16-bit links and
+    # fp16 clover; fmt="r8" selects COLA_F32_R8 (8-real links, 48-real A)
     @staticmethod
-    def _op_prec(t: torch.Tensor, h16: bool) -> int:
+    def _op_prec(t: torch.Tensor, h16: bool, fmt=None) -> int:
         pr = _PREC[t.dtype]
-        if h16:
+        if fmt not in (None, "h16", "r8"):
+            raise ValueError("fmt must be None, 'h16' or 'r8'")
+        if h16 or fmt is not None:
             if pr != COLA_F32:
-                raise ValueError("h16 operators take fp32 spinors")
-            return COLA_F32_H16
+                raise ValueError("h16 / r8 operators take fp32 spinors")
+            return COLA_F32_R8 if fmt == "r8" else COLA_F32_H16
         return pr
 
-    def dslash_apply(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
-        pr = self._op_prec(inp, h16)
+    def dslash_apply(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None, h16=False, fmt=None) -> torch.Tensor:
+        pr = self._op_prec(inp, h16, fmt)
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.Vh * 24
         if out is None:
             out = self.empty_internal(inp.dtype, full=False)
         self._ck(_lib.cola_dslash_apply(self._h, pr, int(out_parity), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def fermion_matrix_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
-        pr = self._op_prec(inp, h16)
+    def fermion_matrix_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False, fmt=None) -> torch.Tensor:
+        pr = self._op_prec(inp, h16, fmt)
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.V * 24
         if out is None:
             out = self.empty_internal(inp.dtype, full=True)
         self._ck(_lib.cola_fermion_matrix_apply(self._h, pr, int(bool(dagger)), ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def schur_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
-        pr = self._op_prec(inp, h16)
+    def schur_apply(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False, fmt=None) -> torch.Tensor:
+        pr = self._op_prec(inp, h16, fmt)
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == self.Vh * 24
         if out is None:
             out = self.empty_internal(inp.dtype, full=False)
@@ -482,8 +497,8 @@ class Cola:
         one = self.empty_internal(prec, full=full)
         return torch.empty((int(nrhs),) + tuple(one.shape), dtype=one.dtype, device=self.device)
 
-    def dslash_apply_mrhs(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
-        pr, nrhs = self._op_prec(inp, h16), inp.shape[0]
+    def dslash_apply_mrhs(self, out_parity: int, inp: torch.Tensor, out: torch.Tensor | None = None, h16=False, fmt=None) -> torch.Tensor:
+        pr, nrhs = self._op_prec(inp, h16, fmt), inp.shape[0]
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.Vh * 24
         self._need_mrhs(nrhs)
         if out is None:
@@ -491,8 +506,8 @@ class Cola:
         self._ck(_lib.cola_dslash_apply_mrhs(self._h, pr, int(out_parity), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def fermion_matrix_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
-        pr, nrhs = self._op_prec(inp, h16), inp.shape[0]
+    def fermion_matrix_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False, fmt=None) -> torch.Tensor:
+        pr, nrhs = self._op_prec(inp, h16, fmt), inp.shape[0]
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.V * 24
         self._need_mrhs(nrhs)
         if out is None:
@@ -500,8 +515,8 @@ class Cola:
         self._ck(_lib.cola_fermion_matrix_apply_mrhs(self._h, pr, int(bool(dagger)), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def schur_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False) -> torch.Tensor:
-        pr, nrhs = self._op_prec(inp, h16), inp.shape[0]
+    def schur_apply_mrhs(self, inp: torch.Tensor, dagger=False, out: torch.Tensor | None = None, h16=False, fmt=None) -> torch.Tensor:
+        pr, nrhs = self._op_prec(inp, h16, fmt), inp.shape[0]
         assert inp.is_cuda and inp.is_contiguous() and inp.numel() == nrhs * self.Vh * 24
         self._need_mrhs(nrhs)
         if out is None:

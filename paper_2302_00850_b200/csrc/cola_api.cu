@@ -23,9 +23,12 @@ struct cola_ctx {
     char *clovA64, *clovA32;        // [parity][chunk][Vh]
     char *clovI64, *clovI32;        // odd parity only
     char *gauge16, *clovA16, *clovI16;   // 16-bit copies for COLA_F32_H16 (same index structure)
+    char *gauge8, *clovG32;         // COLA_F32_R8: links as 8 fp32 reals, A as its 48-real field-strength form (COLA_FEAT_R8)
+    int r8_valid;                   // the 8-real links / 48-real A hold what the kernels assume (unitary links, traceless F)
+    int compact;                    // bit 0: COLA_F32_R8 reads the 8-real links; bit 1: the fp32 operators read A in its 48-real form (cola_set_compact)
     unsigned features;              // COLA_FEAT_* parts of the workspace that are carved (cola_set_features)
     int h16_valid;                  // the 16-bit link copy holds what the kernels assume (12 reals of a unitary matrix)
-    int sloppy16;                   // the running solve's inner operator reads the 16-bit fields
+    cola_prec inner_prec;           // operator precision of the running solve's fp32 iteration: COLA_F32, _H16 (mixed = 2) or _R8 (mixed = 3)
     double *hist;                   // HOST array of the running solve's residual history or nullptr (cola_cg_solve_history)
     int hist_len;
     int *upd_iters;                 // HOST array receiving the iterations at which reliable updates fired, or nullptr
@@ -50,6 +53,8 @@ struct cola_ctx {
     CtlB *ctlb;                     // device, inside the control block (BiCGStab scalars)
     unsigned long long *max_dev_bits;   // device (inside the same allocation)
     unsigned long long *min_pivot_key;  // device (inside the same allocation): see launch_clover_invert
+    unsigned long long *min_u00_bits;   // device (inside the same allocation): min |U00|^2 over the links of the last upload
+    double min_u00sq;
     double min_pivot;               // smallest Gauss-Jordan pivot of the 6x6 inverses of the last upload
     double *h_pinned;               // pinned host scalars
     HostStatus *h_status;           // mapped pinned host memory the device publishes the iteration status to
@@ -112,7 +117,7 @@ static size_t half_bytes(const cola_ctx *c, cola_prec prec) { return c->Vh * 24 
 static size_t scratch_half64(const cola_ctx *c) { return (c->features & COLA_FEAT_FULL_M) ? 12 : 9; }
 
 struct Carve {
-    size_t gauge64, gauge32, clovA64, clovA32, clovI64, clovI32, gauge16, clovA16, clovI16, tmp64, tmp32, partials, scratch, total;
+    size_t gauge64, gauge32, clovA64, clovA32, clovI64, clovI32, gauge16, clovA16, clovI16, gauge8, clovG32, tmp64, tmp32, partials, scratch, total;
 };
 
 static Carve carve(const cola_ctx *c)
@@ -126,12 +131,15 @@ static Carve carve(const cola_ctx *c)
     k.gauge64 = take(8 * 144 * Vh);
     k.gauge32 = take(8 * link_bytes(c->fmt32) * Vh);
     k.clovA64 = take(2 * 576 * Vh);         // fp64 A on both parities: the true residual is always |b - M x| on the full lattice
-    k.clovA32 = take(npar * 288 * Vh);
+    k.clovA32 = take(((c->features & COLA_FEAT_A72) || !c->p.trace_sub ? 1 : 0) * npar * 288 * Vh);
     k.clovI64 = take(576 * Vh);
     k.clovI32 = take(288 * Vh);
     k.gauge16 = take(h16 * 8 * link_bytes(LINK_I16_12) * Vh);
     k.clovA16 = take(h16 * npar * CLOVER_H16_BYTES * Vh);
     k.clovI16 = take(h16 * CLOVER_H16_BYTES * Vh);
+    const size_t r8 = (c->features & COLA_FEAT_R8) ? 1 : 0;
+    k.gauge8 = take(r8 * 8 * link_bytes(LINK_F32_8) * Vh);
+    k.clovG32 = take((c->p.trace_sub ? 1 : 0) * npar * CLOVER_G48_REALS * 4 * Vh);   // the form the fp32 kernels read A in (needs a traceless F)
     k.tmp64 = take(192 * Vh);
     k.tmp32 = take(96 * Vh);
     {
@@ -179,6 +187,8 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     c->fmt32 = p->compress12 ? LINK_F32_12 : LINK_F32_18;
     c->l2_budget = (size_t)40 << 20;
     c->features = COLA_FEAT_ALL;
+    c->compact = 3;
+    c->inner_prec = COLA_F32;
     c->stream = (cudaStream_t)p->stream;
     char *blk = nullptr;
     cudaError_t e = cudaMalloc(&blk, 4096);
@@ -206,6 +216,7 @@ cola_status cola_create(cola_ctx **out, const cola_params *p)
     c->ctlm = reinterpret_cast<CtlM *>(blk + 512);
     c->max_dev_bits = reinterpret_cast<unsigned long long *>(blk + 2048);
     c->min_pivot_key = reinterpret_cast<unsigned long long *>(blk + 2056);
+    c->min_u00_bits = reinterpret_cast<unsigned long long *>(blk + 2064);
     c->ctlb = reinterpret_cast<CtlB *>(blk + 2304);
     static_assert(sizeof(CtlB) <= 512, "control block layout");
     *out = c;
@@ -300,6 +311,14 @@ cola_status cola_set_features(cola_ctx *c, unsigned features)
     return COLA_OK;
 }
 
+cola_status cola_set_compact(cola_ctx *c, int mask)
+{
+    if (!c) return COLA_EINVAL;
+    if (mask < 0 || mask > 3) return fail(c, COLA_EINVAL, "cola_set_compact: mask must be 0..3");
+    c->compact = mask;
+    return COLA_OK;
+}
+
 cola_status cola_set_staging(cola_ctx *c, int mode)
 {
     if (!c) return COLA_EINVAL;
@@ -352,6 +371,9 @@ cola_status cola_set_workspace(cola_ctx *c, void *dev_ptr, size_t bytes)
     c->scratch = c->ws + k.scratch;
     c->scratch_bytes = scratch_half64(c) * 192 * c->Vh;
     if (!(c->features & COLA_FEAT_H16)) c->gauge16 = c->clovA16 = c->clovI16 = nullptr;
+    c->gauge8 = (c->features & COLA_FEAT_R8) ? c->ws + k.gauge8 : nullptr;
+    c->clovG32 = c->p.trace_sub ? c->ws + k.clovG32 : nullptr;
+    if (!((c->features & COLA_FEAT_A72) || !c->p.trace_sub)) c->clovA32 = nullptr;
     return COLA_OK;
 }
 
@@ -368,17 +390,26 @@ static cola_status need_ready(cola_ctx *c, const char *who)
     return COLA_OK;
 }
 
-static int fmt_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? (int)LINK_F64_18 : (prec == COLA_F32_H16 ? (int)LINK_I16_12 : c->fmt32); }
+static bool r8_links(const cola_ctx *c, cola_prec prec) { return prec == COLA_F32_R8 && (c->compact & 1); }
+// the fp32 operators (COLA_F32, COLA_F32_R8) read A in its 48-real form unless told otherwise (or F has a trace)
+static bool r8_clover(const cola_ctx *c, cola_prec prec) { return (prec == COLA_F32_R8 || prec == COLA_F32) && c->clovG32 && ((c->compact & 2) || !c->clovA32); }
+static int fmt_of(const cola_ctx *c, cola_prec prec)
+{
+    if (r8_links(c, prec)) return (int)LINK_F32_8;
+    return prec == COLA_F64 ? (int)LINK_F64_18 : (prec == COLA_F32_H16 ? (int)LINK_I16_12 : c->fmt32);
+}
 static char *gauge_of(const cola_ctx *c, cola_prec prec, int parity)
 {
     if (prec == COLA_F64) return c->gauge64 + (size_t)parity * 4 * 144 * c->Vh;
     if (prec == COLA_F32_H16) return c->gauge16 + (size_t)parity * 4 * link_bytes(LINK_I16_12) * c->Vh;
+    if (r8_links(c, prec)) return c->gauge8 + (size_t)parity * 4 * link_bytes(LINK_F32_8) * c->Vh;
     return c->gauge32 + (size_t)parity * 4 * link_bytes(c->fmt32) * c->Vh;
 }
 static char *clovA_of(const cola_ctx *c, cola_prec prec, int parity)
 {
     if (prec == COLA_F64) return c->clovA64 + (size_t)parity * 576 * c->Vh;
     if (prec == COLA_F32_H16) return c->clovA16 + (size_t)parity * CLOVER_H16_BYTES * c->Vh;
+    if (r8_clover(c, prec)) return c->clovG32 + (size_t)parity * CLOVER_G48_REALS * 4 * c->Vh;
     return c->clovA32 + (size_t)parity * 288 * c->Vh;
 }
 static char *clovI_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64 ? c->clovI64 : (prec == COLA_F32_H16 ? c->clovI16 : c->clovI32); }
@@ -388,7 +419,12 @@ static char *tmp_of(const cola_ctx *c, cola_prec prec) { return prec == COLA_F64
 // reads A on `parity` (the fp32 / fp16 copies of A_oo exist only with COLA_FEAT_FULL_M).
 static cola_status check_prec(cola_ctx *c, cola_prec prec, int parity, int uses_A)
 {
-    if ((int)prec < 0 || (int)prec > (int)COLA_F32_H16) return fail(c, COLA_EINVAL, "unknown cola_prec");
+    if ((int)prec < 0 || (int)prec > (int)COLA_F32_R8) return fail(c, COLA_EINVAL, "unknown cola_prec");
+    if (prec == COLA_F32_R8) {
+        if (!(c->features & COLA_FEAT_R8)) return fail(c, COLA_EINVAL, "COLA_F32_R8 / mixed = 3 need COLA_FEAT_R8 (cola_set_features)");
+        if (!c->r8_valid)
+            return fail(c, COLA_EINVAL, "COLA_F32_R8 / mixed = 3: needs links unitary to 1e-10 with every |U00| >= 0.1 (8-real parametrisation of SU(3); cola_gauge_info_r8)");
+    }
     if (prec == COLA_F32_H16) {
         if (!(c->features & COLA_FEAT_H16)) return fail(c, COLA_EINVAL, "COLA_F32_H16 / mixed = 2 need COLA_FEAT_H16 (cola_set_features)");
         if (!c->h16_valid)
@@ -413,6 +449,7 @@ static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, c
     a.gauge_q = gauge_of(c, prec, 1 - parity);
     a.y = y;
     a.clov_y = (y && clov_on_y) ? clovA_of(c, prec, parity) : nullptr;
+    a.clov_y_g48 = (a.clov_y && r8_clover(c, prec)) ? 1 : 0;
     a.clov_post = post_inv ? clovI_of(c, prec) : nullptr;
     a.coef = coef;
     a.sgn = dagger ? +1.0 : -1.0;
@@ -483,12 +520,16 @@ static cola_status gauge_finish(cola_ctx *c)
     CK(cudaMemcpyAsync(&bits, c->max_dev_bits, sizeof(bits), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     memcpy(&c->max_unitarity_dev, &bits, sizeof(double));
+    CK(cudaMemcpyAsync(&bits, c->min_u00_bits, sizeof(bits), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    memcpy(&c->min_u00sq, &bits, sizeof(double));
     if (c->p.compress12 && !(c->max_unitarity_dev <= 1e-10))
         return fail(c, COLA_EINVAL, "cola_gauge_upload: links are not unitary to 1e-10; 12-real compression would be wrong");
     // the 16-bit copy stores rows 1 and 2 clamped to [-1, 1] and rebuilds row 3: only right for unitary links
     c->h16_valid = (c->features & COLA_FEAT_H16) && c->max_unitarity_dev <= 1e-10;
+    c->r8_valid = (c->features & COLA_FEAT_R8) && c->max_unitarity_dev <= 1e-10 && c->min_u00sq >= R8_MIN_U00SQ;
     CK(launch_clover_build(c->g, c->gauge64, c->p.kappa * c->p.csw, c->p.trace_sub, c->clovA64, c->clovA32, (c->features & COLA_FEAT_FULL_M) ? 2 : 1,
-                           c->clovA16, c->stream));
+                           c->clovA16, c->clovG32, c->stream));
     CK(cudaMemsetAsync(c->min_pivot_key, 0xff, sizeof(unsigned long long), c->stream));
     CK(launch_clover_invert(c->g, c->clovA64 + 576 * c->Vh, c->clovI64, c->clovI32, c->clovI16, c->min_pivot_key, c->stream));
     c->launches += 2;
@@ -510,8 +551,9 @@ static cola_status gauge_upload_impl(cola_ctx *c, const double *links, int on_ho
     CK(cudaSetDevice(c->p.device));
     c->ready = 0;
     CK(cudaMemsetAsync(c->max_dev_bits, 0, sizeof(unsigned long long), c->stream));
+    CK(cudaMemsetAsync(c->min_u00_bits, 0x7f, sizeof(unsigned long long), c->stream));   // 0x7f7f...: a huge positive double
     if (!on_host) {
-        CK(launch_gauge_reorder(c->g, links, 0, (long)c->V, c->gauge64, c->gauge32, c->fmt32, c->gauge16, c->max_dev_bits, c->stream));
+        CK(launch_gauge_reorder(c->g, links, 0, (long)c->V, c->gauge64, c->gauge32, c->fmt32, c->gauge16, c->gauge8, c->max_dev_bits, c->min_u00_bits, c->stream));
         c->launches++;
         return gauge_finish(c);
     }
@@ -521,7 +563,7 @@ static cola_status gauge_upload_impl(cola_ctx *c, const double *links, int on_ho
     for (size_t lo = 0; lo < c->V; lo += chunk_sites) {
         const size_t n = (c->V - lo < chunk_sites) ? c->V - lo : chunk_sites;
         CK(cudaMemcpyAsync(c->scratch, links + lo * 72, n * per_site, cudaMemcpyHostToDevice, c->stream));
-        CK(launch_gauge_reorder(c->g, (const double *)c->scratch, (long)lo, (long)n, c->gauge64, c->gauge32, c->fmt32, c->gauge16, c->max_dev_bits, c->stream));
+        CK(launch_gauge_reorder(c->g, (const double *)c->scratch, (long)lo, (long)n, c->gauge64, c->gauge32, c->fmt32, c->gauge16, c->gauge8, c->max_dev_bits, c->min_u00_bits, c->stream));
         c->launches++;
     }
     return gauge_finish(c);
@@ -539,8 +581,8 @@ struct System {            // K x = rhs on n_sites sites; K = S (even_odd) or M
 
 cola_status apply_K(cola_ctx *c, const System &sy, cola_prec prec, int dagger, const void *in, void *out, double *norm_out, const int *skip = nullptr)
 {
-    // the inner fp32 iteration of a mixed = 2 solve reads the 16-bit links and clover (same fp32 vectors)
-    const cola_prec op = (prec == COLA_F32 && c->sloppy16) ? COLA_F32_H16 : prec;
+    // the inner fp32 iteration of a mixed = 2 / 3 solve reads the 16-bit / compact fields (same fp32 vectors)
+    const cola_prec op = (prec == COLA_F32) ? c->inner_prec : prec;
     return sy.even_odd ? schur(c, op, dagger, in, out, norm_out, skip) : fmatrix(c, op, dagger, in, out, norm_out, skip);
 }
 
@@ -629,11 +671,12 @@ static cola_status solve_impl(cola_ctx *c, const cola_solve_params *sp, const vo
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve: tol must be > 0 and max_iter >= 1");
     CK(cudaSetDevice(c->p.device));
     memset(info, 0, sizeof(*info));
-    if (sp->mixed < 0 || sp->mixed > 2) return fail(c, COLA_EINVAL, "cola_cg_solve: mixed must be 0, 1 or 2");
+    if (sp->mixed < 0 || sp->mixed > 3) return fail(c, COLA_EINVAL, "cola_cg_solve: mixed must be 0, 1, 2 or 3");
     if (sp->mixed == 2) ST(check_prec(c, COLA_F32_H16, 0, 0));
+    if (sp->mixed == 3) ST(check_prec(c, COLA_F32_R8, 0, 0));
     if (!sp->even_odd && !(c->features & COLA_FEAT_FULL_M))
         return fail(c, COLA_EINVAL, "cola_cg_solve: even_odd = 0 (CGNR on M) needs COLA_FEAT_FULL_M (cola_set_features)");
-    c->sloppy16 = sp->mixed == 2;
+    c->inner_prec = sp->mixed == 2 ? COLA_F32_H16 : (sp->mixed == 3 ? COLA_F32_R8 : COLA_F32);
     const double delta = sp->delta > 0 ? sp->delta : 0.1;
     const double kappa = c->p.kappa;
     const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32);
@@ -859,10 +902,11 @@ static cola_status solve_bicgstab_impl(cola_ctx *c, const cola_solve_params *sp,
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve: tol must be > 0 and max_iter >= 1");
     CK(cudaSetDevice(c->p.device));
     memset(info, 0, sizeof(*info));
-    if (sp->mixed < 0 || sp->mixed > 2) return fail(c, COLA_EINVAL, "cola_cg_solve: mixed must be 0, 1 or 2");
+    if (sp->mixed < 0 || sp->mixed > 3) return fail(c, COLA_EINVAL, "cola_cg_solve: mixed must be 0, 1, 2 or 3");
     if (!sp->even_odd) return fail(c, COLA_EINVAL, "cola_cg_solve: BiCGStab is offered on the Schur system only (even_odd = 1)");
     if (sp->mixed == 2) ST(check_prec(c, COLA_F32_H16, 0, 0));
-    c->sloppy16 = sp->mixed == 2;
+    if (sp->mixed == 3) ST(check_prec(c, COLA_F32_R8, 0, 0));
+    c->inner_prec = sp->mixed == 2 ? COLA_F32_H16 : (sp->mixed == 3 ? COLA_F32_R8 : COLA_F32);
     const double delta = sp->delta > 0 ? sp->delta : 0.1;
     const double kappa = c->p.kappa;
     const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32);
@@ -1322,6 +1366,7 @@ cola_status dslash_m(cola_ctx *c, cola_prec prec, int parity, int dagger, const 
     a.gauge_q = gauge_of(c, prec, 1 - parity);
     a.y = y;
     a.clov_y = (y && clov_on_y) ? clovA_of(c, prec, parity) : nullptr;
+    a.clov_y_g48 = (a.clov_y && r8_clover(c, prec)) ? 1 : 0;
     a.clov_post = post_inv ? clovI_of(c, prec) : nullptr;
     a.coef = coef;
     a.sgn = dagger ? +1.0 : -1.0;
@@ -1388,7 +1433,7 @@ cola_status first_half_m(cola_ctx *c, int k, const MrhsList &A, int na)
     CtlM *cm = c->ctlm;
     const size_t h32 = half_bytes(c, COLA_F32);
     const int nb = blas_mrhs_blocks(c->Vh, COLA_F32);
-    ST(schur_m(c, c->sloppy16 ? COLA_F32_H16 : COLA_F32, 0, A, na, c->m_p32, h32, c->m_tmp32, c->m_q32, h32, cm->qq, &cm->flag));
+    ST(schur_m(c, c->inner_prec, 0, A, na, c->m_p32, h32, c->m_tmp32, c->m_q32, h32, cm->qq, &cm->flag));
     CK(launch_r_update_mrhs(COLA_F32, c->m_r32, c->m_q32, h32, cm, k & 1, A, na, &cm->flag, c->Vh, c->m_partials, c->stream));
     CK(launch_mrhs_reduce(c->m_partials, nb, na, A.v, cm->rr, 0, &cm->flag, c->stream));
     CK(launch_decide_mrhs(cm, A, na, k + 1, &cm->flag, c->d_statusm + (k & 1), c->stream));
@@ -1401,7 +1446,7 @@ cola_status second_half_m(cola_ctx *c, int k, int do_x, const MrhsList &A, int n
 {
     CtlM *cm = c->ctlm;
     const size_t h32 = half_bytes(c, COLA_F32);
-    ST(schur_m(c, c->sloppy16 ? COLA_F32_H16 : COLA_F32, 1, A, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[(k & 1) ^ 1], &cm->flag));
+    ST(schur_m(c, c->inner_prec, 1, A, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[(k & 1) ^ 1], &cm->flag));
     CK(launch_xp_update_mrhs(COLA_F32, c->m_x32, c->m_p32, c->m_q32, h32, cm, k & 1, A, na, do_x, 1, &cm->flag, c->Vh, c->stream));
     c->launches++;
     return COLA_OK;
@@ -1421,11 +1466,12 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
     ST(need_mrhs(c, "cola_cg_solve_mrhs", nrhs));
     if (!sp || !b_canon_dev || !x_canon_dev || !infos) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: NULL argument");
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: tol must be > 0 and max_iter >= 1");
-    if (!sp->even_odd || sp->mixed < 1 || sp->mixed > 2 || sp->method != COLA_CGNR)
-        return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd CGNR solver is batched (even_odd = 1, mixed = 1 or 2, method = COLA_CGNR)");
+    if (!sp->even_odd || sp->mixed < 1 || sp->mixed > 3 || sp->method != COLA_CGNR)
+        return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd CGNR solver is batched (even_odd = 1, mixed = 1, 2 or 3, method = COLA_CGNR)");
     if (sp->mixed == 2) ST(check_prec(c, COLA_F32_H16, 0, 0));
+    if (sp->mixed == 3) ST(check_prec(c, COLA_F32_R8, 0, 0));
     if (!c->m_solver) return fail(c, COLA_ENOTREADY, "cola_cg_solve_mrhs: the multi-rhs workspace was sized for operators only (cola_mrhs_workspace_bytes with for_solver = 1)");
-    c->sloppy16 = sp->mixed == 2;
+    c->inner_prec = sp->mixed == 2 ? COLA_F32_H16 : (sp->mixed == 3 ? COLA_F32_R8 : COLA_F32);
     CK(cudaSetDevice(c->p.device));
     const double delta = sp->delta > 0 ? sp->delta : 0.1, kappa = c->p.kappa;
     const size_t h64 = half_bytes(c, COLA_F64), h32 = half_bytes(c, COLA_F32), f64 = 2 * h64;
@@ -1480,7 +1526,7 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
         st.delta2 = delta * delta;
         CK(cudaMemcpyAsync(cm, &st, sizeof(st), cudaMemcpyHostToDevice, c->stream));
         MrhsList L = list_of(A, na);
-        ST(schur_m(c, c->sloppy16 ? COLA_F32_H16 : COLA_F32, 1, L, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[0], nullptr));    // s0 = S^+ r0, gamma_0
+        ST(schur_m(c, c->inner_prec, 1, L, na, c->m_r32, h32, c->m_tmp32, c->m_q32, h32, cm->gam[0], nullptr));    // s0 = S^+ r0, gamma_0
         CK(cudaMemcpyAsync(c->m_p32, c->m_q32, (size_t)nrhs * h32, cudaMemcpyDeviceToDevice, c->stream));
         for (int j = 0; j < na; j++) flops[A[j]] += flops_K;
         c->h_statusm[0].iters = c->h_statusm[1].iters = 0;
@@ -1599,6 +1645,13 @@ cola_status cola_gauge_info(const cola_ctx *c, double *max_unitarity_dev)
 {
     if (!c || !max_unitarity_dev) return COLA_EINVAL;
     *max_unitarity_dev = c->max_unitarity_dev;
+    return COLA_OK;
+}
+
+cola_status cola_gauge_info_r8(const cola_ctx *c, double *min_abs_u00)
+{
+    if (!c || !min_abs_u00) return COLA_EINVAL;
+    *min_abs_u00 = sqrt(c->min_u00sq);
     return COLA_OK;
 }
 

@@ -170,7 +170,8 @@ __device__ __forceinline__ void store_block(char *c64, char *c32, char *c16, siz
 }
 
 // one thread per site: tid < 2*Vh, parity = tid / Vh
-__global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *gauge64, double k, int trace_sub, char *A64, char *A32, int a32_parities, char *A16)
+__global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *gauge64, double k, int trace_sub, char *A64, char *A32, int a32_parities, char *A16,
+                                                          char *G32)
 {
     const long tid = (long)blockIdx.x * CB + threadIdx.x;
     if (tid >= 2L * g.Vh) return;
@@ -197,9 +198,30 @@ __global__ void __launch_bounds__(CB) clover_build_kernel(Geom g, const char *ga
     char *a64 = A64 + (size_t)parity * 72 * 8 * Vh;
     char *a32 = (A32 && parity < a32_parities) ? A32 + (size_t)parity * 72 * 4 * Vh : nullptr;   // fp32 A on the odd parity is optional
     char *a16 = (A16 && parity < a32_parities) ? A16 + (size_t)parity * CLOVER_H16_BYTES * Vh : nullptr;
+    char *g32 = (G32 && parity < a32_parities) ? G32 + (size_t)parity * CLOVER_G48_REALS * 4 * Vh : nullptr;
 #pragma unroll
     for (int blk = 0; blk < 2; blk++) {
         const double sg = blk == 0 ? 1.0 : -1.0;
+        if (g32) {   // 48-real form: G_j = -k B_j as [d0, d1, l10, l20, l21], order G3, G1, G2 (load_clover_g48 in cola_device.cuh)
+            float f[24];
+            const int e_of[5] = {0, 4, 3, 6, 7};   // (0,0) (1,1) | (1,0) (2,0) (2,1) in row-major 3x3
+#pragma unroll
+            for (int q = 0; q < 5; q++) {
+                const int e = e_of[q];
+                const double B1r = sg * Fxt.r[e] - Fyz.r[e], B1i = sg * Fxt.i[e] - Fyz.i[e];
+                const double B2r = Fxz.r[e] + sg * Fyt.r[e], B2i = Fxz.i[e] + sg * Fyt.i[e];
+                const double B3r = sg * Fzt.r[e] - Fxy.r[e], B3i = sg * Fzt.i[e] - Fxy.i[e];
+                if (q < 2) {
+                    f[q] = (float)(-k * B3r); f[8 + q] = (float)(-k * B1r); f[16 + q] = (float)(-k * B2r);
+                } else {
+                    const int o = 2 + 2 * (q - 2);
+                    f[o] = (float)(-k * B3r); f[o + 1] = (float)(-k * B3i);
+                    f[8 + o] = (float)(-k * B1r); f[8 + o + 1] = (float)(-k * B1i);
+                    f[16 + o] = (float)(-k * B2r); f[16 + o + 1] = (float)(-k * B2i);
+                }
+            }
+            store_reals<float, 24>(reinterpret_cast<float4 *>(g32) + (size_t)blk * 6 * Vh, Vh, i, f);
+        }
         double br[36], bi[36];
 #pragma unroll
         for (int a = 0; a < 3; a++)
@@ -336,10 +358,12 @@ __global__ void __launch_bounds__(CB) clover_unpack_kernel(Geom g, const char *c
 
 }  // namespace
 
-cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, int a32_parities, void *clovA16, cudaStream_t s)
+cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, int a32_parities, void *clovA16,
+                                void *clovG32, cudaStream_t s)
 {
     const long n = 2L * g.Vh;
-    clover_build_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)gauge64, kappa_csw, trace_sub, (char *)clovA64, (char *)clovA32, a32_parities, (char *)clovA16);
+    clover_build_kernel<<<(unsigned)((n + CB - 1) / CB), CB, 0, s>>>(g, (const char *)gauge64, kappa_csw, trace_sub, (char *)clovA64, (char *)clovA32, a32_parities, (char *)clovA16,
+                                                                     (char *)clovG32);
     return cudaGetLastError();
 }
 

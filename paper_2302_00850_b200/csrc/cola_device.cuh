@@ -155,6 +155,7 @@ template <> struct LinkT<LINK_F64_18> { typedef double T; };
 template <> struct LinkT<LINK_F32_18> { typedef float T; };
 template <> struct LinkT<LINK_F32_12> { typedef float T; };
 template <> struct LinkT<LINK_I16_12> { typedef float T; };
+template <> struct LinkT<LINK_F32_8> { typedef float T; };
 
 // two 16-bit fixed-point reals (x 32767) of one 32-bit word
 __device__ __forceinline__ void unpack_i16(unsigned w, float &a, float &b)
@@ -178,6 +179,74 @@ template <> struct RawLink<LINK_F64_18> { double r[18]; };
 template <> struct RawLink<LINK_F32_18> { float r[18]; };
 template <> struct RawLink<LINK_F32_12> { float r[12]; };
 template <> struct RawLink<LINK_I16_12> { unsigned w[6]; };
+template <> struct RawLink<LINK_F32_8> { float r[8]; };
+
+// ---- 8-real links (LINK_F32_8; layout and flags in cola_internal.h).  With row 1 = (a1, a2, a3), N = |a2|^2 + |a3|^2,
+// |a1| = sqrt(1 - N), (b1, c1) the first-column entries of rows 2 and 3, |c1| = sqrt(N - |b1|^2), unitarity and det = 1 give
+//   b2 = x a2 + y conj(a3),  b3 = x a3 - y conj(a2),   x  = -conj(a1) b1 / N,  y  = -conj(c1) / N,
+//   c2 = x' a2 + y' conj(a3), c3 = x' a3 - y' conj(a2),  x' = -conj(a1) c1 / N,  y' =  conj(b1) / N.
+// MUFU approximations (sin/cos, rcp, sqrt) are accurate to ~4e-7 absolute on a link entry: "additional computation
+// in order to reduce traffic from global memory".  COLA_R8_EXACT_TRIG = 1 uses sincospif instead.
+#ifndef COLA_R8_EXACT_TRIG
+#define COLA_R8_EXACT_TRIG 0
+#endif
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float sqrt_approx(float x)
+{
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ void sincospi_(float x, float &sn, float &cs)
+{
+#if COLA_R8_EXACT_TRIG
+    sincospif(x, &sn, &cs);
+#else
+    __sincosf(3.14159265358979323846f * x, &sn, &cs);
+#endif
+}
+__device__ __forceinline__ void reconstruct8(const float (&s)[8], float (&u)[18])
+{
+    const float a2r = s[0], a2i = s[1], a3r = s[2], a3i = s[3], b1r = s[4], b1i = s[5];
+    const bool blockdiag = (__float_as_uint(s[6]) & 1u) != 0u, swapped = (__float_as_uint(s[7]) & 1u) != 0u;
+    float s1, c1, s2, c2;
+    sincospi_(s[6], s1, c1);
+    sincospi_(s[7], s2, c2);
+    if (blockdiag) {   // U = [[e, 0, 0], [0, p, q], [0, -conj(q) conj(e), conj(p) conj(e)]], e = exp(i th1), p, q in the a2, a3 slots
+        u[0] = c1; u[1] = s1; u[2] = 0; u[3] = 0; u[4] = 0; u[5] = 0;
+        u[6] = 0; u[7] = 0; u[8] = a2r; u[9] = a2i; u[10] = a3r; u[11] = a3i;
+        u[12] = 0; u[13] = 0;
+        u[14] = a3i * s1 - a3r * c1; u[15] = a3r * s1 + a3i * c1;
+        u[16] = a2r * c1 - a2i * s1; u[17] = -(a2r * s1 + a2i * c1);
+        return;
+    }
+    const float N = fma_(a2r, a2r, fma_(a2i, a2i, fma_(a3r, a3r, a3i * a3i)));
+    const float rN = rcp_approx(N);
+    const float m1 = sqrt_approx(fmaxf(1.0f - N, 0.0f));
+    const float mc = sqrt_approx(fmaxf(fma_(-b1r, b1r, fma_(-b1i, b1i, N)), 0.0f));
+    const float a1r = m1 * c1, a1i = m1 * s1, c1r = mc * c2, c1i = mc * s2;
+    const float xr = -rN * fma_(a1r, b1r, a1i * b1i), xi = -rN * fma_(a1r, b1i, -(a1i * b1r));
+    const float pr = -rN * fma_(a1r, c1r, a1i * c1i), pi = -rN * fma_(a1r, c1i, -(a1i * c1r));
+    const float yr = -rN * c1r, yi = rN * c1i;
+    const float qr = rN * b1r, qi = -rN * b1i;
+    // z a2 + w conj(a3),  z a3 - w conj(a2)
+    const float b2r = fma_(yi, a3i, fma_(yr, a3r, fma_(-xi, a2i, xr * a2r))), b2i = fma_(yi, a3r, fma_(-yr, a3i, fma_(xi, a2r, xr * a2i)));
+    const float b3r = fma_(-yi, a2i, fma_(-yr, a2r, fma_(-xi, a3i, xr * a3r))), b3i = fma_(-yi, a2r, fma_(yr, a2i, fma_(xi, a3r, xr * a3i)));
+    const float c2r = fma_(qi, a3i, fma_(qr, a3r, fma_(-pi, a2i, pr * a2r))), c2i = fma_(qi, a3r, fma_(-qr, a3i, fma_(pi, a2r, pr * a2i)));
+    const float c3r = fma_(-qi, a2i, fma_(-qr, a2r, fma_(-pi, a3i, pr * a3r))), c3i = fma_(-qi, a2r, fma_(qr, a2i, fma_(pi, a3r, pr * a3i)));
+    u[0] = a1r; u[1] = a1i; u[2] = a2r; u[3] = a2i; u[4] = a3r; u[5] = a3i;
+    const float rb[6] = {b1r, b1i, b2r, b2i, b3r, b3i}, rc[6] = {c1r, c1i, c2r, c2i, c3r, c3i};
+#pragma unroll
+    for (int k = 0; k < 6; k++) {   // swapped: the stored pair was (U20, -U10): row 2 = -rc, row 3 = rb
+        u[6 + k] = swapped ? -rc[k] : rb[k];
+        u[12 + k] = swapped ? rb[k] : rc[k];
+    }
+}
 
 // base = start of the [chunk][Vh] block of one (parity, mu)
 // STREAM: read-once data, no L1 allocation (single right-hand side); !STREAM: the same link is read by the
@@ -195,6 +264,8 @@ __device__ __forceinline__ void load_raw_link(const char *base, size_t Vh, size_
         raw.w[0] = a.x; raw.w[1] = a.y; raw.w[2] = a.z; raw.w[3] = a.w; raw.w[4] = b.x; raw.w[5] = b.y;
     } else if constexpr (FMT == LINK_F32_12) {
         load_reals<float, 12, STREAM>(base, Vh, i, raw.r);
+    } else if constexpr (FMT == LINK_F32_8) {
+        load_reals<float, 8, STREAM>(base, Vh, i, raw.r);
     } else {
         float r[16];
         load_reals<float, 16, STREAM>(base, Vh, i, r);
@@ -217,6 +288,8 @@ __device__ __forceinline__ void expand_link(const RawLink<FMT> &raw, typename Li
 #pragma unroll
         for (int k = 0; k < 6; k++) unpack_i16(raw.w[k], u[2 * k], u[2 * k + 1]);
         reconstruct_row3(u);
+    } else if constexpr (FMT == LINK_F32_8) {
+        reconstruct8(raw.r, u);
     } else {
 #pragma unroll
         for (int k = 0; k < 12; k++) u[k] = raw.r[k];
@@ -287,6 +360,45 @@ __device__ __forceinline__ void clover_apply(const void *clov, size_t Vh, size_t
         } else {
             load_reals<T, 36, STREAM>(reinterpret_cast<const V *>(clov) + (size_t)b * (36 / N) * Vh, Vh, i, c);
         }
+        clover_block_mul(c, &v[12 * b], &w[12 * b]);
+    }
+}
+
+// Packed 36 reals of chiral block b of A from its 48-real form (CLOVER_G48_REALS in cola_internal.h):
+//   block = 1 + [[G3, G1 - i G2], [G1 + i G2, -G3]],  G_j traceless Hermitian 3x3 as [d0, d1, l10, l20, l21]
+template <typename T, bool STREAM>
+__device__ __forceinline__ void load_clover_g48(const void *clov, size_t Vh, size_t i, int b, T (&c)[36])
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = VT<T>::N;
+    T g[24];
+    load_reals<T, 24, STREAM>(reinterpret_cast<const V *>(clov) + (size_t)b * (24 / N) * Vh, Vh, i, g);
+    const T *G3 = g, *G1 = g + 8, *G2 = g + 16;
+    const T one = 1, d32 = -(G3[0] + G3[1]);
+    c[0] = one + G3[0]; c[1] = one + G3[1]; c[2] = one + d32;
+    c[3] = one - G3[0]; c[4] = one - G3[1]; c[5] = one - d32;
+    c[6] = G3[2]; c[7] = G3[3]; c[8] = G3[4]; c[9] = G3[5]; c[10] = G3[6]; c[11] = G3[7];       // (1,0) (2,0) (2,1)
+    c[12] = G1[0]; c[13] = G2[0];                                                               // (3,0) = W_00, W = G1 + i G2
+    c[14] = G1[2] + G2[3]; c[15] = G2[2] - G1[3];                                               // (3,1) = W_01 = conj(l10_1) + i conj(l10_2)
+    c[16] = G1[4] + G2[5]; c[17] = G2[4] - G1[5];                                               // (3,2) = W_02
+    c[18] = G1[2] - G2[3]; c[19] = G1[3] + G2[2];                                               // (4,0) = W_10 = l10_1 + i l10_2
+    c[20] = G1[1]; c[21] = G2[1];                                                               // (4,1) = W_11
+    c[22] = G1[6] + G2[7]; c[23] = G2[6] - G1[7];                                               // (4,2) = W_12
+    c[24] = -G3[2]; c[25] = -G3[3];                                                             // (4,3) = -G3_10
+    c[26] = G1[4] - G2[5]; c[27] = G1[5] + G2[4];                                               // (5,0) = W_20
+    c[28] = G1[6] - G2[7]; c[29] = G1[7] + G2[6];                                               // (5,1) = W_21
+    c[30] = -(G1[0] + G1[1]); c[31] = -(G2[0] + G2[1]);                                         // (5,2) = W_22
+    c[32] = -G3[4]; c[33] = -G3[5]; c[34] = -G3[6]; c[35] = -G3[7];                             // (5,3) (5,4)
+}
+
+// w = A(site i) v with A in its 48-real form
+template <typename T, bool STREAM = true>
+__device__ __forceinline__ void clover_apply_g48(const void *clov, size_t Vh, size_t i, const T (&v)[24], T (&w)[24])
+{
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+        T c[36];
+        load_clover_g48<T, STREAM>(clov, Vh, i, b, c);
         clover_block_mul(c, &v[12 * b], &w[12 * b]);
     }
 }

@@ -309,7 +309,7 @@ __global__ void __launch_bounds__(DSLASH_BLOCK) clover_apply_kernel(int Vh, cons
 template <int FMT>
 cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
 {
-    const int xpay = a.y ? (a.clov_y ? 2 : 1) : 0;
+    const int xpay = a.y ? (a.clov_y ? (a.clov_y_g48 ? 3 : 2) : 1) : 0;
     const int post = a.clov_post ? 1 : 0;
     const dim3 grid((a.g.Vh + DSLASH_BLOCK - 1) / DSLASH_BLOCK), block(DSLASH_BLOCK);
     if (xpay == 0 && post == 0) launch_pdl(dslash_kernel<FMT, 0, 0>, grid, block, s, a);
@@ -317,7 +317,10 @@ cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
     else if (xpay == 1 && post == 0) launch_pdl(dslash_kernel<FMT, 1, 0>, grid, block, s, a);
     else if (xpay == 1 && post == 1) launch_pdl(dslash_kernel<FMT, 1, 1>, grid, block, s, a);
     else if (xpay == 2 && post == 0) launch_pdl(dslash_kernel<FMT, 2, 0>, grid, block, s, a);
-    else return cudaErrorInvalidValue;
+    else if (xpay == 3 && post == 0) {
+        if constexpr (FMT == LINK_F32_12 || FMT == LINK_F32_8 || FMT == LINK_F32_18) launch_pdl(dslash_kernel<FMT, 3, 0>, grid, block, s, a);
+        else return cudaErrorInvalidValue;   // the 48-real form of A exists in fp32 only
+    } else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
 
@@ -325,7 +328,7 @@ template <int FMT>
 cudaError_t launch_mrhs_fmt(MrhsArgs &m, cudaStream_t s)
 {
     constexpr int NRB = MrhsCfg<FMT>::NRB;
-    const int xpay = m.d.y ? (m.d.clov_y ? 2 : 1) : 0;
+    const int xpay = m.d.y ? (m.d.clov_y ? (m.d.clov_y_g48 ? 3 : 2) : 1) : 0;
     const int post = m.d.clov_post ? 1 : 0;
     m.tile = make_tile(m.d.g, MSITES, COLA_MRHS_TILE_X);
     m.nsb = m.tile.ntiles;
@@ -347,7 +350,10 @@ cudaError_t launch_mrhs_fmt(MrhsArgs &m, cudaStream_t s)
     else if (xpay == 1 && post == 0) dslash_mrhs_kernel<FMT, 1, 0><<<grid, block, 0, s>>>(m);
     else if (xpay == 1 && post == 1) dslash_mrhs_kernel<FMT, 1, 1><<<grid, block, 0, s>>>(m);
     else if (xpay == 2 && post == 0) dslash_mrhs_kernel<FMT, 2, 0><<<grid, block, 0, s>>>(m);
-    else return cudaErrorInvalidValue;
+    else if (xpay == 3 && post == 0) {
+        if constexpr (FMT == LINK_F32_12 || FMT == LINK_F32_8 || FMT == LINK_F32_18) dslash_mrhs_kernel<FMT, 3, 0><<<grid, block, 0, s>>>(m);
+        else return cudaErrorInvalidValue;
+    } else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
 
@@ -428,6 +434,7 @@ cudaError_t launch_dslash_mrhs(int fmt, MrhsArgs &m, cudaStream_t s)
         case LINK_F32_18: return launch_mrhs_fmt<LINK_F32_18>(m, s);
         case LINK_F32_12: return launch_mrhs_fmt<LINK_F32_12>(m, s);
         case LINK_I16_12: return launch_mrhs_fmt<LINK_I16_12>(m, s);
+        case LINK_F32_8: return launch_mrhs_fmt<LINK_F32_8>(m, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -450,6 +457,7 @@ cudaError_t launch_dslash(int fmt, const DslashArgs &a, cudaStream_t s)
         case LINK_F32_18: return launch_fmt<LINK_F32_18>(a, s);
         case LINK_F32_12: return launch_fmt<LINK_F32_12>(a, s);
         case LINK_I16_12: return launch_fmt<LINK_I16_12>(a, s);
+        case LINK_F32_8: return launch_fmt<LINK_F32_8>(a, s);
     }
     return cudaErrorInvalidValue;
 }

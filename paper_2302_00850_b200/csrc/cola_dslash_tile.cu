@@ -259,7 +259,7 @@ template <int FMT>
 cudaError_t launch_tile_fmt(const TileArgs &ta, cudaStream_t s)
 {
     const DslashArgs &a = ta.d;
-    const int xpay = a.y ? (a.clov_y ? 2 : 1) : 0;
+    const int xpay = a.y ? (a.clov_y ? (a.clov_y_g48 ? 3 : 2) : 1) : 0;
     const int post = a.clov_post ? 1 : 0;
     const dim3 grid((unsigned)ta.ntiles), block((unsigned)((ta.nthr + 31) / 32 * 32));
     const size_t smem = (size_t)TILE_STRIDE * 6 * 16;
@@ -268,6 +268,8 @@ cudaError_t launch_tile_fmt(const TileArgs &ta, cudaStream_t s)
     if (xpay == 1 && post == 0) return launch_one<FMT, 1, 0>(ta, grid, block, smem, s);
     if (xpay == 1 && post == 1) return launch_one<FMT, 1, 1>(ta, grid, block, smem, s);
     if (xpay == 2 && post == 0) return launch_one<FMT, 2, 0>(ta, grid, block, smem, s);
+    if constexpr (FMT != LINK_I16_12)
+        if (xpay == 3 && post == 0) return launch_one<FMT, 3, 0>(ta, grid, block, smem, s);
     return cudaErrorInvalidValue;
 }
 
@@ -332,6 +334,7 @@ cudaError_t launch_dslash_tile(int fmt, const DslashArgs &a, cudaStream_t s)
         case LINK_F32_18: return launch_tile_fmt<LINK_F32_18>(ta, s);
         case LINK_F32_12: return launch_tile_fmt<LINK_F32_12>(ta, s);
         case LINK_I16_12: return launch_tile_fmt<LINK_I16_12>(ta, s);
+        case LINK_F32_8: return launch_tile_fmt<LINK_F32_8>(ta, s);
     }
     return cudaErrorNotSupported;
 }

@@ -107,7 +107,8 @@ __device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&
 }
 
 // The epilogues of the fused kernel family on the accumulated hopping term `acc` of output site i:
-//   XPAY 1: acc = y + coef acc;  XPAY 2: acc = A y + coef acc;  POST 1: acc = Cpost acc;  store;  returns |acc|^2 if want_norm.
+//   XPAY 1: acc = y + coef acc;  XPAY 2: acc = A y + coef acc;  XPAY 3: the same with A in its 48-real form;
+//   POST 1: acc = Cpost acc;  store;  returns |acc|^2 if want_norm.
 // STREAM: clover read once per launch (no L1 allocation); !STREAM: shared by the right-hand sides of a block.
 template <int FMT, int XPAY, int POST, bool STREAM>
 __device__ __forceinline__ double dslash_epilogue(const DslashArgs &a, const int i, typename LinkT<FMT>::T (&acc)[24], const void *yin, void *out,
@@ -120,9 +121,10 @@ __device__ __forceinline__ double dslash_epilogue(const DslashArgs &a, const int
         T yv[24];
         load_reals<T, 24, true>(yin, Vh, i, yv);
         const T cf = (T)a.coef;
-        if (XPAY == 2) {
+        if (XPAY == 2 || XPAY == 3) {
             T cy[24];
-            clover_apply<T, STREAM, FMT == LINK_I16_12>(a.clov_y, Vh, i, yv, cy);
+            if constexpr (XPAY == 3) clover_apply_g48<T, STREAM>(a.clov_y, Vh, i, yv, cy);
+            else clover_apply<T, STREAM, FMT == LINK_I16_12>(a.clov_y, Vh, i, yv, cy);
 #pragma unroll
             for (int k = 0; k < 24; k++) acc[k] = cy[k] + cf * acc[k];
         } else {

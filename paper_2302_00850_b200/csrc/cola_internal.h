@@ -43,9 +43,26 @@ struct Geom {
 // Bytes of one link per site in each storage format.
 // LINK_I16_12: rows 1 and 2 as 16-bit fixed point (x 32767), 24 bytes per link = one 16-byte and
 // one 8-byte chunk; it comes with the fp16 clover field (CLOVER_H16_BYTES per site) and fp32 spinors and arithmetic.
-enum LinkFmt { LINK_F64_18 = 0, LINK_F32_18 = 1, LINK_F32_12 = 2, LINK_I16_12 = 3 };
-__host__ __device__ inline size_t link_bytes(int fmt) { return fmt == LINK_F64_18 ? 144 : (fmt == LINK_F32_18 ? 72 : (fmt == LINK_F32_12 ? 48 : 24)); }
+// LINK_F32_8 (COLA_F32_R8): 8 fp32 reals per link = two 16-byte chunks
+//   [Re U01, Im U01, Re U02, Im U02 | Re b1, Im b1, arg(U00)/pi, arg(c1)/pi],
+// (b1, c1) = (U10, U20), or (U20, -U10) when |U10| > |U20| (flag = mantissa LSB of the second angle), so that
+// |c1|^2 = 1 - |U00|^2 - |b1|^2 is formed without cancellation; the rest of rows 2 and 3 follows from unitarity and
+// det U = 1 (reconstruct8 in cola_device.cuh).  |U00| = sqrt(1 - |U01|^2 - |U02|^2) is ill-conditioned for |U00| -> 0 (absolute
+// error ~ eps/(2 |U00|), sqrt(eps) at worst): the upload measures min |U00|^2 and offers the format only if it is >= R8_MIN_U00SQ.
+// Links with U01 = U02 = 0 (block diagonal, e.g. the unit matrix) are
+// not covered by that parametrisation: they are flagged (mantissa LSB of the first angle) and store U11, U12 instead.
+enum LinkFmt { LINK_F64_18 = 0, LINK_F32_18 = 1, LINK_F32_12 = 2, LINK_I16_12 = 3, LINK_F32_8 = 4 };
+__host__ __device__ inline size_t link_bytes(int fmt)
+{
+    return fmt == LINK_F64_18 ? 144 : (fmt == LINK_F32_18 ? 72 : (fmt == LINK_F32_12 ? 48 : (fmt == LINK_F32_8 ? 32 : 24)));
+}
+constexpr double R8_MIN_U00SQ = 0.01;
 constexpr size_t CLOVER_H16_BYTES = 144;   // 2 blocks x (4 x 16 B + 1 x 8 B) = 72 halfs
+// 48-real form of A (SURVEY 8(f) NEXT-2 "rebuilding A from the 48-real field strength in-kernel"): per chiral block the
+// three traceless Hermitian 3x3 matrices G_j = -kappa*csw*B_j of  block = 1 + [[G3, G1 - i G2], [G1 + i G2, -G3]]
+// (B_j: the field-strength combinations in cola_clover.cu), each as [d0, d1, Re l10, Im l10 | Re l20, Im l20, Re l21, Im l21]
+// (d2 = -d0 - d1), order G3, G1, G2: 24 reals per block, [block][chunk][Vh].  Needs trace_sub (traceless F).
+constexpr size_t CLOVER_G48_REALS = 48;
 
 // Device-resident scalars of the CG recurrence (all reductions land here; alpha and beta are
 // formed inside the consuming kernels, so the host only ever reads `rr`).
@@ -151,6 +168,7 @@ struct DslashArgs {
     const void *gauge_q;    // links of parity 1-p
     const void *y;          // parity p half spinor or nullptr
     const void *clov_y;     // packed clover of parity p or nullptr
+    int clov_y_g48;         // clov_y is the 48-real field-strength form (CLOVER_G48_REALS), expanded in the kernel
     const void *clov_post;  // packed clover applied to the result or nullptr
     double coef;
     double sgn;             // -1: D (forward hop projects with 1 - gamma_mu); +1: gamma_5 D gamma_5
@@ -227,12 +245,14 @@ cudaError_t launch_clover_apply(cola_prec prec, const Geom &g, const void *clov,
 
 // layout / setup kernels (cola_layout.cu, cola_clover.cu)
 cudaError_t launch_gauge_reorder(const Geom &g, const double *canon_dev, long site_lo, long n_sites, void *gauge64, void *gauge32,
-                                 int fmt32, void *gauge16, unsigned long long *max_dev_bits, cudaStream_t s);
+                                 int fmt32, void *gauge16, void *gauge8, unsigned long long *max_dev_bits, unsigned long long *min_u00_bits, cudaStream_t s);
 cudaError_t launch_spinor_pack(cola_prec prec, const Geom &g, const void *canon, void *internal, cudaStream_t s);
 cudaError_t launch_spinor_unpack(cola_prec prec, const Geom &g, const void *internal, void *canon, cudaStream_t s);
 cudaError_t launch_spinor_convert(cola_prec dst_prec, const void *src, void *dst, size_t n_sites, cudaStream_t s);
 // a32_parities: 2 = fp32 copy of A on both parities, 1 = even parity only (no COLA_FEAT_FULL_M)
-cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, int a32_parities, void *clovA16, cudaStream_t s);
+// clovG32: 48-real fp32 form of A on a32_parities parities, or nullptr
+cudaError_t launch_clover_build(const Geom &g, const void *gauge64, double kappa_csw, int trace_sub, void *clovA64, void *clovA32, int a32_parities, void *clovA16,
+                                void *clovG32, cudaStream_t s);
 // *min_pivot_key (device, initialised to ~0ull) receives the order-preserving key of the smallest Gauss-Jordan pivot: decode with pivot_from_key
 cudaError_t launch_clover_invert(const Geom &g, const void *clovA64_odd, void *clovI64, void *clovI32, void *clovI16, unsigned long long *min_pivot_key, cudaStream_t s);
 inline double pivot_from_key(unsigned long long k)

@@ -22,10 +22,11 @@ __device__ __forceinline__ void lex_to_cb(const Geom &g, long lex, int &parity, 
 
 // one thread per (lex site, mu) of the staged canonical chunk
 __global__ void __launch_bounds__(LB) gauge_reorder_kernel(Geom g, const double *canon, long site_lo, long n_sites, char *gauge64,
-                                                           char *gauge32, int fmt32, char *gauge16, unsigned long long *max_dev_bits)
+                                                           char *gauge32, int fmt32, char *gauge16, char *gauge8, unsigned long long *max_dev_bits,
+                                                           unsigned long long *min_u00_bits)
 {
     const long tid = (long)blockIdx.x * LB + threadIdx.x;
-    double dev = 0.0;
+    double dev = 0.0, u00 = 2.0;
     if (tid < 4 * n_sites) {
         const long ls = tid >> 2;
         const int mu = (int)(tid & 3);
@@ -62,6 +63,29 @@ __global__ void __launch_bounds__(LB) gauge_reorder_kernel(Geom g, const double 
             reinterpret_cast<uint4 *>(b16)[cb] = make_uint4(w[0], w[1], w[2], w[3]);
             reinterpret_cast<uint2 *>(b16 + 16 * Vh)[cb] = make_uint2(w[4], w[5]);
         }
+        u00 = u[0] * u[0] + u[1] * u[1];
+        if (gauge8) {   // LINK_F32_8 (cola_internal.h): [a2, a3 | b1, arg(a1)/pi, arg(c1)/pi] with the two flags in the angles' mantissa LSBs
+            const double N = u[2] * u[2] + u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
+            const bool blockdiag = N < 1e-16;    // |U01|, |U02| < 1e-8: below fp32 resolution of an O(1) entry
+            const bool swapped = !blockdiag && (u[6] * u[6] + u[7] * u[7] > u[12] * u[12] + u[13] * u[13]);   // |U10| > |U20|: store (U20, -U10)
+            float f[8];
+            const double inv_pi = 0.31830988618379067154;
+            if (blockdiag) {
+                f[0] = (float)u[8]; f[1] = (float)u[9]; f[2] = (float)u[10]; f[3] = (float)u[11];   // U11, U12
+                f[4] = 0.0f; f[5] = 0.0f;
+                f[7] = 0.0f;
+            } else {
+                f[0] = (float)u[2]; f[1] = (float)u[3]; f[2] = (float)u[4]; f[3] = (float)u[5];
+                const double b1r = swapped ? u[12] : u[6], b1i = swapped ? u[13] : u[7];
+                const double c1r = swapped ? -u[6] : u[12], c1i = swapped ? -u[7] : u[13];
+                f[4] = (float)b1r; f[5] = (float)b1i;
+                f[7] = (float)(atan2(c1i, c1r) * inv_pi);
+            }
+            f[6] = (float)(atan2(u[1], u[0]) * inv_pi);
+            f[6] = __uint_as_float((__float_as_uint(f[6]) & ~1u) | (blockdiag ? 1u : 0u));
+            f[7] = __uint_as_float((__float_as_uint(f[7]) & ~1u) | (swapped ? 1u : 0u));
+            store_reals<float, 8>(gauge8 + (size_t)(parity * 4 + mu) * link_bytes(LINK_F32_8) * Vh, Vh, cb, f);
+        }
         // max |U U^+ - 1| (entry-wise)
 #pragma unroll
         for (int a = 0; a < 3; a++)
@@ -81,6 +105,11 @@ __global__ void __launch_bounds__(LB) gauge_reorder_kernel(Geom g, const double 
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dev = fmax(dev, __shfl_xor_sync(0xffffffffu, dev, o));
     if ((threadIdx.x & 31) == 0 && dev > 0.0) atomicMax(max_dev_bits, (unsigned long long)__double_as_longlong(dev));
+    if (min_u00_bits) {   // min |U00|^2 over all links (non-negative doubles order like their bit patterns): see LINK_F32_8
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) u00 = fmin(u00, __shfl_xor_sync(0xffffffffu, u00, o));
+        if ((threadIdx.x & 31) == 0) atomicMin(min_u00_bits, (unsigned long long)__double_as_longlong(u00));
+    }
 }
 
 template <typename T, bool PACK>
@@ -126,11 +155,11 @@ __global__ void __launch_bounds__(LB) convert_kernel(const void *src, void *dst,
 }  // namespace
 
 cudaError_t launch_gauge_reorder(const Geom &g, const double *canon_dev, long site_lo, long n_sites, void *gauge64, void *gauge32,
-                                 int fmt32, void *gauge16, unsigned long long *max_dev_bits, cudaStream_t s)
+                                 int fmt32, void *gauge16, void *gauge8, unsigned long long *max_dev_bits, unsigned long long *min_u00_bits, cudaStream_t s)
 {
     const long n = 4 * n_sites;
     gauge_reorder_kernel<<<(unsigned)((n + LB - 1) / LB), LB, 0, s>>>(g, canon_dev, site_lo, n_sites, (char *)gauge64, (char *)gauge32,
-                                                                     fmt32, (char *)gauge16, max_dev_bits);
+                                                                     fmt32, (char *)gauge16, (char *)gauge8, max_dev_bits, min_u00_bits);
     return cudaGetLastError();
 }
 

@@ -146,8 +146,8 @@ def test_bad_precision_and_mode_are_rejected(binding):
     c.gauge_upload(inputs.links_haar(dims, 1))
     v = c.empty_internal(torch.float32, full=False).normal_()
     out = torch.empty_like(v)
-    assert b._lib.cola_dslash_apply(c._h, 3, 0, v.data_ptr(), out.data_ptr()) == b.COLA_EINVAL
+    assert b._lib.cola_dslash_apply(c._h, 4, 0, v.data_ptr(), out.data_ptr()) == b.COLA_EINVAL
     with pytest.raises(b.ColaError) as e:
-        c.cg_solve(inputs.source_gaussian(dims, 2).cuda(), mixed=3)
+        c.cg_solve(inputs.source_gaussian(dims, 2).cuda(), mixed=4)
     assert e.value.status == b.COLA_EINVAL
     c.close()
