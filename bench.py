@@ -191,7 +191,7 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
             out[f"{name}_{fmt}"] = {"ms": round(ms, 5), "launches": launches, "GB/s": round(gbs, 1), "GFLOP/s": round(flops / (ms * 1e-3) / 1e9, 1),
                                     "frac_measured": round(gbs / peak, 4), "frac_nominal_8TBs": round(gbs / NOMINAL_HBM_GBS, 4)}
         del full, dst
-        if nrhs > 1 and of is None:
+        if nrhs > 1 and fmt in ("f32x12", "f32x18", "f64x18"):
             ctx.set_mrhs_workspace(nrhs)
             vin = ctx.empty_internal_mrhs(nrhs, prec, full=False).normal_()
             vout = torch.empty_like(vin)
@@ -199,7 +199,8 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
             w = 4 if prec == torch.float32 else 8
             G = {"f32x12": 12, "f32x18": 18, "f64x18": 18}[fmt]
             # per site and vector: links and clover of both kernels shared by nrhs vectors + 5 spinor passes
-            nbytes = ((2 * 8 * G + 2 * 72) * w / nrhs + 5 * 24 * w) * Vh * nrhs
+            clov = 72 + (48 if prec == torch.float32 else 72)   # A^-1 (72 reals) + A (fp32: its 48-real form)
+            nbytes = ((2 * 8 * G + clov) * w / nrhs + 5 * 24 * w) * Vh * nrhs
             flops = (FLOPS["dslash_clover_inv"] + FLOPS["dslash_clover_xpay"]) * Vh * nrhs
             single = out[f"schur_{fmt}"]["ms"]
             out[f"schur_mrhs{nrhs}_{fmt}"] = {"ms": round(ms, 5), "launches": 2, "ms_per_rhs": round(ms / nrhs, 5), "speedup_vs_single": round(single / (ms / nrhs), 3),

@@ -332,34 +332,41 @@ __device__ __forceinline__ void clover_block_mul(const T *c, const T *v, T *w)
     }
 }
 
-// w = C(site i) v on the full 24-real spinor; clov = [72/N chunks][Vh]
+// The 36 packed reals of chiral block b of the clover field at site i; clov = [72/N chunks][Vh]
 // H16: the field is stored in fp16, per block 4 chunks of 8 halfs + 1 chunk of 4 halfs (72 bytes), [block][chunk][Vh]
-template <typename T, bool STREAM = true, bool H16 = false>
-__device__ __forceinline__ void clover_apply(const void *clov, size_t Vh, size_t i, const T (&v)[24], T (&w)[24])
+template <typename T, bool STREAM, bool H16>
+__device__ __forceinline__ void load_clover_block(const void *clov, size_t Vh, size_t i, int b, T (&c)[36])
 {
     typedef typename VT<T>::V V;
     constexpr int N = VT<T>::N;
+    if constexpr (H16) {
+        const char *base = reinterpret_cast<const char *>(clov) + (size_t)b * 72 * Vh;
+#pragma unroll
+        for (int k = 0; k < 4; k++) {
+            const uint4 *p = reinterpret_cast<const uint4 *>(base + (size_t)k * 16 * Vh) + i;
+            const uint4 q = STREAM ? ld_stream(p) : __ldg(p);
+            unpack_h16(q.x, c[8 * k], c[8 * k + 1]);
+            unpack_h16(q.y, c[8 * k + 2], c[8 * k + 3]);
+            unpack_h16(q.z, c[8 * k + 4], c[8 * k + 5]);
+            unpack_h16(q.w, c[8 * k + 6], c[8 * k + 7]);
+        }
+        const uint2 *p2 = reinterpret_cast<const uint2 *>(base + (size_t)64 * Vh) + i;
+        const uint2 q2 = STREAM ? ld_stream(p2) : __ldg(p2);
+        unpack_h16(q2.x, c[32], c[33]);
+        unpack_h16(q2.y, c[34], c[35]);
+    } else {
+        load_reals<T, 36, STREAM>(reinterpret_cast<const V *>(clov) + (size_t)b * (36 / N) * Vh, Vh, i, c);
+    }
+}
+
+// w = C(site i) v on the full 24-real spinor
+template <typename T, bool STREAM = true, bool H16 = false>
+__device__ __forceinline__ void clover_apply(const void *clov, size_t Vh, size_t i, const T (&v)[24], T (&w)[24])
+{
 #pragma unroll
     for (int b = 0; b < 2; b++) {
         T c[36];
-        if constexpr (H16) {
-            const char *base = reinterpret_cast<const char *>(clov) + (size_t)b * 72 * Vh;
-#pragma unroll
-            for (int k = 0; k < 4; k++) {
-                const uint4 *p = reinterpret_cast<const uint4 *>(base + (size_t)k * 16 * Vh) + i;
-                const uint4 q = STREAM ? ld_stream(p) : __ldg(p);
-                unpack_h16(q.x, c[8 * k], c[8 * k + 1]);
-                unpack_h16(q.y, c[8 * k + 2], c[8 * k + 3]);
-                unpack_h16(q.z, c[8 * k + 4], c[8 * k + 5]);
-                unpack_h16(q.w, c[8 * k + 6], c[8 * k + 7]);
-            }
-            const uint2 *p2 = reinterpret_cast<const uint2 *>(base + (size_t)64 * Vh) + i;
-            const uint2 q2 = STREAM ? ld_stream(p2) : __ldg(p2);
-            unpack_h16(q2.x, c[32], c[33]);
-            unpack_h16(q2.y, c[34], c[35]);
-        } else {
-            load_reals<T, 36, STREAM>(reinterpret_cast<const V *>(clov) + (size_t)b * (36 / N) * Vh, Vh, i, c);
-        }
+        load_clover_block<T, STREAM, H16>(clov, Vh, i, b, c);
         clover_block_mul(c, &v[12 * b], &w[12 * b]);
     }
 }

@@ -178,6 +178,145 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
     return nrm;
 }
 
+// ---- R right-hand sides per thread (register blocking): the thread of output site i applies each
+// link, loaded, converted and completed ONCE, to the spin-projected neighbours of R vectors, and each clover block, loaded
+// once, to R spinors.  Per vector the arithmetic is the same sequence of calls as in dslash_site (results bit-identical,
+// tested); what is shared is everything that does not depend on the vector: index arithmetic, boundary signs, 8 link
+// loads + reconstructions, 2-4 clover block loads + conversions.  in/yin/out: the R vectors' arrays (entries past
+// `nvalid` alias a valid vector: computed, not stored).
+// Pipelining: one spinor buffer per vector, refilled with the next hop's neighbour right after the projection that
+// consumed it; two raw-link buffers alternate between hops, refilled two hops ahead.
+template <int FMT, int H, int R, bool STREAM, typename T>
+__device__ __forceinline__ void hop_r(const char *const (&in)[R], const char *gauge_next2, size_t Vh, int nb_next, int li_next2, T (&psi)[R][24],
+                                      RawLink<FMT> &raw, T eta, T s, T (&acc)[R][24])
+{
+    constexpr int MU = H >> 1;
+    constexpr bool BACK = (H & 1) != 0;
+    T u[18];
+    expand_link<FMT>(raw, u);
+    if (H < 6) load_raw_link<FMT, STREAM>(gauge_next2, Vh, li_next2, raw);   // the link of hop H + 2
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+        T h[12], g[12];
+        project<MU>(psi[r], s, h);
+        if (H < 7) load_reals<T, 24, false>(in[r], Vh, nb_next, psi[r]);   // vector r's neighbour of hop H + 1
+        su3_mul<BACK>(u, h, g);
+        reconstruct_accumulate<MU>(g, eta, s, acc[r]);
+    }
+}
+
+template <int FMT, int XPAY, int POST, int R, bool STREAM>
+__device__ __forceinline__ void dslash_site_r(const DslashArgs &a, const int i, const char *const (&in)[R], const char *const (&yin)[R], char *const (&out)[R],
+                                              const int nvalid, const bool want_norm, double (&nrm)[R])
+{
+    typedef typename LinkT<FMT>::T T;
+    typedef typename VT<T>::V V;
+    constexpr int N = VT<T>::N;
+    const Geom &g = a.g;
+    const size_t Vh = g.Vh;
+    const unsigned r1 = g.dXh.div((unsigned)i), r2 = g.dY.div(r1), r3 = g.dZ.div(r2);
+    const int xh = i - (int)r1 * g.Xh, y = (int)r1 - (int)r2 * g.Y, z = (int)r2 - (int)r3 * g.Z, t = (int)r3;
+    const int odd = (y + z + t + a.parity) & 1;
+    const int sY = g.Xh, sZ = g.Xh * g.Y, sT = g.Xh * g.Y * g.Z;
+    const int xf = odd ? (xh + 1 == g.Xh ? i - xh : i + 1) : i;
+    const int xb = odd ? i : (xh == 0 ? i + g.Xh - 1 : i - 1);
+    const bool cxf = odd && (xh + 1 == g.Xh), cxb = !odd && (xh == 0);
+    const int yf = (y + 1 == g.Y) ? i - (g.Y - 1) * sY : i + sY;
+    const int yb = (y == 0) ? i + (g.Y - 1) * sY : i - sY;
+    const int zf = (z + 1 == g.Z) ? i - (g.Z - 1) * sZ : i + sZ;
+    const int zb = (z == 0) ? i + (g.Z - 1) * sZ : i - sZ;
+    const int tf = (t + 1 == g.T) ? i - (g.T - 1) * sT : i + sT;
+    const int tb = (t == 0) ? i + (g.T - 1) * sT : i - sT;
+    const T one = 1;
+    const T ex_f = (cxf && g.bc[0] < 0) ? -one : one, ex_b = (cxb && g.bc[0] < 0) ? -one : one;
+    const T ey_f = (y + 1 == g.Y && g.bc[1] < 0) ? -one : one, ey_b = (y == 0 && g.bc[1] < 0) ? -one : one;
+    const T ez_f = (z + 1 == g.Z && g.bc[2] < 0) ? -one : one, ez_b = (z == 0 && g.bc[2] < 0) ? -one : one;
+    const T et_f = (t + 1 == g.T && g.bc[3] < 0) ? -one : one, et_b = (t == 0 && g.bc[3] < 0) ? -one : one;
+    const T sf = (T)a.sgn, sb = -(T)a.sgn;
+    const size_t lb = link_bytes(FMT) * Vh;
+    const char *gp = reinterpret_cast<const char *>(a.gauge_p);
+    const char *gq = reinterpret_cast<const char *>(a.gauge_q);
+
+    T acc[R][24], psi[R][24];
+#pragma unroll
+    for (int r = 0; r < R; r++)
+#pragma unroll
+        for (int k = 0; k < 24; k++) acc[r][k] = 0;
+    RawLink<FMT> rawA, rawB;
+    load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, rawA);
+#pragma unroll
+    for (int r = 0; r < R; r++) load_reals<T, 24, false>(in[r], Vh, xf, psi[r]);
+    load_raw_link<FMT, STREAM>(gq + 0 * lb, Vh, xb, rawB);
+    hop_r<FMT, 0, R, STREAM>(in, gp + 1 * lb, Vh, xb, i, psi, rawA, ex_f, sf, acc);
+    hop_r<FMT, 1, R, STREAM>(in, gq + 1 * lb, Vh, yf, yb, psi, rawB, ex_b, sb, acc);
+    hop_r<FMT, 2, R, STREAM>(in, gp + 2 * lb, Vh, yb, i, psi, rawA, ey_f, sf, acc);
+    hop_r<FMT, 3, R, STREAM>(in, gq + 2 * lb, Vh, zf, zb, psi, rawB, ey_b, sb, acc);
+    hop_r<FMT, 4, R, STREAM>(in, gp + 3 * lb, Vh, zb, i, psi, rawA, ez_f, sf, acc);
+    hop_r<FMT, 5, R, STREAM>(in, gq + 3 * lb, Vh, tf, tb, psi, rawB, ez_b, sb, acc);
+    hop_r<FMT, 6, R, STREAM>(in, nullptr, Vh, tb, 0, psi, rawA, et_f, sf, acc);
+    hop_r<FMT, 7, R, STREAM>(in, nullptr, Vh, 0, 0, psi, rawB, et_b, sb, acc);
+
+    // epilogues (dslash_epilogue in cola_hop.cuh, per chiral block so that a clover block is loaded once for the R vectors)
+    if (XPAY != 0) {
+        const T cf = (T)a.coef;
+#pragma unroll
+        for (int b = 0; b < 2; b++) {
+            T c[36];
+            if constexpr (XPAY == 3) load_clover_g48<T, STREAM>(a.clov_y, Vh, i, b, c);
+            else if constexpr (XPAY == 2) load_clover_block<T, STREAM, FMT == LINK_I16_12>(a.clov_y, Vh, i, b, c);
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                T yv[12];
+                load_reals<T, 12, true>(reinterpret_cast<const V *>(yin[r]) + (size_t)b * (12 / N) * Vh, Vh, i, yv);
+                if constexpr (XPAY == 1) {
+#pragma unroll
+                    for (int k = 0; k < 12; k++) acc[r][12 * b + k] = yv[k] + cf * acc[r][12 * b + k];
+                } else {
+                    T cy[12];
+                    clover_block_mul(c, yv, cy);
+#pragma unroll
+                    for (int k = 0; k < 12; k++) acc[r][12 * b + k] = cy[k] + cf * acc[r][12 * b + k];
+                }
+            }
+        }
+    }
+    if (POST != 0) {
+#pragma unroll
+        for (int b = 0; b < 2; b++) {
+            T c[36];
+            load_clover_block<T, STREAM, FMT == LINK_I16_12>(a.clov_post, Vh, i, b, c);
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                T w[12];
+                clover_block_mul(c, &acc[r][12 * b], w);
+#pragma unroll
+                for (int k = 0; k < 12; k++) acc[r][12 * b + k] = w[k];
+            }
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+        if (r < nvalid) store_reals<T, 24>(out[r], Vh, i, acc[r]);
+        nrm[r] = 0.0;
+        if (want_norm) {
+            T s2 = 0;
+#pragma unroll
+            for (int k = 0; k < 24; k++) s2 += acc[r][k] * acc[r][k];
+            nrm[r] = (double)s2;
+        }
+    }
+}
+
+// Sweep position -> run of DSLASH_BLOCK consecutive sites (identity, or the z-banded order of Sweep in cola_internal.h)
+__device__ __forceinline__ unsigned sweep_run(const Sweep &w, const Geom &g, unsigned pos)
+{
+    if (!w.on) return pos;
+    const unsigned q1 = w.d_up.div(pos), u = pos - q1 * w.d_up.d;
+    const unsigned q2 = w.d_zb.div(q1), zi = q1 - q2 * w.d_zb.d;
+    const unsigned band = w.d_t.div(q2), t = q2 - band * w.d_t.d;
+    return ((t * (unsigned)g.Z + band * w.d_zb.d + zi) * w.d_up.d) + u;
+}
+
 template <int FMT, int XPAY, int POST>
 __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
 {
@@ -187,13 +326,9 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
         pdl_wait();
         if (a.skip && *a.skip) return;
     }
-    unsigned run = blockIdx.x;   // which run of DSLASH_BLOCK consecutive sites this block covers
-    if (a.sweep.on) {            // z-banded sweep (Sweep in cola_internal.h): block order = [unit in plane, z in band, t, band]
-        const unsigned q1 = a.sweep.d_up.div(run), u = run - q1 * a.sweep.d_up.d;
-        const unsigned q2 = a.sweep.d_zb.div(q1), zi = q1 - q2 * a.sweep.d_zb.d;
-        const unsigned band = a.sweep.d_t.div(q2), t = q2 - band * a.sweep.d_t.d;
-        run = ((t * (unsigned)a.g.Z + band * a.sweep.d_zb.d + zi) * a.sweep.d_up.d) + u;
-    }
+    // which run of DSLASH_BLOCK consecutive sites this block covers: linear, or the z-banded sweep (block order =
+    // [unit in plane, z in band, t, band])
+    const unsigned run = sweep_run(a.sweep, a.g, blockIdx.x);
     const int i = (int)run * DSLASH_BLOCK + (int)threadIdx.x;
     const bool want_norm = a.red.partials != nullptr;
     double nrm = 0.0;
@@ -214,8 +349,11 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
 #ifndef COLA_MRHS_PER_BLOCK_F64
 #define COLA_MRHS_PER_BLOCK_F64 2
 #endif
-#ifndef COLA_MRHS_MINB_F32
-#define COLA_MRHS_MINB_F32 4
+#ifndef COLA_MRHS_R
+#define COLA_MRHS_R 2     // right-hand sides per thread of the fp32 / 16-bit multi-rhs kernels (dslash_site_r); fp64: 1
+#endif
+#ifndef COLA_MRHS_MINB_F32   // register budget: 128 (R = 1), 168 (R = 2), 255 (R >= 3) at 128 threads per block
+#define COLA_MRHS_MINB_F32 (COLA_MRHS_R == 1 ? 4 : (COLA_MRHS_R == 2 ? 3 : 2))
 #endif
 #ifndef COLA_MRHS_MINB_F64
 #define COLA_MRHS_MINB_F64 3
@@ -228,19 +366,20 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
 #endif
 constexpr int MSITES = COLA_MRHS_SITES;
 template <int FMT> struct MrhsCfg {
-    static constexpr int NRB = (FMT == LINK_F64_18) ? COLA_MRHS_PER_BLOCK_F64 : COLA_MRHS_PER_BLOCK_F32;
+    static constexpr int NRB = (FMT == LINK_F64_18) ? COLA_MRHS_PER_BLOCK_F64 : COLA_MRHS_PER_BLOCK_F32;   // rows of threads (threadIdx.y)
     static constexpr int MINB = (FMT == LINK_F64_18) ? COLA_MRHS_MINB_F64 : COLA_MRHS_MINB_F32;
+    static constexpr int R = (FMT == LINK_F64_18) ? 1 : COLA_MRHS_R;                                       // vectors per thread
 };
 
 template <int FMT, int XPAY, int POST>
 __global__ void __launch_bounds__(MSITES * MrhsCfg<FMT>::NRB, MrhsCfg<FMT>::MINB) dslash_mrhs_kernel(const __grid_constant__ MrhsArgs m)
 {
-    constexpr int NRB = MrhsCfg<FMT>::NRB;
+    constexpr int NRB = MrhsCfg<FMT>::NRB, R = MrhsCfg<FMT>::R;
     if (m.d.skip && *m.d.skip) return;
     const Geom &g = m.d.g;
     const Tile &tl = m.tile;
     const unsigned sb = blockIdx.x / (unsigned)m.ngroups, grp = blockIdx.x - sb * (unsigned)m.ngroups;
-    const int k = (int)grp * NRB + (int)threadIdx.y;
+    const int k0 = ((int)grp * NRB + (int)threadIdx.y) * R;   // first vector of this thread
     // site of this thread: tile origin (block-uniform) + position inside the tile
     const unsigned b1 = tl.nb[0].div(sb), b2 = tl.nb[1].div(b1);
     unsigned bz, bt;
@@ -261,23 +400,46 @@ __global__ void __launch_bounds__(MSITES * MrhsCfg<FMT>::NRB, MrhsCfg<FMT>::MINB
     const int t = (int)(bt << tl.sh[3]) + (int)(l >> (s0 + s1 + s2));
     const int i = xh + g.Xh * (y + g.Y * (z + g.Z * t));
     const bool want_norm = m.partials != nullptr;
-    const bool live = k < m.nrhs && (int)l < tl.vol;
-    const size_t vec = k < m.nrhs ? (size_t)m.list[k] : 0;
-    double nrm = 0.0;
-    if (live)
-        nrm = dslash_site<FMT, XPAY, POST, false>(m.d, i, reinterpret_cast<const char *>(m.d.in) + vec * m.in_stride,
-                                                  reinterpret_cast<const char *>(m.d.y) + vec * m.y_stride,
-                                                  reinterpret_cast<char *>(m.d.out) + vec * m.out_stride, want_norm);
-    if (want_norm) {   // one partial per (vector, site block): the warps of a row (threadIdx.y) hold one right-hand side
-        __shared__ double sm[NRB][MSITES / 32];
-        const double w = warp_sum(nrm);
-        if ((threadIdx.x & 31) == 0) sm[threadIdx.y][threadIdx.x >> 5] = w;
+    const bool live = k0 < m.nrhs && (int)l < tl.vol;
+    double nrm[R];
+    size_t vec[R];
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+        nrm[r] = 0.0;
+        const int kr = k0 + r < m.nrhs ? k0 + r : m.nrhs - 1;   // past the end: alias the last vector (computed, not stored)
+        vec[r] = (size_t)m.list[kr];
+    }
+    if (live) {
+        if constexpr (R == 1) {
+            nrm[0] = dslash_site<FMT, XPAY, POST, false>(m.d, i, reinterpret_cast<const char *>(m.d.in) + vec[0] * m.in_stride,
+                                                         reinterpret_cast<const char *>(m.d.y) + vec[0] * m.y_stride,
+                                                         reinterpret_cast<char *>(m.d.out) + vec[0] * m.out_stride, want_norm);
+        } else {
+            const char *in[R], *yin[R];
+            char *out[R];
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                in[r] = reinterpret_cast<const char *>(m.d.in) + vec[r] * m.in_stride;
+                yin[r] = reinterpret_cast<const char *>(m.d.y) + vec[r] * m.y_stride;
+                out[r] = reinterpret_cast<char *>(m.d.out) + vec[r] * m.out_stride;
+            }
+            const int nvalid = m.nrhs - k0 < R ? m.nrhs - k0 : R;
+            dslash_site_r<FMT, XPAY, POST, R, NRB == 1>(m.d, i, in, yin, out, nvalid, want_norm, nrm);   // one row of threads: links and clover are read once
+        }
+    }
+    if (want_norm) {   // one partial per (vector, site block): the warps of a row (threadIdx.y) hold R right-hand sides
+        __shared__ double sm[NRB][R][MSITES / 32];
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            const double w = warp_sum(nrm[r]);
+            if ((threadIdx.x & 31) == 0) sm[threadIdx.y][r][threadIdx.x >> 5] = w;
+        }
         __syncthreads();
-        if (threadIdx.x == 0 && k < m.nrhs) {
+        if (threadIdx.x < R && k0 + (int)threadIdx.x < m.nrhs) {
             double tsum = 0.0;
 #pragma unroll
-            for (int q = 0; q < MSITES / 32; q++) tsum += sm[threadIdx.y][q];
-            m.partials[vec * (size_t)m.nsb + sb] = tsum;
+            for (int q = 0; q < MSITES / 32; q++) tsum += sm[threadIdx.y][threadIdx.x][q];
+            m.partials[(size_t)m.list[k0 + threadIdx.x] * (size_t)m.nsb + sb] = tsum;
         }
     }
 }
@@ -327,7 +489,7 @@ cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
 template <int FMT>
 cudaError_t launch_mrhs_fmt(MrhsArgs &m, cudaStream_t s)
 {
-    constexpr int NRB = MrhsCfg<FMT>::NRB;
+    constexpr int NRB = MrhsCfg<FMT>::NRB * MrhsCfg<FMT>::R;   // vectors per block
     const int xpay = m.d.y ? (m.d.clov_y ? (m.d.clov_y_g48 ? 3 : 2) : 1) : 0;
     const int post = m.d.clov_post ? 1 : 0;
     m.tile = make_tile(m.d.g, MSITES, COLA_MRHS_TILE_X);
@@ -344,7 +506,7 @@ cudaError_t launch_mrhs_fmt(MrhsArgs &m, cudaStream_t s)
             m.tsweep.d_t = make_fastdiv((unsigned)nbt);
         }
     }
-    const dim3 grid((unsigned)m.nsb * (unsigned)m.ngroups), block(MSITES, NRB);
+    const dim3 grid((unsigned)m.nsb * (unsigned)m.ngroups), block(MSITES, MrhsCfg<FMT>::NRB);
     if (xpay == 0 && post == 0) dslash_mrhs_kernel<FMT, 0, 0><<<grid, block, 0, s>>>(m);
     else if (xpay == 0 && post == 1) dslash_mrhs_kernel<FMT, 0, 1><<<grid, block, 0, s>>>(m);
     else if (xpay == 1 && post == 0) dslash_mrhs_kernel<FMT, 1, 0><<<grid, block, 0, s>>>(m);
