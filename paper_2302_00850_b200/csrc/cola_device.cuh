@@ -54,6 +54,16 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, cud
     return launch_pdl_smem(kern, grid, block, 0, s, args...);
 }
 
+// Asynchronous 16-byte copy global -> shared (LDGSTS): the data in flight needs no destination register.  A thread that
+// only reads back what it copied itself needs no barrier: cp_async_wait<N>() returns when all but the N most recently
+// committed groups of THIS thread have landed.
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 template <typename T> struct VT;
 template <> struct VT<float> {
     typedef float4 V;

@@ -69,6 +69,44 @@ __device__ __forceinline__ void hop_pipe(const void *in, const char *gauge_next,
     reconstruct_accumulate<MU>(g, eta, s, acc);
 }
 
+// COLA_PIPE == 3: the neighbour spinors of the coming hops are fetched with asynchronous copies into a per-thread FIFO in
+// shared memory ([slot][chunk][thread]: conflict-free, no barrier: a thread reads back only what it copied itself),
+// FIFO_DEPTH hops ahead, instead of into registers one or two hops ahead; the raw links stay register-pipelined two hops
+// ahead.  Loads in flight then cost shared memory, not registers.
+#ifndef COLA_FIFO_DEPTH
+#define COLA_FIFO_DEPTH 4
+#endif
+constexpr int FIFO_DEPTH = COLA_FIFO_DEPTH;
+__device__ __forceinline__ void fifo_issue(float4 *fifo, const int slot, const void *in, const size_t Vh, const int nb)
+{
+    const float4 *src = reinterpret_cast<const float4 *>(in) + nb;
+#pragma unroll
+    for (int k = 0; k < 6; k++) cp_async16(&fifo[(slot * 6 + k) * DSLASH_BLOCK + threadIdx.x], src + (size_t)k * Vh);
+    cp_async_commit();
+}
+template <int FMT, int H, bool STREAM, typename T>
+__device__ __forceinline__ void hop_fifo(float4 *fifo, const void *in, const int nb_refill, const char *gauge_next2, size_t Vh, int li_next2, RawLink<FMT> &raw,
+                                         T eta, T s, T (&acc)[24])
+{
+    constexpr int MU = H >> 1;
+    constexpr bool BACK = (H & 1) != 0;
+    constexpr int issued = (H + FIFO_DEPTH < 8) ? H + FIFO_DEPTH : 8;   // groups committed before this hop's wait
+    T psi[24], h[12], g[12], u[18];
+    cp_async_wait<issued - 1 - H>();
+    constexpr int slot = H % FIFO_DEPTH;
+#pragma unroll
+    for (int k = 0; k < 6; k++) {
+        const float4 v = fifo[(slot * 6 + k) * DSLASH_BLOCK + threadIdx.x];
+        psi[4 * k] = v.x; psi[4 * k + 1] = v.y; psi[4 * k + 2] = v.z; psi[4 * k + 3] = v.w;
+    }
+    project<MU>(psi, s, h);
+    if (H + FIFO_DEPTH < 8) fifo_issue(fifo, slot, in, Vh, nb_refill);   // hop H + FIFO_DEPTH takes the slot just read
+    expand_link<FMT>(raw, u);
+    if (H < 6) load_raw_link<FMT, STREAM>(gauge_next2, Vh, li_next2, raw);
+    su3_mul<BACK>(u, h, g);
+    reconstruct_accumulate<MU>(g, eta, s, acc);
+}
+
 // One output site i of parity a.parity:  v = D in;  v = [A] y + coef v (XPAY);  v = Cpost v (POST);  out = v.
 // Returns |v|^2 if want_norm.  XPAY: 0 none, 1 v = y + coef v, 2 v = A y + coef v.   POST: 0 none, 1 v = Cpost v.
 // STREAM: links and clover are read once (no L1 allocation); !STREAM: they are shared by the right-hand sides of a block.
@@ -121,7 +159,31 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
             // software-pipelined hops: the loads of hop h+1 (neighbour spinor and raw link) are issued right after the
             // projection of hop h, whose spinor registers are dead by then, so they are in flight during the SU(3)
             // multiply and the accumulation of hop h
-#if COLA_PIPE == 2
+#if COLA_PIPE == 3
+            if constexpr (STREAM) {
+                extern __shared__ float4 cola_fifo[];
+                const int nbs[8] = {xf, xb, yf, yb, zf, zb, tf, tb};
+                RawLink<FMT> rawA, rawB;
+                load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, rawA);
+                load_raw_link<FMT, STREAM>(gq + 0 * lb, Vh, xb, rawB);
+                if (PDLW) {
+                    pdl_wait();
+                    if (a.skip && *a.skip) return -1.0;
+                }
+#pragma unroll
+                for (int h = 0; h < FIFO_DEPTH; h++) fifo_issue(cola_fifo, h, in, Vh, nbs[h]);
+                hop_fifo<FMT, 0, STREAM>(cola_fifo, in, nbs[(0 + FIFO_DEPTH) & 7], gp + 1 * lb, Vh, i, rawA, ex_f, sf, acc);
+                hop_fifo<FMT, 1, STREAM>(cola_fifo, in, nbs[(1 + FIFO_DEPTH) & 7], gq + 1 * lb, Vh, yb, rawB, ex_b, sb, acc);
+                hop_fifo<FMT, 2, STREAM>(cola_fifo, in, nbs[(2 + FIFO_DEPTH) & 7], gp + 2 * lb, Vh, i, rawA, ey_f, sf, acc);
+                hop_fifo<FMT, 3, STREAM>(cola_fifo, in, nbs[(3 + FIFO_DEPTH) & 7], gq + 2 * lb, Vh, zb, rawB, ey_b, sb, acc);
+                hop_fifo<FMT, 4, STREAM>(cola_fifo, in, nbs[(4 + FIFO_DEPTH) & 7], gp + 3 * lb, Vh, i, rawA, ez_f, sf, acc);
+                hop_fifo<FMT, 5, STREAM>(cola_fifo, in, nbs[(5 + FIFO_DEPTH) & 7], gq + 3 * lb, Vh, tb, rawB, ez_b, sb, acc);
+                hop_fifo<FMT, 6, STREAM>(cola_fifo, in, nbs[(6 + FIFO_DEPTH) & 7], nullptr, Vh, 0, rawA, et_f, sf, acc);
+                hop_fifo<FMT, 7, STREAM>(cola_fifo, in, nbs[(7 + FIFO_DEPTH) & 7], nullptr, Vh, 0, rawB, et_b, sb, acc);
+            } else
+#endif
+#if COLA_PIPE >= 2
+            {
             // two hops ahead: buffers A (even hops) and B (odd hops); hop h refills its buffer with hop h+2
             T psiA[24], psiB[24];
             RawLink<FMT> rawA, rawB;
@@ -146,6 +208,7 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
             hop_pipe<FMT, 5, STREAM, 6>(in, gq + 3 * lb, Vh, tb, tb, psiB, rawB, ez_b, sb, acc);
             hop_pipe<FMT, 6, STREAM, 6>(in, nullptr, Vh, 0, 0, psiA, rawA, et_f, sf, acc);
             hop_pipe<FMT, 7, STREAM, 6>(in, nullptr, Vh, 0, 0, psiB, rawB, et_b, sb, acc);
+            }
 #else
             T psi[24];
             RawLink<FMT> raw;
@@ -320,7 +383,7 @@ __device__ __forceinline__ unsigned sweep_run(const Sweep &w, const Geom &g, uns
 template <int FMT, int XPAY, int POST>
 __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
 {
-    constexpr bool LATE_WAIT = (FMT == LINK_I16_12) && (COLA_PIPE == 2);   // see dslash_site<.., PDLW>
+    constexpr bool LATE_WAIT = (FMT == LINK_I16_12) && (COLA_PIPE >= 2);   // see dslash_site<.., PDLW>
     pdl_trigger();
     if (!LATE_WAIT) {
         pdl_wait();
@@ -474,13 +537,14 @@ cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
     const int xpay = a.y ? (a.clov_y ? (a.clov_y_g48 ? 3 : 2) : 1) : 0;
     const int post = a.clov_post ? 1 : 0;
     const dim3 grid((a.g.Vh + DSLASH_BLOCK - 1) / DSLASH_BLOCK), block(DSLASH_BLOCK);
-    if (xpay == 0 && post == 0) launch_pdl(dslash_kernel<FMT, 0, 0>, grid, block, s, a);
-    else if (xpay == 0 && post == 1) launch_pdl(dslash_kernel<FMT, 0, 1>, grid, block, s, a);
-    else if (xpay == 1 && post == 0) launch_pdl(dslash_kernel<FMT, 1, 0>, grid, block, s, a);
-    else if (xpay == 1 && post == 1) launch_pdl(dslash_kernel<FMT, 1, 1>, grid, block, s, a);
-    else if (xpay == 2 && post == 0) launch_pdl(dslash_kernel<FMT, 2, 0>, grid, block, s, a);
+    const size_t sm = (COLA_PIPE == 3 && FMT != LINK_F64_18) ? (size_t)FIFO_DEPTH * 6 * DSLASH_BLOCK * 16 : 0;   // the spinor FIFO
+    if (xpay == 0 && post == 0) launch_pdl_smem(dslash_kernel<FMT, 0, 0>, grid, block, sm, s, a);
+    else if (xpay == 0 && post == 1) launch_pdl_smem(dslash_kernel<FMT, 0, 1>, grid, block, sm, s, a);
+    else if (xpay == 1 && post == 0) launch_pdl_smem(dslash_kernel<FMT, 1, 0>, grid, block, sm, s, a);
+    else if (xpay == 1 && post == 1) launch_pdl_smem(dslash_kernel<FMT, 1, 1>, grid, block, sm, s, a);
+    else if (xpay == 2 && post == 0) launch_pdl_smem(dslash_kernel<FMT, 2, 0>, grid, block, sm, s, a);
     else if (xpay == 3 && post == 0) {
-        if constexpr (FMT == LINK_F32_12 || FMT == LINK_F32_8 || FMT == LINK_F32_18) launch_pdl(dslash_kernel<FMT, 3, 0>, grid, block, s, a);
+        if constexpr (FMT == LINK_F32_12 || FMT == LINK_F32_8 || FMT == LINK_F32_18) launch_pdl_smem(dslash_kernel<FMT, 3, 0>, grid, block, sm, s, a);
         else return cudaErrorInvalidValue;   // the 48-real form of A exists in fp32 only
     } else return cudaErrorInvalidValue;
     return cudaGetLastError();
