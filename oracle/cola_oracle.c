@@ -23,8 +23,10 @@
  * covariance; pure-gauge = transformed free field; uniform Abelian field F_12 = sin(B) T;
  * clover sign via zero-mode shift; dense brute force on 2^4 (built independently in numpy) and
  * its explicit inverse vs the CGNR solution; Schur identity; monotone CGLS residual.
- * Nothing here is "parity unpinned" except the mixed-precision iteration (oracle_cgnr_mixed),
- * which is pinned only through its fp64 true residual and its agreement with oracle_cgnr.
+ * oracle_cgnr_mixed: its fp64 true residual, its agreement with oracle_cgnr, and its reliable-update
+ * schedule (the iterations at which updates fire = the rule of SURVEY O8 applied to oracle_cgnr's
+ * fp64 residual history, tests/schedule.py).  oracle_bicgstab: the dense inverse on 2^4, oracle_cgnr's
+ * solution, scipy's iterates.  Nothing here is "parity unpinned".
  *
  * Canonical arrays (C order, complex double = two doubles):
  *   psi[i][s][c]        i = x + Lx*(y + Ly*(z + Lz*t)), s = spin 0..3, c = colour 0..2   (O1)

@@ -298,3 +298,35 @@ def test_r8_needs_its_feature_and_unitary_links(binding):
     with pytest.raises(b.ColaError):
         c.dslash_apply(0, v, fmt="r8")
     c.close()
+
+
+def test_trace_not_removed_uses_the_72_real_blocks(binding):
+    """trace_sub = 0 (the other convention of reading A6): F keeps its trace, the 48-real form does not exist, the fp32
+    operators read the packed 72-real A -- checked against the oracle's clover field built with the same flag."""
+    dims = (4, 6, 4, 8)
+    kappa, csw = 0.124, 1.3
+    U = inputs.links_smooth(dims, 0.4, 23)
+    Un = U.numpy()
+    A = oracle.clover(dims, Un, kappa, csw, trace_sub=False)
+    A1 = oracle.clover(dims, Un, kappa, csw, trace_sub=True)
+    assert np.abs(A - A1).max() > 1e-6          # the flag matters on these links
+    Ainv = oracle.clover_inverse(A)
+    c = binding.Cola(dims, kappa, csw, bc=BC, trace_sub=False)
+    c.gauge_upload(U)
+    psi = inputs.source_gaussian(dims, 77)
+    par = oracle.parity_mask(dims)
+    xe = (psi * torch.from_numpy((par == 0)[..., None, None])).numpy()
+    want_m = oracle.M(dims, BC, Un, A, kappa, psi.numpy())
+    want_s = oracle.schur(dims, BC, Un, A, Ainv, kappa, xe)
+    v64 = c.spinor_pack(psi.cuda())
+    assert rel(c.spinor_unpack(c.fermion_matrix_apply(v64)).cpu().numpy(), want_m) < 1e-12
+    v = pack32(c, psi)
+    for fmt in (None, "r8"):
+        check(c.spinor_unpack(c.fermion_matrix_apply(v, fmt=fmt)).cpu().numpy(), want_m, "smooth")
+        out = torch.zeros_like(v)
+        c.schur_apply(v[0].contiguous(), out=out[0], fmt=fmt)
+        check(c.spinor_unpack(out).cpu().numpy(), want_s, "smooth")
+    x, info = c.cg_solve(psi.cuda(), tol=1e-10, even_odd=True, mixed=1)
+    res = np.linalg.norm((psi.numpy() - oracle.M(dims, BC, Un, A, kappa, x.cpu().numpy())).ravel()) / np.linalg.norm(psi.numpy().ravel())
+    assert info["converged"] and res <= 1.05e-10
+    c.close()
