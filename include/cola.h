@@ -282,9 +282,11 @@ cola_status cola_dslash_apply_mrhs(cola_ctx *c, cola_prec prec, cola_parity out_
 cola_status cola_fermion_matrix_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int nrhs, const void *in_full_dev, void *out_full_dev);
 /* out_e[n] = S in_e[n] (S^+ if dagger): nrhs half-lattice (even) internal DEVICE vectors each. */
 cola_status cola_schur_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int nrhs, const void *in_even_dev, void *out_even_dev);
-/* Batched solve of M x_n = b_n, n < nrhs, by mixed-precision even-odd CGNR (sp->even_odd and sp->mixed must be 1):
- * the systems advance in lock step, each with its own alpha, beta, stopping test and reliable-update schedule
- * (SURVEY O7/O8 per system); a system that has converged drops out of the batch.  b_canon_dev / x_canon_dev: nrhs
+/* Batched solve of M x_n = b_n, n < nrhs, by the mixed-precision even-odd solvers (sp->even_odd = 1, sp->mixed = 1, 2 or 3;
+ * sp->method COLA_CGNR or COLA_BICGSTAB): the systems advance in lock step, each with its own scalars, stopping test and
+ * reliable-update schedule (SURVEY O7/O8 per system); a system that has converged drops out of the batch.  With
+ * COLA_BICGSTAB the two applications of S per pass are multi-rhs launches and the vector updates are the single-system
+ * BiCGStab's kernels, one system after the other.  b_canon_dev / x_canon_dev: nrhs
  * canonical complex128 DEVICE arrays back to back (b and x must not overlap; during the call x also holds the
  * solver's internal iterates, its final content is the canonical solution); infos: HOST array of nrhs entries
  * (seconds = time of the whole batch).  COLA_ENOCONV if any system hit max_iter (its info has the last residual).  COLA_ENOTREADY without a

@@ -524,16 +524,16 @@ class Cola:
         self._ck(_lib.cola_schur_apply_mrhs(self._h, pr, int(bool(dagger)), nrhs, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr())))
         return out
 
-    def cg_solve_mrhs(self, b: torch.Tensor, tol=1e-10, max_iter=20000, delta=0.1, x: torch.Tensor | None = None, mixed=1):
+    def cg_solve_mrhs(self, b: torch.Tensor, tol=1e-10, max_iter=20000, delta=0.1, x: torch.Tensor | None = None, mixed=1, method="cgnr"):
         """b: nrhs canonical complex128 sources, shape (nrhs, t, z, y, x, 4, 3), on the device.
-        Returns (x, [info dict per system])."""
+        method: "cgnr" or "bicgstab" (both on the Schur system, mixed precision).  Returns (x, [info dict per system])."""
         assert b.is_cuda and b.dtype == torch.complex128 and b.dim() == 7 and b[0].numel() == self.V * 12
         b = b.contiguous()
         nrhs = b.shape[0]
         self._need_mrhs(nrhs, for_solver=True)
         if x is None:
             x = torch.empty_like(b)
-        sp = self._solve_params(tol, max_iter, True, mixed, delta)
+        sp = self._solve_params(tol, max_iter, True, mixed, delta, method)
         infos = (ColaSolveInfo * nrhs)()
         st = _lib.cola_cg_solve_mrhs(self._h, ctypes.byref(sp), nrhs, ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), infos)
         self._ck(st, ok=(COLA_OK, COLA_ENOCONV))

@@ -66,6 +66,11 @@ struct cola_ctx {
     char *m_r64;                    // [m_nrhs] fp64 half vectors: Schur temporary of the operator API; r of the batched solver
     char *m_rhs, *m_qs;             // [m_nrhs] fp64 half vectors: prepared sources, K x of the reliable updates
     char *m_x32, *m_r32, *m_p32, *m_q32;   // [m_nrhs] fp32 half vectors of the inner iteration
+    char *m_rhat32;                 // [m_nrhs] fp32 shadow residuals of the batched BiCGStab
+    CtlB *m_ctlb;                   // [MRHS_MAX] device scalars of the batched BiCGStab, one block per system
+    HostStatus *m_statb;            // [MRHS_MAX] device: what each system's x/r update publishes
+    double *m_tt;                   // [MRHS_MAX] device: |t_n|^2 as the multi-rhs operator reduces them
+    HostStatus *h_statb;            // pinned host copy of m_statb (allocated on first use)
     double *m_partials;             // [m_nrhs][m_nsb]
     int m_nsb;
     CtlM *ctlm;                     // device, inside the control block
@@ -230,6 +235,7 @@ cola_status cola_destroy(cola_ctx *c)
     cudaStreamSynchronize(c->stream);
     cudaFree(c->ctl);
     cudaFreeHost(c->h_pinned);
+    if (c->h_statb) cudaFreeHost(c->h_statb);
     cudaEventDestroy(c->ev0);
     cudaEventDestroy(c->ev1);
     if (c->prof_ev) {
@@ -1304,7 +1310,7 @@ namespace {
 
 struct CarveM {
     size_t tmp32, r64, partials, op_total;          // what the multi-rhs operators need
-    size_t rhs, qs, x32, r32, p32, q32, total;      // + the vectors of the batched solver
+    size_t rhs, qs, x32, r32, p32, q32, rhat32, ctlb, total;      // + the vectors of the batched solvers
     int nsb;
 };
 
@@ -1331,6 +1337,8 @@ CarveM carve_m(const cola_ctx *c, int nrhs)
     k.r32 = take(n * h32);
     k.p32 = take(n * h32);
     k.q32 = take(n * h32);
+    k.rhat32 = take(n * h32);
+    k.ctlb = take(MRHS_MAX * (sizeof(CtlB) + sizeof(HostStatus) + sizeof(double)));
     k.total = off;
     return k;
 }
@@ -1466,8 +1474,8 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
     ST(need_mrhs(c, "cola_cg_solve_mrhs", nrhs));
     if (!sp || !b_canon_dev || !x_canon_dev || !infos) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: NULL argument");
     if (!(sp->tol > 0) || sp->max_iter < 1) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: tol must be > 0 and max_iter >= 1");
-    if (!sp->even_odd || sp->mixed < 1 || sp->mixed > 3 || sp->method != COLA_CGNR)
-        return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd CGNR solver is batched (even_odd = 1, mixed = 1, 2 or 3, method = COLA_CGNR)");
+    if (!sp->even_odd || sp->mixed < 1 || sp->mixed > 3 || (sp->method != COLA_CGNR && sp->method != COLA_BICGSTAB))
+        return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: only the mixed-precision even-odd solvers are batched (even_odd = 1, mixed = 1, 2 or 3)");
     if (sp->mixed == 2) ST(check_prec(c, COLA_F32_H16, 0, 0));
     if (sp->mixed == 3) ST(check_prec(c, COLA_F32_R8, 0, 0));
     if (!c->m_solver) return fail(c, COLA_ENOTREADY, "cola_cg_solve_mrhs: the multi-rhs workspace was sized for operators only (cola_mrhs_workspace_bytes with for_solver = 1)");
@@ -1519,7 +1527,112 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
         else A[na++] = n;
     }
 
-    if (na > 0) {
+    if (na > 0 && sp->method == COLA_BICGSTAB) {
+        // Batched BiCGStab (SURVEY 8(f) NEXT-4 on NEXT-1's kernels): the systems advance pass by pass in lock step, the two
+        // applications of S per pass are multi-rhs launches over the active systems, everything else is the single-system
+        // BiCGStab's own kernels and scalars (one CtlB per system), so each system follows its sequential recurrence (the
+        // fused |t|^2 is summed in the multi-rhs kernels' order).  No speculative queueing: one stream synchronisation per
+        // pass reads every system's |r|^2 and flag.  s and t of system n live in its fp64 slot of m_qs (K x64 of the reliable
+        // update, dead during a pass), v in m_q32.
+        if (!c->h_statb) CK(cudaHostAlloc(reinterpret_cast<void **>(&c->h_statb), MRHS_MAX * sizeof(HostStatus), cudaHostAllocDefault));
+        const double delta2 = delta * delta;
+        const cola_prec P = COLA_F32;
+        const size_t nv = c->Vh;
+        auto v32 = [&](char *base, int n) { return base + (size_t)n * h32; };
+        auto s32 = [&](int n) { return c->m_qs + (size_t)n * h64; };
+        auto t32 = [&](int n) { return c->m_qs + (size_t)n * h64 + h32; };
+        for (int j = 0; j < na; j++) {
+            const int n = A[j];
+            CtlB init;
+            memset(&init, 0, sizeof(init));
+            init.rv[0] = init.ts[0] = init.tt = 1.0;
+            init.rho[0] = 1.0;
+            init.rmax2 = rr[n]; init.target2 = target2[n]; init.delta2 = delta2;
+            CK(cudaMemcpyAsync(&c->m_ctlb[n], &init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
+            CK(cudaMemcpyAsync(v32(c->m_rhat32, n), v32(c->m_r32, n), h32, cudaMemcpyDeviceToDevice, c->stream));
+            CK(cudaMemcpyAsync(v32(c->m_p32, n), v32(c->m_r32, n), h32, cudaMemcpyDeviceToDevice, c->stream));
+            CK(launch_bicg_dot(P, v32(c->m_rhat32, n), v32(c->m_r32, n), &c->m_ctlb[n], 2, nullptr, nv, c->red, c->stream));   // rho_1 = <rhat, r_0>
+            c->launches++;
+        }
+        CK(cudaStreamSynchronize(c->stream));   // `init` is a stack object of this loop
+        for (int k = 0;; k++) {
+            const int more = (k + 1 < sp->max_iter);
+            const MrhsList L = list_of(A, na);
+            ST(schur_m(c, c->inner_prec, 0, L, na, c->m_p32, h32, c->m_tmp32, c->m_q32, h32, nullptr, nullptr));             // v = S p
+            for (int j = 0; j < na; j++) {
+                const int n = A[j];
+                CK(launch_bicg_dot(P, v32(c->m_rhat32, n), v32(c->m_q32, n), &c->m_ctlb[n], 0, nullptr, nv, c->red, c->stream));
+                CK(launch_bicg_s_update(P, s32(n), v32(c->m_r32, n), v32(c->m_q32, n), &c->m_ctlb[n], nullptr, nv, c->stream));
+            }
+            ST(schur_m(c, c->inner_prec, 0, L, na, c->m_qs, h64, c->m_tmp32, c->m_qs + h32, h64, c->m_tt, nullptr));          // t = S s, |t|^2
+            for (int j = 0; j < na; j++) {
+                const int n = A[j];
+                CK(cudaMemcpyAsync(&c->m_ctlb[n].tt, &c->m_tt[n], sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+                CK(launch_bicg_dot(P, t32(n), s32(n), &c->m_ctlb[n], 1, nullptr, nv, c->red, c->stream));
+                CK(launch_bicg_xr_update(P, v32(c->m_x32, n), v32(c->m_r32, n), v32(c->m_p32, n), s32(n), t32(n), v32(c->m_rhat32, n), &c->m_ctlb[n], k + 1,
+                                         nullptr, c->m_statb + n, nv, c->red, c->stream));
+            }
+            c->launches += 4 * (unsigned long long)na;
+            CK(cudaMemcpyAsync(c->h_statb, c->m_statb, MRHS_MAX * sizeof(HostStatus), cudaMemcpyDeviceToHost, c->stream));
+            CK(cudaStreamSynchronize(c->stream));
+            int S[MRHS_MAX], ns = 0;
+            for (int j = 0; j < na; j++) {
+                const int n = A[j];
+                rr[n] = c->h_statb[n].rr;
+                iters[n] = k + 1;
+                flops[n] += 2 * flops_K;
+                if (!(rr[n] <= DBL_MAX))
+                    return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: BiCGStab broke down or met NaN/Inf (<rhat, v>, <t, t> or rho vanished, or bad input)");
+                if (c->h_statb[n].flag) S[ns++] = n;
+            }
+            if (ns > 0) {   // reliable updates of the systems that asked for one (or converged in the inner precision)
+                for (int j = 0; j < ns; j++) {
+                    CK(launch_accumulate(Xall + (size_t)S[j] * f64, v32(c->m_x32, S[j]), c->Vh, c->stream));   // x64 += x32, x32 = 0
+                    c->launches++;
+                }
+                const MrhsList LS = list_of(S, ns);
+                ST(schur_m(c, COLA_F64, 0, LS, ns, Xall, f64, c->m_r64, c->m_qs, h64, nullptr, nullptr));      // K x64 into the (dead) s / t slot
+                for (int j = 0; j < ns; j++) {
+                    const size_t n = (size_t)S[j];
+                    CK(launch_axpby64(c->m_r64 + n * h64, 1.0, c->m_rhs + n * h64, -1.0, c->m_qs + n * h64, c->m_r32 + n * h32, c->Vh, &c->red,
+                                      &ctl->counter[3], &c->m_tt[n], c->stream));                              // r64 = rhs - S x64, r32 = float(r64)
+                    c->launches++;
+                }
+                CK(cudaMemcpyAsync(c->h_pinned, c->m_tt, sizeof(double) * MRHS_MAX, cudaMemcpyDeviceToHost, c->stream));
+                CK(cudaStreamSynchronize(c->stream));
+                struct { double rmax2, target2, delta2; int flag, iters; } st[MRHS_MAX];
+                static_assert(offsetof(CtlB, iters) - offsetof(CtlB, rmax2) == 28, "decision block layout");
+                for (int j = 0; j < ns; j++) {
+                    const int n = S[j];
+                    rr[n] = c->h_pinned[n];
+                    updates[n]++;
+                    flops[n] += flops_K;
+                    if (!(rr[n] <= DBL_MAX)) return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: the fp64 residual is not a number (NaN or Inf in the gauge field)");
+                    if (rr[n] <= target2[n]) { conv[n] = 1; continue; }
+                    if (!more) continue;
+                    st[j].rmax2 = rr[n]; st[j].target2 = target2[n]; st[j].delta2 = delta2; st[j].flag = 0; st[j].iters = k + 1;
+                    CK(cudaMemcpyAsync(&c->m_ctlb[n].rmax2, &st[j], sizeof(st[j]), cudaMemcpyHostToDevice, c->stream));
+                    CK(launch_bicg_dot(P, v32(c->m_rhat32, n), v32(c->m_r32, n), &c->m_ctlb[n], 2, nullptr, nv, c->red, c->stream));   // rho' and beta with the replaced residual
+                    c->launches++;
+                }
+                CK(cudaStreamSynchronize(c->stream));   // `st` is a stack object of this block
+            }
+            int na2 = 0;
+            for (int j = 0; j < na; j++)
+                if (!conv[A[j]]) A[na2++] = A[j];
+            na = na2;
+            if (na == 0 || !more) break;
+            for (int j = 0; j < na; j++) {   // p = r + beta (p - omega v)
+                const int n = A[j];
+                CK(launch_bicg_p_update(P, v32(c->m_p32, n), v32(c->m_r32, n), v32(c->m_q32, n), &c->m_ctlb[n], nullptr, nv, c->stream));
+                c->launches++;
+            }
+        }
+        for (int j = 0; j < na; j++) {   // max_iter: fold the fp32 parts into the fp64 iterates
+            CK(launch_accumulate(Xall + (size_t)A[j] * f64, c->m_x32 + (size_t)A[j] * h32, c->Vh, c->stream));
+            c->launches++;
+        }
+    } else if (na > 0) {
         CtlM st;
         memset(&st, 0, sizeof(st));
         for (int n = 0; n < nrhs; n++) { st.rmax2[n] = rr[n]; st.target2[n] = target2[n]; }
@@ -1830,6 +1943,10 @@ cola_status cola_set_mrhs_workspace(cola_ctx *c, void *dev_ptr, size_t bytes, in
     char *w = (char *)dev_ptr;
     c->m_tmp32 = w + k.tmp32; c->m_r64 = w + k.r64; c->m_rhs = w + k.rhs; c->m_qs = w + k.qs;
     c->m_x32 = w + k.x32; c->m_r32 = w + k.r32; c->m_p32 = w + k.p32; c->m_q32 = w + k.q32;
+    c->m_rhat32 = w + k.rhat32;
+    c->m_ctlb = (CtlB *)(w + k.ctlb);
+    c->m_statb = (HostStatus *)(w + k.ctlb + MRHS_MAX * sizeof(CtlB));
+    c->m_tt = (double *)(w + k.ctlb + MRHS_MAX * (sizeof(CtlB) + sizeof(HostStatus)));
     c->m_partials = (double *)(w + k.partials);
     c->m_nsb = k.nsb;
     c->m_nrhs = nrhs;

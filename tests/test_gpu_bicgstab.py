@@ -68,3 +68,42 @@ def test_bicgstab_matches_the_oracle(dims, kind):
     xx, info = c.cg_solve(b.cuda(), max_iter=2, method="bicgstab", mixed=1)
     assert not info["converged"] and info["iters"] == 2 and 0 < info["true_residual"] < 1
     c.close()
+
+
+@pytest.mark.parametrize("mixed", [1, 2])
+def test_batched_bicgstab_matches_the_oracle_and_the_sequential_solver(mixed):
+    """cola_cg_solve_mrhs with method = COLA_BICGSTAB: every system's solution against the oracle (true residual with the
+    ORACLE's M, solution against oracle.cgnr's), pass counts against the sequential CUDA BiCGStab of the same system
+    (the recurrences differ only in the summation order of the fused |t|^2) and against the oracle's BiCGStab."""
+    from paper_2302_00850_b200 import binding
+
+    dims, kappa, csw = (8, 8, 8, 16), 0.1245, 1.0
+    U = inputs.links_smooth(dims, 0.3, 33)
+    Un = U.numpy()
+    A = oracle.clover(dims, Un, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    c = binding.Cola(dims, kappa, csw, bc=BC)
+    c.gauge_upload(U)
+    srcs = [inputs.source_point(dims, s, s % 3) for s in range(4)] + [inputs.source_gaussian(dims, 66), torch.zeros_like(inputs.source_gaussian(dims, 1))]
+    x, infos = c.cg_solve_mrhs(torch.stack(srcs).cuda(), tol=1e-10, mixed=mixed, method="bicgstab")
+    for n, s in enumerate(srcs[:-1]):
+        bn = s.numpy()
+        xn = x[n].cpu().numpy()
+        res = np.linalg.norm((bn - oracle.M(dims, BC, Un, A, kappa, xn)).ravel()) / np.linalg.norm(bn.ravel())
+        assert res <= 1.05e-10 and infos[n]["true_residual"] <= 1.05e-10, (n, res, infos[n])
+        assert infos[n]["reliable_updates"] >= 1
+        x1, i1 = c.cg_solve(s.cuda(), tol=1e-10, even_odd=True, mixed=mixed, method="bicgstab")
+        assert abs(infos[n]["iters"] - i1["iters"]) <= max(2, math.ceil(0.1 * i1["iters"])), (n, infos[n]["iters"], i1["iters"])
+        assert rel(xn, x1.cpu().numpy()) < 5e-9
+        if n in (0, 4):
+            ref = oracle.bicgstab(dims, BC, Un, A, Ainv, kappa, bn, even_odd=True, tol=1e-10)
+            cg = oracle.cgnr(dims, BC, Un, A, Ainv, kappa, bn, even_odd=True, tol=1e-10)
+            assert rel(xn, ref["x"]) < 5e-9 and rel(xn, cg["x"]) < 5e-9
+            assert abs(infos[n]["iters"] - ref["iters"]) <= max(2, math.ceil(0.15 * ref["iters"])), (infos[n]["iters"], ref["iters"])
+            assert infos[n]["iters"] < cg["iters"]
+    # the zero source: solution zero, no passes
+    assert infos[-1]["iters"] == 0 and float(x[-1].abs().max()) == 0.0
+    # max_iter: COLA_ENOCONV, the last iterates returned with their true residuals
+    xx, inf2 = c.cg_solve_mrhs(torch.stack(srcs[:3]).cuda(), tol=1e-10, mixed=mixed, method="bicgstab", max_iter=3)
+    assert all(i["iters"] == 3 and not i["converged"] and 0 < i["true_residual"] < 1 for i in inf2)
+    c.close()
