@@ -124,6 +124,34 @@ def test_operators_on_sampled_sites(big, dtype):
         check_op(got, oracle.apply_sites(*args, which, psin, even), dtype)
 
 
+def test_r8_operators_on_sampled_sites(big):
+    """COLA_F32_R8 (8-real links + 48-real A) at full size, fp32 tolerance, and its solver mode."""
+    c, dims, cfg = big.ctx, big.dims, big.cfg
+    if big.k == 4:
+        pytest.skip("64^3x128 context is carved without COLA_FEAT_R8 (workspace)")
+    psi = inputs.source_gaussian(dims, 4343 + big.k, device="cuda")
+    psin = psi.cpu().numpy()
+    internal = c.spinor_pack(psi.to(torch.complex64))
+    if c.gauge_info_r8() < 0.1:      # a link in the tail of the ensemble with |U00| < 0.1: the format is refused, not wrong
+        from paper_2302_00850_b200 import binding
+        with pytest.raises(binding.ColaError):
+            c.fermion_matrix_apply(internal, fmt="r8")
+        return
+    args = (dims, inputs.BC, big.Un, cfg["kappa"], cfg["csw"])
+    got = at_sites(c.spinor_unpack(c.fermion_matrix_apply(internal, fmt="r8")), big.sites)
+    check_op(got, oracle.apply_sites(*args, "M", psin, big.sites), torch.float32)
+    even = big.sites[big.par == 0]
+    out = torch.zeros_like(internal)
+    c.schur_apply(internal[0], dagger=True, out=out[0], fmt="r8")
+    check_op(at_sites(c.spinor_unpack(out), even), oracle.apply_sites(*args, "Sdag", psin, even), torch.float32)
+    if big.k == 2:
+        b = inputs.source_gaussian(dims, inputs.config_seed_source(big.k), device="cuda")
+        x, info = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=3)
+        x1, info1 = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=1)
+        assert info["converged"] and info["true_residual"] <= 1.05e-10
+        assert abs(info["iters"] - info1["iters"]) <= 1 and info["reliable_updates"] == info1["reliable_updates"]
+
+
 def test_mixed_precision_solve(big):
     c, dims, cfg, k = big.ctx, big.dims, big.cfg, big.k
     if cfg["source"] == "point":
