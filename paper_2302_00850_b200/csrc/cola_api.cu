@@ -443,7 +443,7 @@ static cola_status check_prec(cola_ctx *c, cola_prec prec, int parity, int uses_
 
 // out_p = [post] ( [A] y + coef * D_{p,1-p} in ), optional |out|^2 -> norm_out
 static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, const void *in, void *out, const void *y, int clov_on_y,
-                          double coef, int post_inv, double *norm_out, int norm_accumulate, const int *skip = nullptr)
+                          double coef, int post_inv, double *norm_out, int norm_accumulate, const int *skip = nullptr, double *dot_out = nullptr)
 {
     ST(check_prec(c, prec, parity, (y && clov_on_y) ? 1 : 0));
     DslashArgs a;
@@ -467,11 +467,12 @@ static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, c
         a.counter = &c->ctl->counter[0];
         a.norm_out = norm_out;
         a.norm_accumulate = norm_accumulate;
+        a.dot_out = y ? dot_out : nullptr;     // <out, y>, fused with the norm (direct kernels only)
     }
     if (post_inv && parity != 1) return fail(c, COLA_EINVAL, "internal: A^-1 is stored on the odd parity only");
     const bool timed = c->prof_on && c->prof_created == 2 * PROF_MAX && c->prof_n < PROF_MAX && prec != COLA_F64 && a.clov_y;   // Schur kernel 2 / M of the inner precision
     if (timed) CK(cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream));
-    cudaError_t le = c->staging ? launch_dslash_tile(fmt_of(c, prec), a, c->stream) : cudaErrorNotSupported;
+    cudaError_t le = (c->staging && !a.dot_out) ? launch_dslash_tile(fmt_of(c, prec), a, c->stream) : cudaErrorNotSupported;
     if (le == cudaErrorNotSupported) le = launch_dslash(fmt_of(c, prec), a, c->stream);
     CK(le);
     if (timed) {
@@ -483,11 +484,12 @@ static cola_status dslash(cola_ctx *c, cola_prec prec, int parity, int dagger, c
 }
 
 // out_e = S in_e  (2 launches; norm of the result optional)
-static cola_status schur(cola_ctx *c, cola_prec prec, int dagger, const void *in_e, void *out_e, double *norm_out, const int *skip = nullptr)
+static cola_status schur(cola_ctx *c, cola_prec prec, int dagger, const void *in_e, void *out_e, double *norm_out, const int *skip = nullptr,
+                         double *dot_out = nullptr)   // dot_out (with norm_out): <S in, in>
 {
     const double k = c->p.kappa;
     ST(dslash(c, prec, 1, dagger, in_e, tmp_of(c, prec), nullptr, 0, 0.0, 1, nullptr, 0, skip));          // t_o = A_oo^-1 D_oe x_e
-    ST(dslash(c, prec, 0, dagger, tmp_of(c, prec), out_e, in_e, 1, -k * k, 0, norm_out, 0, skip));        // A_ee x_e - k^2 D_eo t_o
+    ST(dslash(c, prec, 0, dagger, tmp_of(c, prec), out_e, in_e, 1, -k * k, 0, norm_out, 0, skip, dot_out));   // A_ee x_e - k^2 D_eo t_o
     return COLA_OK;
 }
 
@@ -585,11 +587,12 @@ struct System {            // K x = rhs on n_sites sites; K = S (even_odd) or M
     size_t n_sites;
 };
 
-cola_status apply_K(cola_ctx *c, const System &sy, cola_prec prec, int dagger, const void *in, void *out, double *norm_out, const int *skip = nullptr)
+cola_status apply_K(cola_ctx *c, const System &sy, cola_prec prec, int dagger, const void *in, void *out, double *norm_out, const int *skip = nullptr,
+                    double *dot_out = nullptr)   // Schur system only: <K in, in> next to |K in|^2
 {
     // the inner fp32 iteration of a mixed = 2 / 3 solve reads the 16-bit / compact fields (same fp32 vectors)
     const cola_prec op = (prec == COLA_F32) ? c->inner_prec : prec;
-    return sy.even_odd ? schur(c, op, dagger, in, out, norm_out, skip) : fmatrix(c, op, dagger, in, out, norm_out, skip);
+    return sy.even_odd ? schur(c, op, dagger, in, out, norm_out, skip, dot_out) : fmatrix(c, op, dagger, in, out, norm_out, skip);
 }
 
 // (re)arm the device-side decision state: rmax2, target2, delta2, flag = 0, iters
@@ -884,10 +887,9 @@ cola_status bicg_first_half(cola_ctx *c, const System &sy, cola_prec P, int k, c
     ST(apply_K(c, sy, P, 0, pi, vi, nullptr, &cb->flag));
     CK(launch_bicg_dot(P, rhat, vi, cb, 0, &cb->flag, sy.n_sites, c->red, c->stream));
     CK(launch_bicg_s_update(P, si, ri, vi, cb, &cb->flag, sy.n_sites, c->stream));
-    ST(apply_K(c, sy, P, 0, si, ti, &cb->tt, &cb->flag));
-    CK(launch_bicg_dot(P, ti, si, cb, 1, &cb->flag, sy.n_sites, c->red, c->stream));
+    ST(apply_K(c, sy, P, 0, si, ti, &cb->tt, &cb->flag, cb->ts));   // t = S s with |t|^2 and <t, s> from the same kernel (s and t are in its registers)
     CK(launch_bicg_xr_update(P, xi, ri, pi, si, ti, rhat, cb, k + 1, &cb->flag, c->d_status + (k & 1), sy.n_sites, c->red, c->stream));
-    c->launches += 4;
+    c->launches += 3;
     return COLA_OK;
 }
 

@@ -114,8 +114,9 @@ __device__ __forceinline__ void hop_fifo(float4 *fifo, const void *in, const int
 // yet: the index arithmetic and the raw links of the first two hops run before pdl_wait(); a raised skip flag
 // (grid-uniform) is reported by returning -1.  (+2 % for the SM-bound 16-bit kernels; the fp32 kernels lose 1.7 % with
 // the reordered first loads and wait at the top of the kernel instead.)
-template <int FMT, int XPAY, int POST, bool STREAM, bool PDLW = false>
-__device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, const void *in, const void *yin, void *out, const bool want_norm)
+template <int FMT, int XPAY, int POST, bool STREAM, bool PDLW = false, bool DOT = false>
+__device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, const void *in, const void *yin, void *out, const bool want_norm,
+                                              double *dot = nullptr)
 {
     typedef typename LinkT<FMT>::T T;
     const Geom &g = a.g;
@@ -236,7 +237,7 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
         hop<FMT, 3, true, STREAM>(in, gq + 3 * lb, Vh, tb, tb, et_b, sb, acc);
         }
 
-        nrm = dslash_epilogue<FMT, XPAY, POST, STREAM>(a, i, acc, yin, out, want_norm);
+        nrm = dslash_epilogue<FMT, XPAY, POST, STREAM, DOT>(a, i, acc, yin, out, want_norm, dot);
     }
     return nrm;
 }
@@ -380,7 +381,8 @@ __device__ __forceinline__ unsigned sweep_run(const Sweep &w, const Geom &g, uns
     return ((t * (unsigned)g.Z + band * w.d_zb.d + zi) * w.d_up.d) + u;
 }
 
-template <int FMT, int XPAY, int POST>
+// DOT (XPAY != 0, POST == 0, with a norm): also reduces <out, y> into a.dot_out (BiCGStab's <t, s> for t = S s)
+template <int FMT, int XPAY, int POST, bool DOT = false>
 __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
 {
     constexpr bool LATE_WAIT = (FMT == LINK_I16_12) && (COLA_PIPE >= 2);   // see dslash_site<.., PDLW>
@@ -394,15 +396,23 @@ __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_ke
     const unsigned run = sweep_run(a.sweep, a.g, blockIdx.x);
     const int i = (int)run * DSLASH_BLOCK + (int)threadIdx.x;
     const bool want_norm = a.red.partials != nullptr;
-    double nrm = 0.0;
+    double nrm = 0.0, dot[2] = {0.0, 0.0};
     if (i < a.g.Vh) {
-        nrm = dslash_site<FMT, XPAY, POST, true, LATE_WAIT>(a, i, a.in, a.y, a.out, want_norm);
+        nrm = dslash_site<FMT, XPAY, POST, true, LATE_WAIT, DOT>(a, i, a.in, a.y, a.out, want_norm, dot);
     } else if (LATE_WAIT) {
         pdl_wait();
         nrm = (a.skip && *a.skip) ? -1.0 : 0.0;
     }
     if (LATE_WAIT && nrm < 0.0) return;   // skip flag raised: the same for every thread of the grid
-    if (want_norm) grid_sum_finalize(nrm, a.red, a.counter, a.norm_out, a.norm_accumulate != 0);
+    if constexpr (DOT) {   // |out|^2 and <out, y> in one deterministic reduction (the launcher guarantees norm_out and dot_out)
+        const double v3[3] = {nrm, dot[0], dot[1]};
+        double tot[3];
+        if (grid_sum_last_n<3>(v3, a.red, a.counter, tot)) {
+            *a.norm_out = a.norm_accumulate ? *a.norm_out + tot[0] : tot[0];
+            a.dot_out[0] = tot[1];
+            a.dot_out[1] = tot[2];
+        }
+    } else if (want_norm) grid_sum_finalize(nrm, a.red, a.counter, a.norm_out, a.norm_accumulate != 0);
 }
 
 // ---- multi-right-hand-side variant (MrhsArgs in cola_internal.h)
@@ -542,9 +552,14 @@ cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
     else if (xpay == 0 && post == 1) launch_pdl_smem(dslash_kernel<FMT, 0, 1>, grid, block, sm, s, a);
     else if (xpay == 1 && post == 0) launch_pdl_smem(dslash_kernel<FMT, 1, 0>, grid, block, sm, s, a);
     else if (xpay == 1 && post == 1) launch_pdl_smem(dslash_kernel<FMT, 1, 1>, grid, block, sm, s, a);
-    else if (xpay == 2 && post == 0) launch_pdl_smem(dslash_kernel<FMT, 2, 0>, grid, block, sm, s, a);
-    else if (xpay == 3 && post == 0) {
-        if constexpr (FMT == LINK_F32_12 || FMT == LINK_F32_8 || FMT == LINK_F32_18) launch_pdl_smem(dslash_kernel<FMT, 3, 0>, grid, block, sm, s, a);
+    else if (xpay == 2 && post == 0) {
+        if (a.dot_out && a.norm_out) launch_pdl_smem(dslash_kernel<FMT, 2, 0, true>, grid, block, sm, s, a);
+        else launch_pdl_smem(dslash_kernel<FMT, 2, 0>, grid, block, sm, s, a);
+    } else if (xpay == 3 && post == 0) {
+        if constexpr (FMT == LINK_F32_12 || FMT == LINK_F32_8 || FMT == LINK_F32_18) {
+            if (a.dot_out && a.norm_out) launch_pdl_smem(dslash_kernel<FMT, 3, 0, true>, grid, block, sm, s, a);
+            else launch_pdl_smem(dslash_kernel<FMT, 3, 0>, grid, block, sm, s, a);
+        }
         else return cudaErrorInvalidValue;   // the 48-real form of A exists in fp32 only
     } else return cudaErrorInvalidValue;
     return cudaGetLastError();

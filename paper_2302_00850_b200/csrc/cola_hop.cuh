@@ -110,15 +110,18 @@ __device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&
 //   XPAY 1: acc = y + coef acc;  XPAY 2: acc = A y + coef acc;  XPAY 3: the same with A in its 48-real form;
 //   POST 1: acc = Cpost acc;  store;  returns |acc|^2 if want_norm.
 // STREAM: clover read once per launch (no L1 allocation); !STREAM: shared by the right-hand sides of a block.
-template <int FMT, int XPAY, int POST, bool STREAM>
+// dot (nullable, XPAY != 0 only): dot[0..1] = this site's part of sum conj(out) * y, e.g. BiCGStab's <t, s> for t = S s, whose
+// kernel 2 holds s (= y) and t (= out) in registers anyway.
+// DOT is a compile-time switch: the kernels without it are the ones of the CGNR iteration and stay as they were.
+template <int FMT, int XPAY, int POST, bool STREAM, bool DOT = false>
 __device__ __forceinline__ double dslash_epilogue(const DslashArgs &a, const int i, typename LinkT<FMT>::T (&acc)[24], const void *yin, void *out,
-                                                  const bool want_norm)
+                                                  const bool want_norm, double *dot = nullptr)
 {
     typedef typename LinkT<FMT>::T T;
     const size_t Vh = a.g.Vh;
     double nrm = 0.0;
+    T yv[24];
     if (XPAY != 0) {
-        T yv[24];
         load_reals<T, 24, true>(yin, Vh, i, yv);
         const T cf = (T)a.coef;
         if (XPAY == 2 || XPAY == 3) {
@@ -144,6 +147,16 @@ __device__ __forceinline__ double dslash_epilogue(const DslashArgs &a, const int
 #pragma unroll
         for (int k = 0; k < 24; k++) s2 += acc[k] * acc[k];
         nrm = (double)s2;
+        if constexpr (XPAY != 0 && DOT) {
+            T dr = 0, di = 0;
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                dr += acc[2 * k] * yv[2 * k] + acc[2 * k + 1] * yv[2 * k + 1];
+                di += acc[2 * k] * yv[2 * k + 1] - acc[2 * k + 1] * yv[2 * k];
+            }
+            dot[0] = (double)dr;
+            dot[1] = (double)di;
+        }
     }
     return nrm;
 }

@@ -176,6 +176,7 @@ struct DslashArgs {
     ReduceWs red;           // reduction buffers (red.partials == nullptr: no norm)
     unsigned *counter;
     double *norm_out;
+    double *dot_out;        // with norm_out and y: dot_out[0..1] = sum conj(out) * y (complex), reduced together with the norm
     int norm_accumulate;    // 1: *norm_out += sum (second half of a full-lattice operator)
     const int *skip;        // if non-null and *skip != 0 the launch is a no-op (speculatively queued iteration)
 };
