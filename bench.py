@@ -16,10 +16,13 @@ roofline= the dominant kernel (fused dslash + clover + xpay, fp32 with 12-real l
           events: algorithmic bytes per launch / average launch time, against MEASURED_PEAKS.json hbm_gbs;
           roofline.in_solve = the same kernel inside a solve (CUDA-event pair around each of its launches in one extra
           step; cola_profile_kernel).
-extras  : solve_h16 = the same step with 16-bit links + fp16 clover in the inner iteration (mixed = 2, SURVEY 8(f)
-          NEXT-2); batched (config 3) = its 12 sources as one multi-rhs solve (NEXT-1); operators = every operator
-          x {fp32 x12, fp64 x18, 16-bit}.  --operators-only [--nrhs N] [--lattice X,Y,Z,T] is the short launch sequence
-          the ncu captures and the volume sweep in profiles/ come from.
+extras  : (N = 1 only) solve_h16 / solve_r8 = the same step with 16-bit links + fp16 clover (mixed = 2) or 8-real links
+          (mixed = 3) in the inner iteration; solve_bicgstab = the same step by BiCGStab on the Schur
+          system and low_modes = the lowest modes of S^+S + the deflated step (NEXT-4); batched (config 3) = its 12 sources
+          as one multi-rhs solve, CGNR and BiCGStab (NEXT-1); operators = every operator x {fp32 x12, fp64 x18, 16-bit,
+          8-real, fp32 x12 with the 72-real A}.  --operators-only [--nrhs N] [--lattice X,Y,Z,T] [--staging 1] is the short
+          launch sequence the ncu captures and the volume sweep in profiles/ come from; --ab-formats the interleaved
+          comparison of the storage formats.
 N > 1   : replicas only (the path has no inter-GPU exchange): every rank solves its own
           source on its own GPU; value = all ranks' flops / max-over-ranks time ("weak").
 """
@@ -561,13 +564,14 @@ def main():
                 "max_true_residual": max(i["true_residual"] for i in infs_h), "converged": all(i["converged"] for i in infs_h)}
 
     solve_h16 = solve_r8 = None
-    if rank == 0 and not args.no_h16:
+    extras = rank == 0 and world == 1   # the extra modes are single-GPU context for the line, not part of the scaling runs
+    if extras and not args.no_h16:
         solve_h16 = extra_solve(2)
         solve_r8 = extra_solve(3)
 
     # ---- the same step by BiCGStab on the Schur system (two S per pass instead of S and S^+)
     solve_bicgstab = None
-    if rank == 0 and not args.no_bicgstab:
+    if extras and not args.no_bicgstab:
         solve_bicgstab = {}
         for key, mode in (("fp32_inner", 1), ("h16_inner", 2), ("r8_inner", 3)):
             def bi_step():
@@ -598,7 +602,7 @@ def main():
 
     # ---- the lowest modes of S^+S and the same step started from the deflated guess
     low_modes = None
-    if rank == 0 and not args.no_eig and (ctx.Vh <= (1 << 20) or args.eig):   # larger lattices: minutes of Lanczos for nothing
+    if extras and not args.no_eig and (ctx.Vh <= (1 << 20) or args.eig):   # larger lattices: minutes of Lanczos for nothing
         try:
             torch.cuda.synchronize()
             t0 = time.time()
@@ -628,7 +632,7 @@ def main():
 
     # ---- the same sources as ONE batched solve (links and clover read once per pass for all)
     batched = None
-    if n_src > 1 and rank == 0 and not args.no_batched:
+    if n_src > 1 and extras and not args.no_batched:
         del b_host, x_host
         torch.cuda.empty_cache()
         try:
@@ -665,7 +669,7 @@ def main():
 
     # ---- roofline of the dominant kernel + operator table (rank 0, kernels timed alone)
     peak, peak_src = measured_peaks()
-    table = {} if args.no_operator_table else operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed)
+    table = {} if (args.no_operator_table or world > 1) else operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed)
     roof = None
     if table:
         k = table["fermion_matrix_f32x12"]   # two launches of the fused dslash + clover + xpay kernel
