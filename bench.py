@@ -240,6 +240,37 @@ def ab_formats(ctx, rounds=12, burst=40):
     return out
 
 
+def timeline(ctx, b, first_iter=40, n_iter=3):
+    """Device timestamps (CUPTI activity records through torch.profiler) of every kernel of `n_iter` consecutive CGLS
+    iterations of one solve: start, duration and the gap to the end of the previous kernel.  Not a bench line."""
+    from torch.profiler import ProfilerActivity, profile
+
+    ctx.cg_solve(b, tol=1e-10, even_odd=True, mixed=True)     # warm
+    torch.cuda.synchronize()
+    with profile(activities=[ProfilerActivity.CUDA]) as prof:
+        ctx.cg_solve(b, tol=1e-10, even_odd=True, mixed=True)
+        torch.cuda.synchronize()
+    evs = sorted((e for e in prof.events() if e.device_type == torch.autograd.DeviceType.CUDA and "Memcpy" not in e.name and "Memset" not in e.name),
+                 key=lambda e: e.time_range.start)
+    # an iteration ends with xp_update<float,1,1>; find the launches of iterations first_iter .. first_iter + n_iter - 1
+    ends = [i for i, e in enumerate(evs) if "xp_update_kernel<float, true, true>" in e.name or "xp_update_kernel<float, 1, 1>" in e.name]
+    # the first window of n_iter iterations from first_iter on without a reliable update (whose speculative launches return at once)
+    while first_iter + n_iter < len(ends) and any((e.time_range.end - e.time_range.start) < 20.0
+                                                   for e in evs[ends[first_iter - 1] + 1:ends[first_iter + n_iter - 1] + 1]):
+        first_iter += 1
+    lo, hi = ends[first_iter - 1] + 1, ends[first_iter + n_iter - 1] + 1
+    rows, prev_end, t0 = [], None, evs[lo].time_range.start
+    for e in evs[lo:hi]:
+        st, en = e.time_range.start, e.time_range.end
+        name = e.name.replace("void ", "").replace("cola::(anonymous namespace)::", "").split("(")[0]
+        rows.append({"kernel": name, "start_us": round(st - t0, 2), "dur_us": round(en - st, 2), "gap_us": None if prev_end is None else round(st - prev_end, 2)})
+        prev_end = en
+    busy = sum(r["dur_us"] for r in rows)
+    span = rows[-1]["start_us"] + rows[-1]["dur_us"]
+    return {"iterations": [first_iter, first_iter + n_iter - 1], "kernels": rows, "span_us": round(span, 2), "kernel_sum_us": round(busy, 2),
+            "gaps_us": round(span - busy, 2), "note": "gap < 0: the next kernel's blocks started under programmatic dependent launch before the previous grid had drained"}
+
+
 def _set_oracle_threads(n):
     """OpenMP thread count of the oracle's site loops (the oracle itself is untouched: same library, same code)."""
     import ctypes
@@ -388,6 +419,7 @@ def main():
     ap.add_argument("--staging", type=int, default=0, choices=[0, 1],
                     help="kernel family of the fp32 / 16-bit single-rhs operators: 0 direct global loads (default), 1 neighbour spinors staged in shared memory")
     ap.add_argument("--ab-formats", action="store_true", help="measurement aid: interleaved A/B of the fp32 link / clover storage formats, then exit")
+    ap.add_argument("--timeline", action="store_true", help="measurement aid: device timestamps of the kernels of three consecutive iterations, then exit")
     ap.add_argument("--op-warm", type=int, default=20)
     ap.add_argument("--op-timed", type=int, default=200)
     args = ap.parse_args()
@@ -478,6 +510,9 @@ def main():
         return fl, infos
 
     b = source(0) if n_src == 1 else None
+    if args.timeline:         # not a bench line: kernel start times of three consecutive iterations (profiles/r2_timeline.md)
+        print(json.dumps({"timeline": True, "lattice": list(dims), **timeline(ctx, b if b is not None else source(0))}))
+        return
     # ---- device-resident steps
     for _ in range(args.warmup):
         one_step()
