@@ -91,7 +91,7 @@ typedef struct {
 cola_status cola_create(cola_ctx **out, const cola_params *p);
 cola_status cola_destroy(cola_ctx *c);
 /* Message of the last failure on c (valid until the next call on c); "" if none.  c may be NULL
- * (returns the message of the last failed cola_create in this thread). */
+ * (returns the message of the last failed context-free call -- cola_create, cola_spinor_norm2_static -- in this thread). */
 const char *cola_last_error(const cola_ctx *c);
 /* Tuning: bytes of L2 the kernels' sweep order may count on for the reuse of neighbour spinors (default 40 MB; 0
  * restores it).  A neighbour spinor is used from three consecutive time slices; when three slices of reused spinors
@@ -170,6 +170,47 @@ cola_status cola_spinor_unpack(cola_ctx *c, cola_prec prec, const void *internal
 /* Internal fp64 <-> internal fp32 (round to nearest even), n_half = 1 (half lattice) or 2 (full).
  * cola_spinor_pack / unpack / convert take COLA_F64 or COLA_F32 only (COLA_EINVAL otherwise). */
 cola_status cola_spinor_convert(cola_ctx *c, cola_prec dst_prec, const void *src_dev, void *dst_dev, int n_half);
+
+/* ---- |v|^2 of an internal spinor buffer (the reduction of the fused BLAS-1 layer on its own).
+ * The sum is accumulated in fp64 also for fp32 vectors and is bitwise reproducible: warp shuffle, block, then the last
+ * thread block to finish adds the per-block partials in index order.  Asynchronous on the context's stream.
+ *   v_dev    DEVICE, internal buffer of precision prec (COLA_F64 or COLA_F32); n_half = 1: one half lattice, 2: full
+ *   out_dev  DEVICE, one double
+ * The per-block partials and the tickets of the reduction live in the workspace lent to the context: COLA_ENOTREADY
+ * without one.  No gauge field is needed. */
+cola_status cola_spinor_norm2(cola_ctx *c, cola_prec prec, const void *v_dev, int n_half, double *out_dev);
+
+/* The same |v|^2 for callers that cannot allocate device memory at all -- the only entry point of this library that needs
+ * neither a context (cola_create allocates a control block and pinned host memory) nor a lent workspace (someone has to
+ * allocate that too).  Who that is: code that is handed device pointers by a host application and nothing else, e.g.
+ * a callback running after the application's memory pool has claimed the whole GPU, so that a raw cudaMalloc would
+ * report out-of-memory; or a monitoring hook in a time-critical loop, where cudaMalloc / cudaFree are unwelcome
+ * because they synchronise the whole device.  Such a caller can still measure a source or a residual with this call.
+ *
+ * It runs the kernel of cola_spinor_norm2 with the reduction's scratch (per-block partials, tickets) in a fixed
+ * COLA_STATIC_SCRATCH_BYTES (16 KB) array that is part of libcola.so's device image: every GPU that loads the library
+ * carries it until the process exits.  The call itself performs no cudaMalloc, cudaFree or other allocating call; it
+ * issues one 36-byte cudaMemsetAsync (the tickets must start from zero, whatever an earlier call left behind) and one
+ * kernel on `stream`.  The result equals cola_spinor_norm2's bit for bit (same grid, same summation order).
+ *   device   CUDA device ordinal (0..63) the pointers belong to; made current for the call, the caller's device is restored
+ *   stream   cudaStream_t of that device to launch on, NULL = default stream.  Asynchronous: out_dev is valid once
+ *            the stream has reached this point
+ *   prec     COLA_F64 or COLA_F32
+ *   v_dev    DEVICE, n_sites sites of an internal buffer, i.e. 24 * n_sites reals, 16-byte aligned, owned by the caller
+ *   n_sites  1 .. COLA_STATIC_MAX_SITES (2^25 = the full 64^3x128 lattice of the largest configuration; the call is
+ *            tested up to that size and refuses more with COLA_EINVAL -- the scratch itself cannot overflow, the
+ *            kernel's grid is capped at 1184 blocks)
+ *   out_dev  DEVICE, one double, owned by the caller
+ * First use: the first call on each device looks up that device's address of the array (cudaGetSymbolAddress) and
+ * remembers it.  Make that first call during set-up, outside any stream capture.
+ * Sharing: all calls in the process use the same array, and it keeps what the last call wrote.  Two calls whose
+ * kernels can overlap on one GPU (different streams, different host threads) race on it and return garbage:
+ * order them on one stream or with events.  Calls on different GPUs do not interact.
+ * Errors: COLA_EINVAL (NULL pointer, n_sites = 0 or above the maximum, bad prec or device), COLA_ECUDA; the message is
+ * available from cola_last_error(NULL) in the calling thread. */
+#define COLA_STATIC_SCRATCH_BYTES 16384
+#define COLA_STATIC_MAX_SITES 33554432
+cola_status cola_spinor_norm2_static(int device, void *stream, cola_prec prec, const void *v_dev, size_t n_sites, double *out_dev);
 
 /* H3-H5, parity dslash: out_p = D_{p,1-p} in_{1-p}.  in, out: internal half-lattice DEVICE buffers
  * (in holds parity 1-p, out receives parity p); they must not overlap. */

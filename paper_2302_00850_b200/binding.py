@@ -33,6 +33,7 @@ EXPORTS = [
     "cola_schur_apply_mrhs", "cola_cg_solve_mrhs", "cola_set_l2_budget", "cola_selftest_host", "cola_cg_solve_history", "cola_profile_kernel", "cola_profile_result",
     "cola_set_features", "cola_clover_info", "cola_set_staging", "cola_set_compact", "cola_gauge_info_r8",
     "cola_eig_workspace_bytes", "cola_eig_lowest", "cola_cg_solve_deflated",
+    "cola_spinor_norm2", "cola_spinor_norm2_static",
 ]
 
 
@@ -97,6 +98,8 @@ def _load():
                                     ctypes.POINTER(ColaEigInfo)]
     lib.cola_cg_solve_deflated.argtypes = [vp, ctypes.POINTER(ColaSolveParams), vp, vp, ctypes.POINTER(ColaSolveInfo), vp, ctypes.POINTER(cd), ci]
     lib.cola_clover_info.argtypes = [vp, ctypes.POINTER(cd)]
+    lib.cola_spinor_norm2.argtypes = [vp, ci, vp, ci, vp]
+    lib.cola_spinor_norm2_static.argtypes = [ci, vp, ci, vp, ctypes.c_size_t, vp]
     lib.cola_spinor_bytes.argtypes = [vp, ci, ci]
     lib.cola_spinor_bytes.restype = ctypes.c_size_t
     lib.cola_workspace_bytes.argtypes = [vp]
@@ -143,6 +146,32 @@ def selftest_host() -> str:
     if st != COLA_OK:
         raise RuntimeError(buf.value.decode())
     return buf.value.decode()
+
+
+COLA_STATIC_SCRATCH_BYTES = 16384
+COLA_STATIC_MAX_SITES = 1 << 25
+
+
+def spinor_norm2_static(v: torch.Tensor, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """cola_spinor_norm2_static: |v|^2 of an internal spinor buffer without a context, a workspace or any allocation
+    inside the library (its reduction scratch is a fixed 16 KB array in the library's device image, shared by every
+    call in the process).  For callers that own device pointers but may not allocate.  `out`: a CUDA float64 tensor of
+    one element to receive the result (allocated here with torch when omitted -- pass it if even that is not allowed).
+    At most COLA_STATIC_MAX_SITES sites; the first call on a device should happen outside stream capture; calls that
+    overlap on one GPU race on the shared scratch."""
+    if not (v.is_cuda and v.is_contiguous() and v.dtype in (torch.float64, torch.float32)) or v.numel() % 24:
+        raise ValueError("v must be a contiguous CUDA float64 / float32 internal buffer (24 reals per site)")
+    if out is None:
+        out = torch.empty(1, dtype=torch.float64, device=v.device)
+    if not (out.is_cuda and out.dtype == torch.float64 and out.numel() >= 1 and out.device == v.device):
+        raise ValueError("out must be a CUDA float64 tensor on v's device")
+    if stream is None:
+        stream = torch.cuda.current_stream(v.device).cuda_stream
+    st = _lib.cola_spinor_norm2_static(v.device.index, ctypes.c_void_p(stream or 0), _PREC[v.dtype], ctypes.c_void_p(v.data_ptr()),
+                                       v.numel() // 24, ctypes.c_void_p(out.data_ptr()))
+    if st != COLA_OK:
+        raise ColaError(st, _lib.cola_last_error(None).decode())
+    return out
 
 
 class ColaError(RuntimeError):
@@ -323,6 +352,14 @@ class Cola:
         full = src.dim() == 4
         out = self.empty_internal(dp, full=full)
         self._ck(_lib.cola_spinor_convert(self._h, dp, ctypes.c_void_p(src.data_ptr()), ctypes.c_void_p(out.data_ptr()), 2 if full else 1))
+        return out
+
+    def spinor_norm2(self, v: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        """|v|^2 (fp64, deterministic) of a half-lattice or full internal buffer; returns a CUDA float64 tensor of one element."""
+        assert v.is_cuda and v.is_contiguous() and v.numel() in (self.Vh * 24, self.V * 24)
+        if out is None:
+            out = torch.empty(1, dtype=torch.float64, device=self.device)
+        self._ck(_lib.cola_spinor_norm2(self._h, _PREC[v.dtype], ctypes.c_void_p(v.data_ptr()), v.numel() // (self.Vh * 24), ctypes.c_void_p(out.data_ptr())))
         return out
 
     # ---- H3-H8.  fp32 tensors only: h16=True (or fmt="h16") selects COLA_F32_H16, the operator that reads 16-bit links and

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcola.so")
-SOURCES = ["cola_api.cu", "cola_dslash.cu", "cola_dslash_tile.cu", "cola_layout.cu", "cola_clover.cu", "cola_blas.cu", "cola_eig.cu"]
+SOURCES = ["cola_api.cu", "cola_dslash.cu", "cola_dslash_tile.cu", "cola_layout.cu", "cola_clover.cu", "cola_blas.cu", "cola_eig.cu", "cola_static.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "--use_fast_math=false",

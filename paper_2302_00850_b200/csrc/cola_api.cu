@@ -82,6 +82,8 @@ struct cola_ctx {
 };
 
 static thread_local char g_create_err[512] = "";
+// message slot of calls that have no context (cola_create, cola_spinor_norm2_static): what cola_last_error(NULL) returns
+void cola::set_thread_error(const char *msg) { snprintf(g_create_err, sizeof(g_create_err), "%s", msg); }
 static const int PROF_MAX = 4096;   // launches timed per profiling window
 
 static cola_status fail(cola_ctx *c, cola_status st, const char *fmt, const char *a = "", const char *b = "")
@@ -1840,6 +1842,15 @@ cola_status cola_schur_apply(cola_ctx *c, cola_prec prec, int dagger, const void
     ST(need_ready(c, "cola_schur_apply"));
     if (!in_even_dev || !out_even_dev || in_even_dev == out_even_dev) return fail(c, COLA_EINVAL, "cola_schur_apply: NULL or aliased buffers");
     return schur(c, prec, dagger ? 1 : 0, in_even_dev, out_even_dev, nullptr);
+}
+
+cola_status cola_spinor_norm2(cola_ctx *c, cola_prec prec, const void *v_dev, int n_half, double *out_dev)
+{
+    if (!c) return COLA_EINVAL;
+    if (!c->ws) return fail(c, COLA_ENOTREADY, "cola_spinor_norm2: no workspace (call cola_set_workspace)");
+    if (prec != COLA_F64 && prec != COLA_F32) return fail(c, COLA_EINVAL, "cola_spinor_norm2: prec must be COLA_F64 or COLA_F32");
+    if (!v_dev || !out_dev || (n_half != 1 && n_half != 2)) return fail(c, COLA_EINVAL, "cola_spinor_norm2: NULL pointer or n_half not 1 / 2");
+    return norm2(c, prec, v_dev, (size_t)n_half * c->Vh, out_dev);
 }
 
 cola_status cola_cg_solve(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info)

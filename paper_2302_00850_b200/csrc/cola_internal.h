@@ -118,6 +118,9 @@ struct HostStatusM {
 };
 struct MrhsList { int v[MRHS_MAX]; };
 
+// Record `msg` as this thread's context-free error message (returned by cola_last_error(NULL)).  Defined in cola_api.cu.
+void set_thread_error(const char *msg);
+
 constexpr unsigned REDUCE_GROUP = 256;
 __host__ __device__ inline size_t reduce_groups(size_t nblocks) { return (nblocks + REDUCE_GROUP - 1) / REDUCE_GROUP; }
 
