@@ -270,6 +270,11 @@ cola_status cola_cg_solve_history(cola_ctx *c, const cola_solve_params *sp, cons
  *   cheb_order    order p >= 1 of the Chebyshev polynomial T_p (p = 1: plain Lanczos on -H); default when 0: 24
  *   cheb_lo/hi    the filter maps [cheb_lo, cheb_hi] to [-1, 1]: eigenvalues below cheb_lo are amplified.  cheb_hi <= 0:
  *                 1.15 x a power-iteration estimate of the largest eigenvalue; cheb_lo <= 0: cheb_hi / 10.
+ *                 The window is verified after convergence: all n_ev returned eigenvalues must lie below cheb_lo (else
+ *                 fewer than n_ev modes were amplified, or a mode above cheb_hi was -- an even-order T_p amplifies those
+ *                 too -- and the returned pairs, though converged, would not be the lowest).  If not, the run is
+ *                 repeated with cheb_lo raised / cheb_hi widened (up to 3 times; info reports the window finally used
+ *                 and the total work); COLA_ENOCONV if that does not settle it.
  *   seed          of the deterministic start vector
  * Workspace: DEVICE, cola_eig_workspace_bytes(c, ep) bytes (n_kr + (n_kr + n_ev)/2 + 6 fp64 half-lattice vectors),
  * borrowed for the call.  evals_host / resid_host: HOST arrays of n_ev doubles (ascending eigenvalues, |H u - lambda u|

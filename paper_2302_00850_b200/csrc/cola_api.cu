@@ -1111,8 +1111,11 @@ extern "C" size_t cola_eig_workspace_bytes(const cola_ctx *c, const cola_eig_par
     return eig_plan(c, ep).total;
 }
 
-extern "C" cola_status cola_eig_lowest(cola_ctx *c, const cola_eig_params *ep, void *work_dev, size_t work_bytes, double *evals_host, double *resid_host,
-                                       void *evecs_dev, cola_eig_info *info)
+// One run of the filtered Lanczos with a given window.  After convergence the window is verified (see the end of the
+// function); if it was wrong the run is repeated with a corrected window, at most EIG_MAX_ATTEMPTS times in all.
+static const int EIG_MAX_ATTEMPTS = 4;
+static cola_status eig_lowest_run(cola_ctx *c, const cola_eig_params *ep, void *work_dev, size_t work_bytes, double *evals_host, double *resid_host,
+                                  void *evecs_dev, cola_eig_info *info, int attempt)
 {
     ST(need_ready(c, "cola_eig_lowest"));
     if (!ep || !work_dev || !evals_host || !resid_host || !info) return fail(c, COLA_EINVAL, "cola_eig_lowest: NULL argument");
@@ -1201,7 +1204,7 @@ extern "C" cola_status cola_eig_lowest(cola_ctx *c, const cola_eig_params *ep, v
     };
 
     memset(Tm, 0, sizeof(double) * m * m);
-    int k0 = 0, restarts = 0, converged = 0;
+    int k0 = 0, restarts = 0, converged = 0, raise_lo = 0;
     double beta_m = 0.0;
     for (;; restarts++) {
         for (int j = k0; j < m; j++) {
@@ -1232,6 +1235,13 @@ extern "C" cola_status cola_eig_lowest(cola_ctx *c, const cola_eig_params *ep, v
         }
         converged = worst <= q.tol * fabs(th[m - 1]);
         if (converged || restarts + 1 >= q.max_restarts) break;
+        // The n_ev-th largest Ritz value never exceeds the n_ev-th largest eigenvalue of T_p (interlacing).  If it is still
+        // inside [-1, 1] after several restarts, fewer than n_ev modes are likely to lie below cheb_lo, and the run would
+        // grind through max_restarts on the dense band: stop and repeat with a higher lower edge (see the end).
+        if (restarts >= 4 && th[m - n_ev] <= 1.0 && lo < 0.5 * hi && attempt + 1 < EIG_MAX_ATTEMPTS) {
+            raise_lo = 1;
+            break;
+        }
         // thick restart: keep the `keep` largest Ritz pairs and the last Lanczos vector
         for (int j = 0; j < m; j++)
             for (int q2 = 0; q2 < keep; q2++) Ysel[j * keep + q2] = Y[j * m + (m - 1 - q2)];
@@ -1246,6 +1256,22 @@ extern "C" cola_status cola_eig_lowest(cola_ctx *c, const cola_eig_params *ep, v
             Tm[q2 * m + keep] = Tm[keep * m + q2] = beta_m * Y[(m - 1) * m + (m - 1 - q2)];
         }
         k0 = keep;
+    }
+    if (raise_lo) {
+        EK(cudaEventRecord(c->ev1, c->stream));
+        EK(cudaEventSynchronize(c->ev1));
+        float ms0 = 0.f;
+        EK(cudaEventElapsedTime(&ms0, c->ev0, c->ev1));
+        cleanup();
+        cola_eig_params e2 = *ep;
+        e2.cheb_hi = hi;
+        e2.cheb_lo = (3.0 * lo < 0.5 * hi) ? 3.0 * lo : 0.5 * hi;
+        const int restarts0 = restarts + 1, ops0 = ops;
+        const cola_status st = eig_lowest_run(c, &e2, work_dev, work_bytes, evals_host, resid_host, evecs_dev, info, attempt + 1);
+        info->seconds += ms0 * 1e-3;
+        info->restarts += restarts0;
+        info->op_applications += ops0;
+        return st;
     }
     // final Ritz vectors of the wanted pairs -> R[0 .. n_ev), Rayleigh quotients and true residuals with H
     for (int j = 0; j < m; j++)
@@ -1286,7 +1312,36 @@ extern "C" cola_status cola_eig_lowest(cola_ctx *c, const cola_eig_params *ep, v
 #undef EK
 #undef ES
     if (!converged) return fail(c, COLA_ENOCONV, "cola_eig_lowest: max_restarts reached before the residual estimates met tol");
-    return COLA_OK;
+    // Was the window right?  The filter T_p maps eigenvalues of H below cheb_lo to values > 1, monotonically (smaller
+    // lambda, larger value), and [cheb_lo, cheb_hi] into [-1, 1]; the run returns the n_ev LARGEST Ritz pairs of T_p.
+    // Those are the n_ev smallest eigenpairs of H only if (a) at least n_ev eigenvalues lie below cheb_lo -- otherwise the
+    // list is padded with modes of the oscillating band, in no particular order -- and (b) nothing lies above cheb_hi -- an
+    // even-order T_p sends such modes to large positive values as well, and the power iteration behind the default cheb_hi
+    // only bounds lambda_max from below.  Both failures show in the Rayleigh quotients just computed with H itself: a
+    // returned lambda >= cheb_lo.  (The residuals are small either way, so they cannot tell.)
+    double lam_max = evals_host[n_ev - 1];
+    if (lam_max < lo) return COLA_OK;
+    cola_eig_params e2 = *ep;
+    e2.cheb_hi = hi;
+    e2.cheb_lo = lo;
+    if (lam_max > hi) e2.cheb_hi = 1.15 * lam_max;                        // (b): an eigenvalue above the window
+    else e2.cheb_lo = (2.0 * lam_max < 0.5 * hi) ? 2.0 * lam_max : 0.5 * (lam_max + hi);   // (a): raise the lower edge past it
+    if (!(e2.cheb_lo < e2.cheb_hi)) e2.cheb_lo = 0.5 * e2.cheb_hi;
+    if (attempt + 1 >= EIG_MAX_ATTEMPTS)
+        return fail(c, COLA_ENOCONV, "cola_eig_lowest: a returned eigenvalue lies at or above cheb_lo after the window was corrected repeatedly: "
+                                     "the pairs are converged eigenpairs of S^+S but not certified as the lowest; pass cheb_lo / cheb_hi explicitly");
+    const cola_eig_info first = *info;
+    const cola_status st = eig_lowest_run(c, &e2, work_dev, work_bytes, evals_host, resid_host, evecs_dev, info, attempt + 1);
+    info->seconds += first.seconds;          // account for every run
+    info->restarts += first.restarts;
+    info->op_applications += first.op_applications;
+    return st;
+}
+
+extern "C" cola_status cola_eig_lowest(cola_ctx *c, const cola_eig_params *ep, void *work_dev, size_t work_bytes, double *evals_host, double *resid_host,
+                                       void *evecs_dev, cola_eig_info *info)
+{
+    return eig_lowest_run(c, ep, work_dev, work_bytes, evals_host, resid_host, evecs_dev, info, 0);
 }
 
 extern "C" cola_status cola_cg_solve_deflated(cola_ctx *c, const cola_solve_params *sp, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *info,

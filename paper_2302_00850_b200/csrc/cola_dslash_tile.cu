@@ -246,11 +246,16 @@ __global__ void __launch_bounds__(TILE_MAX_THREADS, COLA_TILE_MINB) dslash_tile_
 template <int FMT, int XPAY, int POST>
 cudaError_t launch_one(const TileArgs &ta, dim3 grid, dim3 block, size_t smem, cudaStream_t s)
 {
-    static bool configured = false;   // per instantiation; the attribute is per device function, set once per process and device
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(dslash_tile_kernel<FMT, XPAY, POST>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    // The opt-in to > 48 KB of dynamic shared memory is an attribute of the function ON ONE DEVICE: keep the "done" flag
+    // per instantiation and per device (contexts on different devices share this code).
+    static bool configured[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
+        e = cudaFuncSetAttribute(dslash_tile_kernel<FMT, XPAY, POST>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
     }
     return launch_pdl_smem(dslash_tile_kernel<FMT, XPAY, POST>, grid, block, smem, s, ta);
 }
@@ -270,7 +275,7 @@ cudaError_t launch_tile_fmt(const TileArgs &ta, cudaStream_t s)
     if (xpay == 2 && post == 0) return launch_one<FMT, 2, 0>(ta, grid, block, smem, s);
     if constexpr (FMT != LINK_I16_12)
         if (xpay == 3 && post == 0) return launch_one<FMT, 3, 0>(ta, grid, block, smem, s);
-    return cudaErrorInvalidValue;
+    return cudaErrorNotSupported;   // combination not instantiated: the caller falls back to the direct kernel
 }
 
 }  // namespace
@@ -322,6 +327,9 @@ cudaError_t launch_dslash_tile(int fmt, const DslashArgs &a, cudaStream_t s)
     ta.nent = sh.nent;
     ta.stride = TILE_STRIDE;
     ta.ntiles = (g.Y / sh.TY) * (g.Z / sh.TZ) * (g.T / sh.TT);
+    // a fused norm writes one partial per tile: small tiles (Xh small, extents with few divisors) can mean more tiles
+    // than the reduction buffers have slots -- leave those launches to the direct kernel
+    if (a.red.partials && (unsigned)ta.ntiles > a.red.pstride) return cudaErrorNotSupported;
     ta.off_z = sh.TZ * sh.TT * (sh.TY + 2) * g.Xh;
     ta.off_t = ta.off_z + 2 * sh.TT * g.Xh * sh.TY;
     ta.dTX = make_fastdiv((unsigned)g.Xh);

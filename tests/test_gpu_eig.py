@@ -55,6 +55,29 @@ def test_lowest_modes_match_the_oracle(dims, n_ev):
     c.close()
 
 
+def test_a_wrong_filter_window_is_detected_and_corrected():
+    """The filter amplifies what lies below cheb_lo; the n_ev largest Ritz pairs of the filtered operator are the n_ev lowest
+    modes of H only if at least n_ev eigenvalues lie below cheb_lo and none above cheb_hi (an even-order Chebyshev
+    polynomial amplifies those as well).  Converged pairs from a wrong window have small residuals, so only the check of
+    the returned eigenvalues against the window tells; the library then corrects the window and repeats."""
+    dims, n_ev = (4, 4, 4, 4), 8
+    c, Un, A, Ainv, kappa = setup(dims)
+    want, _ = oracle.lowest_modes(dims, BC, Un, A, Ainv, kappa, n_ev + 2)
+    # (a) only two eigenvalues below cheb_lo, eight wanted
+    lo_req = 0.5 * (want[1] + want[2])
+    ev, _, info = c.eig_lowest(n_ev, tol=1e-11, cheb_lo=lo_req)
+    assert info["converged"] and info["cheb_lo"] > want[n_ev - 1] > lo_req, info
+    assert np.max(np.abs(np.asarray(ev) - want[:n_ev]) / want[:n_ev]) < 1e-8, (ev, want[:n_ev])
+    # (b) the upper edge below the top of the spectrum: the top modes come out first, are recognised, the edge is moved
+    ev0, _, info0 = c.eig_lowest(n_ev, tol=1e-11)
+    hi_req = 0.5 * info0["cheb_hi"] / 1.15
+    ev, _, info = c.eig_lowest(n_ev, tol=1e-11, cheb_hi=hi_req, cheb_lo=min(2.0 * want[n_ev], 0.5 * hi_req))
+    assert info["converged"] and info["cheb_hi"] > hi_req, info
+    assert np.max(np.abs(np.asarray(ev) - want[:n_ev]) / want[:n_ev]) < 1e-8, (ev, want[:n_ev])
+    assert info["op_applications"] > info0["op_applications"]          # the discarded run is accounted for
+    c.close()
+
+
 def test_plain_lanczos_and_parameter_checks():
     dims = (4, 4, 4, 4)
     c, Un, A, Ainv, kappa = setup(dims)

@@ -35,7 +35,8 @@ def test_residual_history_follows_the_oracle(dims, even_odd):
     # unpreconditioned M (cond ~ 10^3) the rounded recurrence loses conjugacy and LAGS the fp64 one; the derived bound is
     # "by less than one pass": the deviation stays below the largest residual reduction of a single fp64 pass
     # (the same bound pins the oracle's own float model in tests/test_oracle_pins.py).
-    one_pass = float(np.max(1.0 - h_ref[1:] / h_ref[:-1]))
+    # Capped: a single pass that happened to cut the residual by a large factor must not make the assertion empty.
+    one_pass = min(float(np.max(1.0 - h_ref[1:] / h_ref[:-1])), 0.25)
     for mixed, tol_rel in ((0, 1e-12), (1, 1e-4 if even_odd else one_pass), (2, 7e-2 if even_odd else one_pass)):
         x, info = c.cg_solve_history(b.cuda(), tol=1e-10, even_odd=even_odd, mixed=mixed)
         h = np.asarray(info["history"])
