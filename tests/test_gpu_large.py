@@ -258,3 +258,118 @@ def test_multi_rhs_operators_at_full_size(big):
         assert torch.equal(outs[n], c.schur_apply(full[n, 0].contiguous(), dagger=True))
     c.release_mrhs_workspace()
     torch.cuda.empty_cache()
+
+
+def oracle_checked_residual(big, b, x, info, note):
+    """b - M x evaluated by the ORACLE at the sampled sites against the library's residual field there, and the
+    library's reported true residual against the norm of that field (as test_mixed_precision_solve)."""
+    c, dims, cfg = big.ctx, big.dims, big.cfg
+    assert info["converged"] and info["true_residual"] <= 1.05e-10, (note, info)
+    # the oracle reads x only at the sampled sites and their neighbours: hand it the full array (host copy)
+    xn = x.cpu().numpy()
+    Mx = oracle.apply_sites(dims, inputs.BC, big.Un, cfg["kappa"], cfg["csw"], "M", xn, big.sites)
+    del xn
+    Mx_gpu = c.spinor_unpack(c.fermion_matrix_apply(c.spinor_pack(x)))
+    r_gpu_field = b - Mx_gpu
+    r_or = at_sites(b, big.sites) - Mx
+    r_gpu = at_sites(r_gpu_field, big.sites)
+    assert np.abs(r_or - r_gpu).max() <= 1e-12 * max(1.0, np.abs(Mx).max()), note
+    bnorm = float(torch.linalg.vector_norm(b).item())
+    glob = float(torch.linalg.vector_norm(r_gpu_field).item()) / bnorm
+    assert glob <= 1.05e-10 and abs(glob - info["true_residual"]) <= 1e-3 * glob + 1e-14, (note, glob, info["true_residual"])
+    del Mx_gpu, r_gpu_field
+    torch.cuda.empty_cache()
+
+
+def config_source(big, n=None):
+    dims, cfg, k = big.dims, big.cfg, big.k
+    if n is not None:
+        return inputs.source_point(dims, n % 4, n % 3, device="cuda")
+    if cfg["source"] == "point":
+        return inputs.source_point(dims, 1, 2, device="cuda")
+    return inputs.source_gaussian(dims, inputs.config_seed_source(k), device="cuda")
+
+
+@pytest.mark.parametrize("mixed", [1, 2])
+def test_bicgstab_at_full_size(big, mixed):
+    """BiCGStab on the Schur system in bench.py's launch configuration.  At these sizes the
+    reductions of its BLAS-1 kernels and of the <t, s> fused into the operator kernel (grid_sum_last_n) span many groups
+    of 256 blocks, a path the small lattices of test_gpu_bicgstab.py never take.  The solution is held to the oracle
+    through b - M x at the sampled sites; at 32^3x64 also to the stored solution of the ORACLE's CGNR solve."""
+    c, dims, k = big.ctx, big.dims, big.k
+    b = config_source(big)
+    x, info = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=mixed, method="bicgstab")
+    assert info["reliable_updates"] >= 1
+    oracle_checked_residual(big, b, x, info, ("bicgstab", k, mixed))
+    xc, infoc = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=mixed)
+    assert info["iters"] < infoc["iters"]                     # two S per pass against S and S^+, and fewer passes
+    assert rel(x.cpu().numpy(), xc.cpu().numpy()) < 5e-9
+    if k == 2:
+        g = json.load(open(GOLD))["2"]["eo"]
+        xs = x.cpu().numpy().reshape(-1, 12)[np.array(g["sites"])]
+        want = np.array(g["x_re"]) + 1j * np.array(g["x_im"])
+        assert np.linalg.norm(xs - want) / np.linalg.norm(want) < 5e-8
+
+
+@pytest.mark.parametrize("method", ["cgnr", "bicgstab"])
+def test_batched_solvers_at_full_size(big, method):
+    """cola_cg_solve_mrhs with 4 point sources at 32^3x64 and 48^3x96: the multi-rhs launches inside
+    a solve (z-banded sweep, per-system reductions over many block groups).  Each system: oracle-sampled residual, pass
+    count and solution against the sequential solver of the same system."""
+    c, dims, k = big.ctx, big.dims, big.k
+    if k == 4:
+        pytest.skip("64^3x128: the batched solver's workspace does not fit beside the 120 GB context")
+    nrhs = 4
+    c.set_mrhs_workspace(nrhs, for_solver=True)
+    srcs = [config_source(big, n) for n in range(nrhs)]
+    x, infos = c.cg_solve_mrhs(torch.stack(srcs), tol=1e-10, mixed=1, method=method)
+    for n in range(nrhs):
+        xs, info = c.cg_solve(srcs[n], tol=1e-10, even_odd=True, mixed=1, method=method)
+        if method == "cgnr":
+            assert abs(info["iters"] - infos[n]["iters"]) <= 1 and info["reliable_updates"] == infos[n]["reliable_updates"], (n, info, infos[n])
+        else:
+            assert abs(info["iters"] - infos[n]["iters"]) <= max(2, math.ceil(0.1 * info["iters"])), (n, info, infos[n])
+        assert rel(x[n].cpu().numpy(), xs.cpu().numpy()) < 5e-9
+        if n in (0, nrhs - 1):
+            oracle_checked_residual(big, srcs[n], x[n].contiguous(), infos[n], (method, k, n))
+        else:
+            assert infos[n]["converged"] and infos[n]["true_residual"] <= 1.05e-10
+    c.release_mrhs_workspace()
+    torch.cuda.empty_cache()
+
+
+def test_low_modes_and_deflated_start_at_full_size(big):
+    """cola_eig_lowest + cola_cg_solve_deflated at 32^3x64: the returned pairs satisfy H u = lambda u with H = S^+S applied
+    by the ORACLE at sampled even sites, and the deflated solve reaches the stored oracle solution."""
+    c, dims, cfg, k = big.ctx, big.dims, big.cfg, big.k
+    if k != 2:
+        pytest.skip("low modes: 32^3x64 only (DESIGN.md section 7)")
+    n_ev = 8                                                 # bench.py's low_modes configuration
+    ev, evecs, info = c.eig_lowest(n_ev, tol=1e-9)
+    assert info["converged"], info
+    ev = np.asarray(ev)
+    assert np.all(ev > 0) and np.all(np.diff(ev) >= 0) and max(info["residuals"]) < 1e-6 * info["cheb_hi"]
+    even = big.sites[big.par == 0]
+    args = (dims, inputs.BC, big.Un, cfg["kappa"], cfg["csw"])
+    full = torch.zeros((2, 12, c.Vh, 2), dtype=torch.float64, device="cuda")
+    for i in (0, n_ev - 1):
+        full[0] = evecs[i]
+        u = c.spinor_unpack(full)
+        Su = torch.zeros_like(full)
+        c.schur_apply(full[0], out=Su[0])                                    # S u on the GPU (fp64, oracle-verified above) ...
+        Su_c = c.spinor_unpack(Su)
+        Hu = oracle.apply_sites(*args, "Sdag", Su_c.cpu().numpy(), even)     # ... S^+ (S u) by the oracle at the sampled sites
+        Su_or = oracle.apply_sites(*args, "S", u.cpu().numpy(), even)
+        assert rel(at_sites(Su_c, even), Su_or) < 1e-12
+        lhs = Hu - ev[i] * at_sites(u, even)
+        # the sample's share of the residual cannot exceed the whole (|H u - lambda u| over all even sites, |u| = 1)
+        assert np.linalg.norm(lhs) <= info["residuals"][i] * (1 + 1e-6) + 1e-11, (i, np.linalg.norm(lhs), info["residuals"][i])
+        assert np.linalg.norm(at_sites(u, even)) > 0
+    b = config_source(big)
+    x0, i0 = c.cg_solve(b, tol=1e-10, even_odd=True, mixed=1)
+    x1, i1 = c.cg_solve_deflated(b, ev, evecs, tol=1e-10, mixed=1)
+    assert i1["converged"] and i1["true_residual"] <= 1.05e-10 and i1["iters"] <= i0["iters"]
+    g = json.load(open(GOLD))["2"]["eo"]
+    xs = x1.cpu().numpy().reshape(-1, 12)[np.array(g["sites"])]
+    want = np.array(g["x_re"]) + 1j * np.array(g["x_im"])
+    assert np.linalg.norm(xs - want) / np.linalg.norm(want) < 5e-8
