@@ -20,7 +20,8 @@ extras  : (N = 1 only) solve_h16 / solve_r8 = the same step with 16-bit links + 
           (mixed = 3) in the inner iteration; solve_bicgstab = the same step by BiCGStab on the Schur
           system and low_modes = the lowest modes of S^+S + the deflated step (NEXT-4); batched (config 3) = its 12 sources
           as one multi-rhs solve, CGNR and BiCGStab (NEXT-1); operators = every operator x {fp32 x12, fp64 x18, 16-bit,
-          8-real, fp32 x12 with the 72-real A}.  --operators-only [--nrhs N] [--lattice X,Y,Z,T] [--staging 1] is the short
+          8-real, fp32 x12 with the 72-real A, fp32 x18 on a second context}, each the median of 10 bursts;
+          compression_x12_vs_x18 = the 12-real and 18-real fp32 operators interleaved (what the compression buys).  --operators-only [--nrhs N] [--lattice X,Y,Z,T] [--staging 1] is the short
           launch sequence the ncu captures and the volume sweep in profiles/ come from; --ab-formats the interleaved
           comparison of the storage formats.
 N > 1   : replicas only (the path has no inter-GPU exchange): every rank solves its own
@@ -147,29 +148,38 @@ def aggregate_over_ranks(local_ms: float, local_units: float, device=None):
     return float(t.item()), float(u.item())
 
 
-def time_launches(fn, n_warm, n_timed):
-    """Average device time (ms) of fn() over n_timed calls, CUDA events on the current stream."""
+def time_launches(fn, n_warm, n_timed, bursts=10):
+    """Device time (ms) of one fn() call: the MEDIAN over `bursts` back-to-back bursts of n_timed / bursts calls each
+    (n_timed calls in all, SURVEY 8(d) "median of >= 200 timed launches"), each burst bracketed by CUDA events on the
+    current stream.  A median of bursts rather than a mean of everything: under the power cap the SM clock moves by ~10 %
+    within a run, and a mean folds that drift into whichever row happens to be measured at the time."""
     for _ in range(n_warm):
         fn()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    bursts = max(1, min(bursts, n_timed))
+    per = max(1, n_timed // bursts)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(bursts + 1)]
     torch.cuda.synchronize()
-    e0.record()
-    for _ in range(n_timed):
-        fn()
-    e1.record()
+    evs[0].record()
+    for k in range(bursts):
+        for _ in range(per):
+            fn()
+        evs[k + 1].record()
     torch.cuda.synchronize()
-    return e0.elapsed_time(e1) / n_timed
+    return statistics.median(evs[k].elapsed_time(evs[k + 1]) / per for k in range(bursts))
 
 
-def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
+def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0, only_fmt32=False):
     """Per-kernel throughput of the operator family, each timed alone (inputs larger than L2).
-    nrhs > 1 adds the multi-right-hand-side Schur operator over nrhs vectors."""
+    nrhs > 1 adds the multi-right-hand-side Schur operator over nrhs vectors.
+    only_fmt32: just the rows of the context's own fp32 link format (the second, 18-real context of the x12 / x18 comparison)."""
     peak, _ = measured_peaks()
     out = {}
     Vh = ctx.Vh
     fmts = [(torch.float32, fmt32), (torch.float64, "f64x18"), (torch.float32, "f32h16")]
     if fmt32 == "f32x12":   # the compact fields are measured against the 12-real links they replace
         fmts += [(torch.float32, "f32r8"), (torch.float32, "f32x12_a72")]
+    if only_fmt32:
+        fmts = fmts[:1]
     for prec, fmt in fmts:
         full = ctx.empty_internal(prec, full=True).normal_()
         dst = ctx.empty_internal(prec, full=True)
@@ -212,6 +222,38 @@ def operator_table(ctx, fmt32, n_warm=20, n_timed=200, nrhs=0):
             ctx.release_mrhs_workspace()
             torch.cuda.empty_cache()
     ctx.set_compact(3)
+    return out
+
+
+def x12_vs_x18(ctx12, ctx18, rounds=10, burst=20):
+    """What the 12-real link compression of BJ:ns buys on B200 ("additional computation in order to reduce traffic"):
+    the same fp32 operators on a 12-real and an 18-real context over the same links, interleaved in short bursts, medians."""
+    out = {}
+    bufs = {}
+    for key, c in (("x12", ctx12), ("x18", ctx18)):
+        bufs[key] = (c, c.empty_internal(torch.float32, full=True).normal_(), c.empty_internal(torch.float32, full=True))
+    ops = {"dslash": lambda c, a, d: c.dslash_apply(0, a[1], out=d[0]),
+           "fermion_matrix": lambda c, a, d: c.fermion_matrix_apply(a, out=d),
+           "schur": lambda c, a, d: c.schur_apply(a[0], out=d[0])}
+    kinds = {"dslash": ("dslash", 1), "fermion_matrix": ("dslash_clover_xpay", 2), "schur": (None, 2)}
+    res = {(o, k): [] for o in ops for k in bufs}
+    for _ in range(rounds):
+        for o, fn in ops.items():
+            for k, (c, a, d) in bufs.items():
+                res[(o, k)].append(time_launches(lambda: fn(c, a, d), 3, burst, bursts=1))
+    peak, _ = measured_peaks()
+    for o in ops:
+        row = {}
+        for k in bufs:
+            ms = statistics.median(res[(o, k)][2:])
+            fmt = "f32" + k
+            kind, launches = kinds[o]
+            nb = (BYTES["dslash_clover_inv"][fmt] + BYTES["dslash_clover_xpay"][fmt]) if kind is None else BYTES[kind][fmt] * launches
+            row[k] = {"ms": round(ms, 5), "GB/s": round(nb * ctx12.Vh / (ms * 1e-3) / 1e9, 1), "frac_measured": round(nb * ctx12.Vh / (ms * 1e-3) / 1e9 / peak, 4)}
+        row["time_x18_over_x12"] = round(row["x18"]["ms"] / row["x12"]["ms"], 3)
+        fmt_b = lambda f: (BYTES["dslash_clover_inv"][f] + BYTES["dslash_clover_xpay"][f]) if kinds[o][0] is None else BYTES[kinds[o][0]][f] * kinds[o][1]
+        row["bytes_x18_over_x12"] = round(fmt_b("f32x18") / fmt_b("f32x12"), 3)
+        out[o] = row
     return out
 
 
@@ -409,6 +451,7 @@ def main():
     ap.add_argument("--operators-only", action="store_true",
                     help="profiling aid: skip the solves, run only the operator table (few launches: --op-warm/--op-timed) and print it")
     ap.add_argument("--lattice", default="", help="test aid: run the config's recipe on other extents, e.g. 16,16,16,32")
+    ap.add_argument("--no-x18", action="store_true", help="skip the 18-real fp32 operator rows and the interleaved 12-real / 18-real comparison")
     ap.add_argument("--no-h16", action="store_true", help="skip the extra solve with 16-bit links/clover in the inner iteration")
     ap.add_argument("--no-bicgstab", action="store_true", help="skip the extra solves by BiCGStab on the Schur system")
     ap.add_argument("--no-eig", action="store_true", help="skip the low-mode solve and the deflated step")
@@ -419,6 +462,7 @@ def main():
     ap.add_argument("--staging", type=int, default=0, choices=[0, 1],
                     help="kernel family of the fp32 / 16-bit single-rhs operators: 0 direct global loads (default), 1 neighbour spinors staged in shared memory")
     ap.add_argument("--ab-formats", action="store_true", help="measurement aid: interleaved A/B of the fp32 link / clover storage formats, then exit")
+    ap.add_argument("--bicgstab-only", action="store_true", help="measurement aid: one mixed-precision BiCGStab solve, then exit")
     ap.add_argument("--timeline", action="store_true", help="measurement aid: device timestamps of the kernels of three consecutive iterations, then exit")
     ap.add_argument("--op-warm", type=int, default=20)
     ap.add_argument("--op-timed", type=int, default=200)
@@ -510,6 +554,10 @@ def main():
         return fl, infos
 
     b = source(0) if n_src == 1 else None
+    if args.bicgstab_only:    # not a bench line: one BiCGStab solve, the launch sequence the ncu captures of its kernels come from
+        x_, inf_ = ctx.cg_solve(b if b is not None else source(0), tol=1e-10, even_odd=True, mixed=1, method="bicgstab")
+        print(json.dumps({"bicgstab_only": True, "lattice": list(dims), "iters": inf_["iters"], "true_residual": inf_["true_residual"]}))
+        return
     if args.timeline:         # not a bench line: kernel start times of three consecutive iterations (profiles/r2_timeline.md)
         print(json.dumps({"timeline": True, "lattice": list(dims), **timeline(ctx, b if b is not None else source(0))}))
         return
@@ -709,6 +757,26 @@ def main():
     # ---- roofline of the dominant kernel + operator table (rank 0, kernels timed alone)
     peak, peak_src = measured_peaks()
     table = {} if (args.no_operator_table or world > 1) else operator_table(ctx, "f32x12", n_warm=args.op_warm, n_timed=args.op_timed)
+    # ---- the fp32 x18 column of SURVEY 8(d) and what 12-real compression buys (second context on the same links)
+    compression = None
+    if table and rank == 0 and not args.no_x18:
+        try:
+            c18 = binding.Cola(dims, cfg["kappa"], cfg["csw"], bc=inputs.BC, compress12=False, device=local, features=binding.COLA_FEAT_FULL_M)
+            need = c18.workspace_bytes() + inputs.volume(dims) * (4 * 18 * 8 + 4 * 24 * 4) + (2 << 30)
+            if torch.cuda.mem_get_info(dev)[0] > need:
+                U18 = inputs.make_links(args.config, dims=dims, device=dev)
+                c18.gauge_upload(U18)
+                del U18
+                torch.cuda.empty_cache()
+                table.update(operator_table(c18, "f32x18", n_warm=args.op_warm, n_timed=args.op_timed, only_fmt32=True))
+                compression = x12_vs_x18(ctx, c18)
+            else:
+                compression = {"unavailable": "a second (18-real) context does not fit beside the first on this lattice"}
+            c18.close()
+            del c18
+            torch.cuda.empty_cache()
+        except (RuntimeError, binding.ColaError) as ex:
+            compression = {"unavailable": str(ex)[:200]}
     roof = None
     if table:
         k = table["fermion_matrix_f32x12"]   # two launches of the fused dslash + clover + xpay kernel
@@ -737,6 +805,10 @@ def main():
                     "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": in_solve["avg_launch_ms"],
                     "traffic": ncu_traffic(dims)[0]}
         roof["in_solve"] = in_solve
+        # the same three figures as flat keys (a record that keeps only the top level of `roofline` still has them)
+        roof["in_solve_avg_launch_ms"] = in_solve["avg_launch_ms"]
+        roof["in_solve_frac"] = in_solve["frac"]
+        roof["in_solve_launches"] = in_solve["launches"]
     cpu = None
     if U_cpu is not None:
         cpu = cpu_baseline_sample(dict(cfg, dims=cpu_dims), U_cpu)
@@ -759,6 +831,7 @@ def main():
         line["solve"]["iters_per_source"] = [i["iters"] for i in infos]
         line["solve"]["max_true_residual"] = max(i["true_residual"] for i in infos)
         line["batched"] = batched
+    line["compression_x12_vs_x18"] = compression
     line["solve_h16"] = solve_h16
     line["solve_r8"] = solve_r8
     line["solve_delta_0.01"] = solve_delta

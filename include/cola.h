@@ -98,7 +98,7 @@ const char *cola_last_error(const cola_ctx *c);
  * (all right-hand sides of a launch) exceed this budget the thread blocks sweep the lattice in bands of z-planes
  * instead of slice by slice, which keeps the reuse inside L2.  Results do not depend on it. */
 cola_status cola_set_l2_budget(cola_ctx *c, size_t bytes);
-/* Optional parts of the workspace (the fields are ~7.3 KB per even site with everything on: 125 GB at 64^3x128).
+/* Optional parts of the workspace (the fields are ~8.0 KB per even site with everything on: 134 GB at 64^3x128).
  * Call before cola_workspace_bytes / cola_set_workspace (it un-lends the workspace and invalidates the gauge field).
  * Default: COLA_FEAT_ALL.
  *   COLA_FEAT_FULL_M  fp32 (and fp16) copies of A on the ODD parity and the larger solver scratch: needed by
@@ -113,17 +113,6 @@ cola_status cola_set_l2_budget(cola_ctx *c, size_t bytes);
  * A call that needs a missing feature returns COLA_EINVAL. */
 typedef enum { COLA_FEAT_FULL_M = 1, COLA_FEAT_H16 = 2, COLA_FEAT_R8 = 4, COLA_FEAT_A72 = 8, COLA_FEAT_ALL = 15 } cola_feature;
 cola_status cola_set_features(cola_ctx *c, unsigned features);
-/* Tuning: which kernel family the single-right-hand-side fp32 / 16-bit operators use.  0: every thread loads its 8
- * neighbour spinors from global memory through L1; 1: a thread block owns a 4-D tile of sites and stages the tile's
- * input spinors and its six faces in shared memory with cp.async, so that neighbours are read with LDS (BJ:ns
- * "shared-memory ... staging of neighbour half-spinors").  Operator results are bit-identical in
- * both modes (fused norms differ in summation order).  fp64 operators and lattices the tiles do not fit (X > 512) use
- * mode 0 regardless.  Default: DESIGN.md section 6 says which and why. */
-cola_status cola_set_staging(cola_ctx *c, int mode);
-/* Measurement aid.  bit 0: COLA_F32_R8 reads the 8-real links (else the context's fp32 links, 12 or 18 reals, i.e. it is
- * COLA_F32); bit 1: the fp32 operators (COLA_F32, COLA_F32_R8) read A in its 48-real form (else the 72-real packed blocks,
- * which needs COLA_FEAT_A72).  Default 3.  COLA_EINVAL outside 0..3. */
-cola_status cola_set_compact(cola_ctx *c, int mask);
 /* Change the stream subsequent calls launch on. */
 cola_status cola_set_stream(cola_ctx *c, void *stream);
 
@@ -233,7 +222,8 @@ typedef struct {
     int method;        /* COLA_CGNR (0, the north_star solver) or COLA_BICGSTAB: BiCGStab in van der
                           Vorst's order on the Schur system (needs even_odd = 1), x0 = 0, shadow residual = r0; one pass =
                           two applications of S (CGNR: S and S^+), `iters` counts passes.  COLA_EINVAL on breakdown
-                          (<rhat, v>, <t, t> or rho vanishing).  Mixed precision and reliable updates as for CGNR. */
+                          (<rhat, v> or rho vanishing).  t = S s = 0 is not one: the half step x + alpha p is then the
+                          exact solution and the pass ends with omega = 0.  Mixed precision and reliable updates as for CGNR. */
 } cola_solve_params;
 typedef enum { COLA_CGNR = 0, COLA_BICGSTAB = 1 } cola_method;
 
@@ -335,11 +325,28 @@ cola_status cola_schur_apply_mrhs(cola_ctx *c, cola_prec prec, int dagger, int n
  * BiCGStab's kernels, one system after the other.  b_canon_dev / x_canon_dev: nrhs
  * canonical complex128 DEVICE arrays back to back (b and x must not overlap; during the call x also holds the
  * solver's internal iterates, its final content is the canonical solution); infos: HOST array of nrhs entries
- * (seconds = time of the whole batch).  COLA_ENOCONV if any system hit max_iter (its info has the last residual).  COLA_ENOTREADY without a
+ * (seconds = time of the whole batch).  COLA_ENOCONV if any system hit max_iter (its info has the last residual).
+ * COLA_EINVAL if BiCGStab broke down in a system: only that system leaves the batch (x = its iterate at its last
+ * reliable update, info filled, converged by its true_residual or not), the others are solved as usual.  COLA_ENOTREADY without a
  * multi-rhs workspace for nrhs systems. */
 cola_status cola_cg_solve_mrhs(cola_ctx *c, const cola_solve_params *sp, int nrhs, const void *b_canon_dev, void *x_canon_dev, cola_solve_info *infos);
 
-/* Measurement aid: with enable != 0 every later launch of the fused dslash + clover + xpay kernel in fp32 / 16-bit
+/* ==== Measurement and tuning aids =====================================================================================
+ * Not part of the method: switches and counters that bench.py and the A/B experiments of DESIGN.md section 6 use.  None of
+ * them changes what an operator or solver computes (bit-identical results, except the summation order of fused norms
+ * under cola_set_staging). */
+
+/* Which kernel family the single-right-hand-side fp32 / 16-bit operators use.  0 (default; DESIGN.md section 6 says why):
+ * every thread loads its 8 neighbour spinors from global memory through L1; 1: a thread block owns a 4-D tile of sites and
+ * stages the tile's input spinors and its six faces in shared memory with bulk asynchronous copies, so that neighbours are
+ * read with LDS (BJ:ns "shared-memory ... staging of neighbour half-spinors").  fp64 operators and lattices the tiles do
+ * not fit (X > 512) use mode 0 regardless. */
+cola_status cola_set_staging(cola_ctx *c, int mode);
+/* bit 0: COLA_F32_R8 reads the 8-real links (else the context's fp32 links, 12 or 18 reals, i.e. it is COLA_F32); bit 1:
+ * the fp32 operators (COLA_F32, COLA_F32_R8) read A in its 48-real form (else the 72-real packed blocks, which needs
+ * COLA_FEAT_A72).  Default 3.  COLA_EINVAL outside 0..3. */
+cola_status cola_set_compact(cola_ctx *c, int mask);
+/* With enable != 0 every later launch of the fused dslash + clover + xpay kernel in fp32 / 16-bit
  * (Schur kernel 2 / M: the dominant kernel of a mixed-precision solve) is bracketed by a pair of CUDA events on the
  * context's stream, up to 4096 launches; cola_profile_result synchronises, returns the average duration in ms of the
  * launches that did work, their count and the number of speculative launches that returned at once, and clears the
@@ -352,7 +359,7 @@ cola_status cola_profile_result(cola_ctx *c, double *avg_ms, int *count, int *sk
  * NULL) receives "ok" or the first failure.  COLA_OK or COLA_EINVAL. */
 cola_status cola_selftest_host(char *msg, size_t msg_len);
 
-/* Benchmark aid: number of kernels this context has launched since creation. */
+/* Measurement aid: number of kernels this context has launched since creation (bench.py's gpu_launches). */
 unsigned long long cola_launch_count(const cola_ctx *c);
 
 #ifdef __cplusplus

@@ -11,8 +11,7 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# COLA_LIBRARY_PATH selects another build of the same ABI (kernel-tuning experiments); default: the in-tree library
-_LIB_PATH = os.environ.get("COLA_LIBRARY_PATH") or os.path.join(_HERE, "libcola.so")
+_LIB_PATH = os.path.join(_HERE, "libcola.so")   # the in-tree library, nothing else: no environment variables are read
 
 COLA_OK, COLA_EINVAL, COLA_ECUDA, COLA_ENOTREADY, COLA_ENOCONV, COLA_ENOMEM = range(6)
 COLA_F64, COLA_F32, COLA_F32_H16, COLA_F32_R8 = 0, 1, 2, 3

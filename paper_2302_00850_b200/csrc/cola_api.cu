@@ -1550,6 +1550,7 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
     const char *Ball = (const char *)b_canon_dev;
     double bb[MRHS_MAX], bnorm[MRHS_MAX], target2[MRHS_MAX], rr[MRHS_MAX], flops[MRHS_MAX];
     int conv[MRHS_MAX], iters[MRHS_MAX], updates[MRHS_MAX];
+    int broken[MRHS_MAX] = {0};   // BiCGStab: systems whose recurrence produced NaN / Inf (dropped from the batch)
     memset(infos, 0, sizeof(cola_solve_info) * nrhs);
     CK(cudaEventRecord(c->ev0, c->stream));
 
@@ -1640,8 +1641,10 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
                 rr[n] = c->h_statb[n].rr;
                 iters[n] = k + 1;
                 flops[n] += 2 * flops_K;
-                if (!(rr[n] <= DBL_MAX))
-                    return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: BiCGStab broke down or met NaN/Inf (<rhat, v>, <t, t> or rho vanished, or bad input)");
+                if (!(rr[n] <= DBL_MAX)) {   // this system broke down: it leaves the batch with its last fp64 iterate, the others go on
+                    broken[n] = 1;
+                    continue;
+                }
                 if (c->h_statb[n].flag) S[ns++] = n;
             }
             if (ns > 0) {   // reliable updates of the systems that asked for one (or converged in the inner precision)
@@ -1678,7 +1681,7 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
             }
             int na2 = 0;
             for (int j = 0; j < na; j++)
-                if (!conv[A[j]]) A[na2++] = A[j];
+                if (!conv[A[j]] && !broken[A[j]]) A[na2++] = A[j];
             na = na2;
             if (na == 0 || !more) break;
             for (int j = 0; j < na; j++) {   // p = r + beta (p - omega v)
@@ -1804,6 +1807,10 @@ static cola_status solve_mrhs_impl(cola_ctx *c, const cola_solve_params *sp, int
     float ms = 0.f;
     CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
     for (int n = 0; n < nrhs; n++) infos[n].seconds = ms * 1e-3;
+    for (int n = 0; n < nrhs; n++)
+        if (broken[n])
+            return fail(c, COLA_EINVAL, "cola_cg_solve_mrhs: BiCGStab broke down or met NaN/Inf in at least one system (<rhat, v>, <t, t> or rho vanished, or bad input); "
+                                        "its x is the iterate of its last reliable update (see its info), the other systems were solved");
     if (!all_conv) return fail(c, COLA_ENOCONV, "cola_cg_solve_mrhs: max_iter reached before |r| <= tol*|b| for every system");
     return COLA_OK;
 }

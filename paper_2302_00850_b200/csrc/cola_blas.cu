@@ -153,7 +153,13 @@ __device__ __forceinline__ void cdot_acc(const double2 &a, const double2 &b, dou
     re += a.x * b.x + a.y * b.y;
     im += a.x * b.y - a.y * b.x;
 }
-__device__ __forceinline__ Cx bicg_omega(const CtlB *ctl) { return Cx{ctl->ts[0] / ctl->tt, ctl->ts[1] / ctl->tt}; }
+// omega = <t, s> / <t, t>.  t = S s vanishes only with s (S is non-singular): the half step x + alpha p already solves the
+// system exactly.  omega = 0 then completes the pass with x += alpha p, r = s = 0 instead of 0/0.
+__device__ __forceinline__ Cx bicg_omega(const CtlB *ctl)
+{
+    if (ctl->tt == 0.0) return Cx{0.0, 0.0};
+    return Cx{ctl->ts[0] / ctl->tt, ctl->ts[1] / ctl->tt};
+}
 // beta = (rho_next / rho) (alpha / omega), alpha = rho / rv  =>  beta = rho_next / (rv omega)
 __device__ __forceinline__ void bicg_set_beta(CtlB *ctl, const double (&rho_next)[2])
 {

@@ -19,7 +19,7 @@ namespace cola {
 namespace {
 
 // Tuning knobs (compile-time).  Defaults = best of the round-1 sweeps on B200: 64 threads per
-// block; fp32 kernels software-pipelined over the hops (COLA_PIPE) with 128 registers (8 blocks = 16 warps per SM);
+// block; fp32 kernels software-pipelined two hops ahead with 128 registers (8 blocks = 16 warps per SM);
 // fp64 kernels unpipelined at 168 registers (6 blocks = 12 warps per SM).  Without pipelining the best fp32 point was
 // 80 registers (12 blocks): the kernels are bound by bytes in flight, which either more warps or loads issued ahead of
 // use provide; two hops ahead at 16 warps beats 24 warps without by 5-9 % (one hop ahead: 4-8 %).
@@ -31,9 +31,6 @@ namespace {
 #endif
 #ifndef COLA_DSLASH_MINB_F64
 #define COLA_DSLASH_MINB_F64 6
-#endif
-#ifndef COLA_PIPE
-#define COLA_PIPE 2   // 0: hop by hop; 1: loads one hop ahead; 2: two hops ahead (two spinor/link buffers), +1-2 % over 1
 #endif
 constexpr int DSLASH_BLOCK = COLA_DSLASH_BLOCK;
 template <int FMT> struct MinBlocks { static constexpr int value = (FMT == LINK_F64_18) ? COLA_DSLASH_MINB_F64 : COLA_DSLASH_MINB_F32; };
@@ -65,44 +62,6 @@ __device__ __forceinline__ void hop_pipe(const void *in, const char *gauge_next,
         load_reals<T, 24, false>(in, Vh, nb_next, psi);
         load_raw_link<FMT, STREAM>(gauge_next, Vh, li_next, raw);
     }
-    su3_mul<BACK>(u, h, g);
-    reconstruct_accumulate<MU>(g, eta, s, acc);
-}
-
-// COLA_PIPE == 3: the neighbour spinors of the coming hops are fetched with asynchronous copies into a per-thread FIFO in
-// shared memory ([slot][chunk][thread]: conflict-free, no barrier: a thread reads back only what it copied itself),
-// FIFO_DEPTH hops ahead, instead of into registers one or two hops ahead; the raw links stay register-pipelined two hops
-// ahead.  Loads in flight then cost shared memory, not registers.
-#ifndef COLA_FIFO_DEPTH
-#define COLA_FIFO_DEPTH 4
-#endif
-constexpr int FIFO_DEPTH = COLA_FIFO_DEPTH;
-__device__ __forceinline__ void fifo_issue(float4 *fifo, const int slot, const void *in, const size_t Vh, const int nb)
-{
-    const float4 *src = reinterpret_cast<const float4 *>(in) + nb;
-#pragma unroll
-    for (int k = 0; k < 6; k++) cp_async16(&fifo[(slot * 6 + k) * DSLASH_BLOCK + threadIdx.x], src + (size_t)k * Vh);
-    cp_async_commit();
-}
-template <int FMT, int H, bool STREAM, typename T>
-__device__ __forceinline__ void hop_fifo(float4 *fifo, const void *in, const int nb_refill, const char *gauge_next2, size_t Vh, int li_next2, RawLink<FMT> &raw,
-                                         T eta, T s, T (&acc)[24])
-{
-    constexpr int MU = H >> 1;
-    constexpr bool BACK = (H & 1) != 0;
-    constexpr int issued = (H + FIFO_DEPTH < 8) ? H + FIFO_DEPTH : 8;   // groups committed before this hop's wait
-    T psi[24], h[12], g[12], u[18];
-    cp_async_wait<issued - 1 - H>();
-    constexpr int slot = H % FIFO_DEPTH;
-#pragma unroll
-    for (int k = 0; k < 6; k++) {
-        const float4 v = fifo[(slot * 6 + k) * DSLASH_BLOCK + threadIdx.x];
-        psi[4 * k] = v.x; psi[4 * k + 1] = v.y; psi[4 * k + 2] = v.z; psi[4 * k + 3] = v.w;
-    }
-    project<MU>(psi, s, h);
-    if (H + FIFO_DEPTH < 8) fifo_issue(fifo, slot, in, Vh, nb_refill);   // hop H + FIFO_DEPTH takes the slot just read
-    expand_link<FMT>(raw, u);
-    if (H < 6) load_raw_link<FMT, STREAM>(gauge_next2, Vh, li_next2, raw);
     su3_mul<BACK>(u, h, g);
     reconstruct_accumulate<MU>(g, eta, s, acc);
 }
@@ -155,35 +114,11 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
 #pragma unroll
         for (int k = 0; k < 24; k++) acc[k] = 0;
 
-#if COLA_PIPE
         if constexpr (FMT != LINK_F64_18) {
-            // software-pipelined hops: the loads of hop h+1 (neighbour spinor and raw link) are issued right after the
+            // software-pipelined hops: the loads of hop h+2 (neighbour spinor and raw link) are issued right after the
             // projection of hop h, whose spinor registers are dead by then, so they are in flight during the SU(3)
-            // multiply and the accumulation of hop h
-#if COLA_PIPE == 3
-            if constexpr (STREAM) {
-                extern __shared__ float4 cola_fifo[];
-                const int nbs[8] = {xf, xb, yf, yb, zf, zb, tf, tb};
-                RawLink<FMT> rawA, rawB;
-                load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, rawA);
-                load_raw_link<FMT, STREAM>(gq + 0 * lb, Vh, xb, rawB);
-                if (PDLW) {
-                    pdl_wait();
-                    if (a.skip && *a.skip) return -1.0;
-                }
-#pragma unroll
-                for (int h = 0; h < FIFO_DEPTH; h++) fifo_issue(cola_fifo, h, in, Vh, nbs[h]);
-                hop_fifo<FMT, 0, STREAM>(cola_fifo, in, nbs[(0 + FIFO_DEPTH) & 7], gp + 1 * lb, Vh, i, rawA, ex_f, sf, acc);
-                hop_fifo<FMT, 1, STREAM>(cola_fifo, in, nbs[(1 + FIFO_DEPTH) & 7], gq + 1 * lb, Vh, yb, rawB, ex_b, sb, acc);
-                hop_fifo<FMT, 2, STREAM>(cola_fifo, in, nbs[(2 + FIFO_DEPTH) & 7], gp + 2 * lb, Vh, i, rawA, ey_f, sf, acc);
-                hop_fifo<FMT, 3, STREAM>(cola_fifo, in, nbs[(3 + FIFO_DEPTH) & 7], gq + 2 * lb, Vh, zb, rawB, ey_b, sb, acc);
-                hop_fifo<FMT, 4, STREAM>(cola_fifo, in, nbs[(4 + FIFO_DEPTH) & 7], gp + 3 * lb, Vh, i, rawA, ez_f, sf, acc);
-                hop_fifo<FMT, 5, STREAM>(cola_fifo, in, nbs[(5 + FIFO_DEPTH) & 7], gq + 3 * lb, Vh, tb, rawB, ez_b, sb, acc);
-                hop_fifo<FMT, 6, STREAM>(cola_fifo, in, nbs[(6 + FIFO_DEPTH) & 7], nullptr, Vh, 0, rawA, et_f, sf, acc);
-                hop_fifo<FMT, 7, STREAM>(cola_fifo, in, nbs[(7 + FIFO_DEPTH) & 7], nullptr, Vh, 0, rawB, et_b, sb, acc);
-            } else
-#endif
-#if COLA_PIPE >= 2
+            // multiplies and accumulations of hops h and h+1.  (Hop by hop, one hop ahead and a shared-memory FIFO
+            // fed by asynchronous copies were measured and dropped: profiles/r3_experiments.md.)
             {
             // two hops ahead: buffers A (even hops) and B (odd hops); hop h refills its buffer with hop h+2
             T psiA[24], psiB[24];
@@ -210,22 +145,7 @@ __device__ __forceinline__ double dslash_site(const DslashArgs &a, const int i, 
             hop_pipe<FMT, 6, STREAM, 6>(in, nullptr, Vh, 0, 0, psiA, rawA, et_f, sf, acc);
             hop_pipe<FMT, 7, STREAM, 6>(in, nullptr, Vh, 0, 0, psiB, rawB, et_b, sb, acc);
             }
-#else
-            T psi[24];
-            RawLink<FMT> raw;
-            load_reals<T, 24, false>(in, Vh, xf, psi);
-            load_raw_link<FMT, STREAM>(gp + 0 * lb, Vh, i, raw);
-            hop_pipe<FMT, 0, STREAM>(in, gq + 0 * lb, Vh, xb, xb, psi, raw, ex_f, sf, acc);
-            hop_pipe<FMT, 1, STREAM>(in, gp + 1 * lb, Vh, yf, i, psi, raw, ex_b, sb, acc);
-            hop_pipe<FMT, 2, STREAM>(in, gq + 1 * lb, Vh, yb, yb, psi, raw, ey_f, sf, acc);
-            hop_pipe<FMT, 3, STREAM>(in, gp + 2 * lb, Vh, zf, i, psi, raw, ey_b, sb, acc);
-            hop_pipe<FMT, 4, STREAM>(in, gq + 2 * lb, Vh, zb, zb, psi, raw, ez_f, sf, acc);
-            hop_pipe<FMT, 5, STREAM>(in, gp + 3 * lb, Vh, tf, i, psi, raw, ez_b, sb, acc);
-            hop_pipe<FMT, 6, STREAM>(in, gq + 3 * lb, Vh, tb, tb, psi, raw, et_f, sf, acc);
-            hop_pipe<FMT, 7, STREAM>(in, nullptr, Vh, 0, 0, psi, raw, et_b, sb, acc);
-#endif
         } else
-#endif
         {
         hop<FMT, 0, false, STREAM>(in, gp + 0 * lb, Vh, xf, i, ex_f, sf, acc);
         hop<FMT, 0, true, STREAM>(in, gq + 0 * lb, Vh, xb, xb, ex_b, sb, acc);
@@ -385,7 +305,7 @@ __device__ __forceinline__ unsigned sweep_run(const Sweep &w, const Geom &g, uns
 template <int FMT, int XPAY, int POST, bool DOT = false>
 __global__ void __launch_bounds__(DSLASH_BLOCK, MinBlocks<FMT>::value) dslash_kernel(const __grid_constant__ DslashArgs a)
 {
-    constexpr bool LATE_WAIT = (FMT == LINK_I16_12) && (COLA_PIPE >= 2);   // see dslash_site<.., PDLW>
+    constexpr bool LATE_WAIT = (FMT == LINK_I16_12);   // see dslash_site<.., PDLW>
     pdl_trigger();
     if (!LATE_WAIT) {
         pdl_wait();
@@ -547,7 +467,7 @@ cudaError_t launch_fmt(const DslashArgs &a, cudaStream_t s)
     const int xpay = a.y ? (a.clov_y ? (a.clov_y_g48 ? 3 : 2) : 1) : 0;
     const int post = a.clov_post ? 1 : 0;
     const dim3 grid((a.g.Vh + DSLASH_BLOCK - 1) / DSLASH_BLOCK), block(DSLASH_BLOCK);
-    const size_t sm = (COLA_PIPE == 3 && FMT != LINK_F64_18) ? (size_t)FIFO_DEPTH * 6 * DSLASH_BLOCK * 16 : 0;   // the spinor FIFO
+    const size_t sm = 0;
     if (xpay == 0 && post == 0) launch_pdl_smem(dslash_kernel<FMT, 0, 0>, grid, block, sm, s, a);
     else if (xpay == 0 && post == 1) launch_pdl_smem(dslash_kernel<FMT, 0, 1>, grid, block, sm, s, a);
     else if (xpay == 1 && post == 0) launch_pdl_smem(dslash_kernel<FMT, 1, 0>, grid, block, sm, s, a);
@@ -612,13 +532,6 @@ Tile make_tile(const Geom &g, int max_sites, int max_x)
         t.sh[0]++;
         vol *= 2;
     }
-#ifdef COLA_MRHS_TILE_LINEAR   // tuning experiment: fill y completely, then z, then t (a contiguous run of sites)
-    for (int k = 1; k < 4; k++)
-        while (vol * 2 <= max_sites && ext[k] % (1 << (t.sh[k] + 1)) == 0) {
-            t.sh[k]++;
-            vol *= 2;
-        }
-#endif
     for (bool grown = true; grown && vol * 2 <= max_sites;) {
         grown = false;
         for (int k = 1; k < 4 && vol * 2 <= max_sites; k++) {

@@ -109,3 +109,34 @@ def test_batched_bicgstab_matches_the_oracle_and_the_sequential_solver(mixed):
     xx, inf2 = c.cg_solve_mrhs(torch.stack(srcs[:3]).cuda(), tol=1e-10, mixed=mixed, method="bicgstab", max_iter=3)
     assert all(i["iters"] == 3 and not i["converged"] and 0 < i["true_residual"] < 1 for i in inf2)
     c.close()
+
+
+@pytest.mark.parametrize("mixed", [0, 1])
+def test_exact_convergence_at_the_half_step_is_not_a_breakdown(mixed):
+    """Unit links (A = 1), periodic boundaries, source psi(x) = (-1)^(x+y) chi: the hops in x and y cancel those in z and t,
+    D psi = 0 exactly in floating point, so S psi_e = psi_e, alpha = 1, s = r - alpha v = 0 and t = S s = 0 in the first pass.
+    omega = <t, s> / <t, t> is 0/0 there; the solver must finish with x = x + alpha p (= b) instead of reporting NaN.  The
+    same source in a batch must not disturb its neighbours."""
+    from paper_2302_00850_b200 import binding
+
+    dims, kappa, bc = (4, 4, 4, 8), 0.1, (1, 1, 1, 1)      # kappa below the free-field critical value 1/8: M is regular
+    U = inputs.links_unit(dims)
+    c = binding.Cola(dims, kappa, 1.0, bc=bc)
+    c.gauge_upload(U)
+    lx, ly, lz, lt = dims
+    sign = (-1.0) ** (np.arange(lx)[None, None, None, :] + np.arange(ly)[None, None, :, None]) * np.ones((lt, lz, 1, 1))
+    chi = (np.arange(12).reshape(4, 3) - 5.0) + 1j * (np.arange(12).reshape(4, 3) % 4)
+    b = torch.from_numpy(sign[..., None, None] * chi).to(torch.complex128)
+    Un = U.numpy()
+    A = oracle.clover(dims, Un, kappa, 1.0)
+    assert np.abs(oracle.M(dims, bc, Un, A, kappa, b.numpy()) - b.numpy()).max() == 0.0     # M b = b: the solution is b
+    x, info = c.cg_solve(b.cuda(), tol=1e-10, even_odd=True, mixed=mixed, method="bicgstab")
+    assert info["converged"] and info["iters"] == 1 and info["true_residual"] == 0.0, info
+    assert torch.equal(x.cpu(), b)
+    if mixed:
+        g = inputs.source_gaussian(dims, 9)
+        xs, infos = c.cg_solve_mrhs(torch.stack([g, b, 2 * g]).cuda(), tol=1e-10, mixed=1, method="bicgstab")
+        assert all(i["converged"] and i["true_residual"] <= 1.05e-10 for i in infos), infos
+        assert torch.equal(xs[1].cpu(), b) and infos[1]["iters"] == 1
+        assert rel(xs[2].cpu().numpy(), 2 * xs[0].cpu().numpy()) < 1e-9
+    c.close()

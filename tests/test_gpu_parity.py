@@ -578,13 +578,8 @@ def test_smallest_pivot_is_reported_and_indefinite_blocks_are_refused(cola_mod):
     cb.close()
 
 
-def test_cuda_failures_surface_as_COLA_ECUDA(cola_mod):
-    """COLA_ECUDA (SURVEY 8(b) error cases).  (1) a device ordinal that does not exist; (2) in a child process, because
-    the fault poisons its CUDA context: a workspace that is freed behind the library's back -- the kernels fault, the
-    next synchronising call reports COLA_ECUDA with the CUDA message, and nothing hangs."""
-    import subprocess
-    import sys
-
+def test_a_missing_device_surfaces_as_COLA_ECUDA(cola_mod):
+    """COLA_ECUDA (SURVEY 8(b) error cases): a device ordinal that does not exist."""
     b = cola_mod
     import ctypes
     lib = ctypes.CDLL(b.lib_path())
@@ -598,6 +593,18 @@ def test_cuda_failures_surface_as_COLA_ECUDA(cola_mod):
     assert lib.cola_create(ctypes.byref(h), ctypes.byref(p)) == b.COLA_ECUDA and not h.value
     assert b"cudaSetDevice" in lib.cola_last_error(None)
     torch.cuda.set_device(0)
+
+
+@pytest.mark.faultinject
+def test_a_faulting_kernel_surfaces_as_COLA_ECUDA(cola_mod):
+    """COLA_ECUDA from a kernel fault, in a child process because the fault poisons its CUDA context: a workspace that is
+    freed behind the library's back -- the kernels fault, the next synchronising call reports COLA_ECUDA with the CUDA
+    message, and nothing hangs.  It raises an MMU fault on the GPU, so it is not part of the routine `-m gpu` run on a
+    shared pool: select it with `-m faultinject`."""
+    import subprocess
+    import sys
+
+    b = cola_mod
     child = r"""
 import ctypes, sys, torch
 sys.path.insert(0, %r)
